@@ -1,0 +1,650 @@
+// =====================================================================================
+// fmm_oracle.cpp  --  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, fp64 CPU restatement of the adaptive point-charge Laplace FMM of
+// arXiv 2511.15269 (jaxFMM), written from /root/reference/PAPER.md only.  It shares no
+// code, header, table or constant generator with the CUDA path under
+// paper_2511_15269_b200/csrc and is imported only by tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs.
+//
+// Every function cites the PAPER.md passage it follows.  Where the paper is silent,
+// garbled or ambiguous the reading of DESIGN.md ("Readings", T1-T7, L1-L5, E1-E7,
+// G1-G5, S1-S7) is used and named.  Nothing is blocked, fused or reordered beyond what
+// those passages state; OpenMP loops run over independent target boxes only, so the
+// arithmetic order inside every result is the same for any thread count.
+//
+// Parity pins (tests/test_oracle_*.py): regular/singular basis vs associated-Legendre
+// closed forms; grad vs finite differences; addition theorem; Wigner-d vs d^1, d(0),
+// orthogonality; rotations vs recomputation from rotated points; M2M/L2L exactness;
+// M2L convergence; tree brute force + PAPER.md:50 counts; list partition identity and
+// the theta=0.7637 cube pin; whole FMM vs O(N^2) direct sum.
+// "parity unpinned": none of the functions below (cross-level lists, Table I are not
+// implemented here).
+//
+// Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py)
+// Coefficient layout: K=(p+1)^2 doubles, index(n,m) = n*n + n + m, -n<=m<=n;
+// m>=0 <-> real part, m<0 <-> imaginary part.
+// =====================================================================================
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+inline int IDX(int n, int m) { return n * n + n + m; }
+inline int sgn(int m) { return m >= 0 ? 1 : -1; }  // sgn(0)=+1
+inline int iabs(int m) { return m < 0 ? -m : m; }
+
+double factorial(int n) {
+    double f = 1.0;
+    for (int i = 2; i <= n; ++i) f *= (double)i;
+    return f;
+}
+
+// integer power, 0^0 = 1
+double ipow(double b, int e) {
+    double r = 1.0;
+    for (int i = 0; i < e; ++i) r *= b;
+    return r;
+}
+
+// -------------------------------------------------------------------------------------
+// App. A.1: real regular basis R^_n^m by recursion.
+// -------------------------------------------------------------------------------------
+void regular_basis(int p, double x, double y, double z, double* R) {
+    const double r2 = x * x + y * y + z * z;
+    R[IDX(0, 0)] = 1.0;
+    if (p >= 1) {
+        R[IDX(1, 1)] = x / 2.0;
+        R[IDX(1, -1)] = -y / 2.0;
+    }
+    for (int n = 2; n <= p; ++n) {
+        R[IDX(n, n)] = (x * R[IDX(n - 1, n - 1)] + y * R[IDX(n - 1, 1 - n)]) / (2.0 * n);
+        R[IDX(n, -n)] = (x * R[IDX(n - 1, 1 - n)] - y * R[IDX(n - 1, n - 1)]) / (2.0 * n);
+    }
+    for (int n = 0; n <= p - 1; ++n) {
+        R[IDX(n + 1, n)] = z * R[IDX(n, n)];
+        R[IDX(n + 1, -n)] = z * R[IDX(n, -n)];
+    }
+    for (int n = 2; n <= p; ++n)
+        for (int m = 2 - n; m <= n - 2; ++m)
+            R[IDX(n, m)] = ((2.0 * n - 1.0) * z * R[IDX(n - 1, m)] - r2 * R[IDX(n - 2, m)]) /
+                           (double)((n - iabs(m)) * (n + iabs(m)));
+}
+
+// -------------------------------------------------------------------------------------
+// App. A.2: real singular basis S^_n^m by recursion.
+// -------------------------------------------------------------------------------------
+void singular_basis(int p, double x, double y, double z, double* S) {
+    const double r2 = x * x + y * y + z * z;
+    const double r = std::sqrt(r2);
+    S[IDX(0, 0)] = 1.0 / r;
+    if (p >= 1) {
+        S[IDX(1, 1)] = x / (r2 * r);
+        S[IDX(1, -1)] = y / (r2 * r);
+    }
+    for (int n = 2; n <= p; ++n) {
+        S[IDX(n, n)] = (2.0 * n - 1.0) * (x * S[IDX(n - 1, n - 1)] - y * S[IDX(n - 1, 1 - n)]) / r2;
+        S[IDX(n, -n)] = (2.0 * n - 1.0) * (x * S[IDX(n - 1, 1 - n)] + y * S[IDX(n - 1, n - 1)]) / r2;
+    }
+    for (int n = 0; n <= p - 1; ++n) {
+        S[IDX(n + 1, n)] = (2.0 * n + 1.0) * z * S[IDX(n, n)] / r2;
+        S[IDX(n + 1, -n)] = (2.0 * n + 1.0) * z * S[IDX(n, -n)] / r2;
+    }
+    for (int n = 2; n <= p; ++n)
+        for (int m = 2 - n; m <= n - 2; ++m)
+            S[IDX(n, m)] = ((2.0 * n - 1.0) * z * S[IDX(n - 1, m)] -
+                            (double)((n - 1 - m) * (n - 1 + m)) * S[IDX(n - 2, m)]) / r2;
+}
+
+// -------------------------------------------------------------------------------------
+// App. A.3: gradient of the regular basis; G[3*idx + {0,1,2}].
+// Reading G1: PAPER.md:419 is printed with a leading minus; it is the derivative of
+// PAPER.md:368 and therefore carries NO minus (pinned by finite differences).
+// R must hold regular_basis(p, x, y, z).
+// -------------------------------------------------------------------------------------
+void regular_grad(int p, double x, double y, double z, const double* R, double* G) {
+    const double r2 = x * x + y * y + z * z;
+    const double rv[3] = {x, y, z};
+    for (int c = 0; c < 3; ++c) G[3 * IDX(0, 0) + c] = 0.0;
+    if (p >= 1) {
+        for (int c = 0; c < 3; ++c) { G[3 * IDX(1, 1) + c] = 0.0; G[3 * IDX(1, -1) + c] = 0.0; }
+        G[3 * IDX(1, 1) + 0] = 0.5;
+        G[3 * IDX(1, -1) + 1] = -0.5;
+    }
+    for (int n = 2; n <= p; ++n) {  // PAPER.md:419-421 (G1)
+        for (int c = 0; c < 3; ++c) {
+            const double ex = (c == 0) ? 1.0 : 0.0, ey = (c == 1) ? 1.0 : 0.0;
+            G[3 * IDX(n, n) + c] = (x * G[3 * IDX(n - 1, n - 1) + c] + y * G[3 * IDX(n - 1, 1 - n) + c] +
+                                    R[IDX(n - 1, n - 1)] * ex + R[IDX(n - 1, 1 - n)] * ey) / (2.0 * n);
+            G[3 * IDX(n, -n) + c] = (x * G[3 * IDX(n - 1, 1 - n) + c] - y * G[3 * IDX(n - 1, n - 1) + c] +
+                                     R[IDX(n - 1, 1 - n)] * ex - R[IDX(n - 1, n - 1)] * ey) / (2.0 * n);
+        }
+    }
+    for (int n = 0; n <= p - 1; ++n) {
+        for (int c = 0; c < 3; ++c) {
+            const double ez = (c == 2) ? 1.0 : 0.0;
+            G[3 * IDX(n + 1, n) + c] = z * G[3 * IDX(n, n) + c] + R[IDX(n, n)] * ez;
+            G[3 * IDX(n + 1, -n) + c] = z * G[3 * IDX(n, -n) + c] + R[IDX(n, -n)] * ez;
+        }
+    }
+    for (int n = 2; n <= p; ++n)
+        for (int m = 2 - n; m <= n - 2; ++m)
+            for (int c = 0; c < 3; ++c) {
+                const double ez = (c == 2) ? 1.0 : 0.0;
+                G[3 * IDX(n, m) + c] = ((2.0 * n - 1.0) * (z * G[3 * IDX(n - 1, m) + c] + R[IDX(n - 1, m)] * ez) -
+                                        r2 * G[3 * IDX(n - 2, m) + c] - 2.0 * R[IDX(n - 2, m)] * rv[c]) /
+                                       (double)(n * n - m * m);
+            }
+}
+
+// -------------------------------------------------------------------------------------
+// Wigner small-d, d^j_{m',m}(beta).  The paper delegates to [14];
+// reading S6: the textbook explicit sum
+//   d^j_{m'm} = sum_s (-1)^{m'-m+s} sqrt((j+m)!(j-m)!(j+m')!(j-m')!) /
+//               ((j+m-s)! s! (m'-m+s)! (j-m'-s)!) cos(b/2)^{2j+m-m'-2s} sin(b/2)^{m'-m+2s}
+// over all s with non-negative factorial arguments.
+// -------------------------------------------------------------------------------------
+double wigner_d(int j, int mp, int m, double beta) {
+    const double cb = std::cos(0.5 * beta), sb = std::sin(0.5 * beta);
+    const double pref = std::sqrt(factorial(j + m) * factorial(j - m) * factorial(j + mp) * factorial(j - mp));
+    const int smin = std::max(0, m - mp), smax = std::min(j + m, j - mp);
+    double sum = 0.0;
+    for (int s = smin; s <= smax; ++s) {
+        const double den = factorial(j + m - s) * factorial(s) * factorial(mp - m + s) * factorial(j - mp - s);
+        const double sign = ((mp - m + s) % 2 == 0) ? 1.0 : -1.0;
+        sum += sign * pref / den * ipow(cb, 2 * j + m - mp - 2 * s) * ipow(sb, mp - m + 2 * s);
+    }
+    return sum;
+}
+
+// -------------------------------------------------------------------------------------
+// App. B.1: azimuthal rotation by dphi, for all m including negative
+// (E-rules: C' = C cos(m dphi) - C^{-m} sin(m dphi);  D' = D cos + D^{-m} sin).
+// -------------------------------------------------------------------------------------
+void rot_azimuthal(int p, int local_type, const double* in, double dphi, double* out) {
+    for (int n = 0; n <= p; ++n)
+        for (int m = -n; m <= n; ++m) {
+            const double c = std::cos(m * dphi), s = std::sin(m * dphi);
+            out[IDX(n, m)] = local_type ? in[IDX(n, m)] * c + in[IDX(n, -m)] * s
+                                        : in[IDX(n, m)] * c - in[IDX(n, -m)] * s;
+        }
+}
+
+// -------------------------------------------------------------------------------------
+// App. B.2: polar rotation by dtheta.  Reading G2: the cases of W are
+// "k>0", "k=0 and m>=0", "k=0 and m<0 -> 0"; d_{n,k}^{|m|} = d^n_{m'=|m|, m=k}.
+//   C'_n^m = sum_{k=0}^n C_n^{sgn(m)k} N W,   D'_n^m = sum_k D_n^{sgn(m)k} W / N,
+//   N = sqrt((n-k)!(n+k)! / ((n-|m|)!(n+|m|)!)).
+// -------------------------------------------------------------------------------------
+void rot_polar(int p, int local_type, const double* in, double dtheta, double* out) {
+    for (int n = 0; n <= p; ++n)
+        for (int m = -n; m <= n; ++m) {
+            const int am = iabs(m);
+            double acc = 0.0;
+            for (int k = 0; k <= n; ++k) {
+                double W;
+                if (k > 0) W = wigner_d(n, am, k, dtheta) + sgn(m) * ((k % 2 == 0) ? 1.0 : -1.0) * wigner_d(n, am, -k, dtheta);
+                else if (m >= 0) W = wigner_d(n, am, 0, dtheta);
+                else continue;  // k=0, m<0: term absent
+                const double N = std::sqrt(factorial(n - k) * factorial(n + k) / (factorial(n - am) * factorial(n + am)));
+                const double v = in[IDX(n, sgn(m) * k)];
+                acc += local_type ? v * W / N : v * N * W;
+            }
+            out[IDX(n, m)] = acc;
+        }
+}
+
+// -------------------------------------------------------------------------------------
+// App. B.3: shifts along +z by r > 0 (reading G3: b = old centre -
+// new centre, brought onto +z by the preceding rotations).
+// -------------------------------------------------------------------------------------
+void shift_m2m(int p, const double* C, double r, double* out) {
+    for (int n = 0; n <= p; ++n)
+        for (int m = -n; m <= n; ++m) {
+            double acc = 0.0;
+            for (int k = iabs(m); k <= n; ++k) acc += ipow(r, n - k) / factorial(n - k) * C[IDX(k, m)];
+            out[IDX(n, m)] = acc;
+        }
+}
+void shift_m2l(int p, const double* C, double r, double* out) {
+    for (int n = 0; n <= p; ++n)
+        for (int m = -n; m <= n; ++m) {
+            double acc = 0.0;
+            for (int k = iabs(m); k <= p; ++k) {
+                const double sign = (((k + m) % 2 + 2) % 2 == 0) ? 1.0 : -1.0;
+                acc += sgn(m) * sign * factorial(n + k) / ipow(r, n + k + 1) * C[IDX(k, m)];
+            }
+            out[IDX(n, m)] = acc;
+        }
+}
+void shift_l2l(int p, const double* D, double r, double* out) {
+    for (int n = 0; n <= p; ++n)
+        for (int m = -n; m <= n; ++m) {
+            double acc = 0.0;
+            for (int k = n; k <= p; ++k) acc += ipow(-r, k - n) / factorial(k - n) * D[IDX(k, m)];
+            out[IDX(n, m)] = acc;
+        }
+}
+
+// -------------------------------------------------------------------------------------
+// PAPER.md:154 "rotate -> transform -> rotate back" (rule T_X of DESIGN.md).
+// b = old expansion centre - new expansion centre (G3).  (r,theta,phi) of b; forward:
+// azimuthal by phi, polar by theta (b now on +z); z-shift of length r; inverse: polar
+// by -theta, azimuthal by -phi.  kind: 0=M2M, 1=M2L, 2=L2L.  phi:=0 when b_x=b_y=0 (S7).
+// -------------------------------------------------------------------------------------
+void translate(int kind, int p, const double* in, const double b[3], double* out) {
+    const int K = (p + 1) * (p + 1);
+    const double r = std::sqrt(b[0] * b[0] + b[1] * b[1] + b[2] * b[2]);
+    std::vector<double> t1(K), t2(K);
+    if (r == 0.0) {  // degenerate (single-child chains with identical bbox): identity for M2M/L2L
+        std::memcpy(out, in, sizeof(double) * K);
+        return;
+    }
+    double ct = b[2] / r;
+    if (ct > 1.0) ct = 1.0;
+    if (ct < -1.0) ct = -1.0;
+    const double theta = std::acos(ct);
+    const double phi = (b[0] == 0.0 && b[1] == 0.0) ? 0.0 : std::atan2(b[1], b[0]);
+    const int in_local = (kind == 2) ? 1 : 0;
+    const int out_local = (kind == 0) ? 0 : 1;
+    rot_azimuthal(p, in_local, in, phi, t1.data());
+    rot_polar(p, in_local, t1.data(), theta, t2.data());
+    if (kind == 0) shift_m2m(p, t2.data(), r, t1.data());
+    else if (kind == 1) shift_m2l(p, t2.data(), r, t1.data());
+    else shift_l2l(p, t2.data(), r, t1.data());
+    rot_polar(p, out_local, t1.data(), -theta, t2.data());
+    rot_azimuthal(p, out_local, t2.data(), -phi, out);
+}
+
+// -------------------------------------------------------------------------------------
+// Hierarchy, PAPER.md:40-43 and Listing 2; rules T1-T7 of DESIGN.md.
+// -------------------------------------------------------------------------------------
+int tree_depth(int64_t N, int N_max, int s) {  // T1: smallest l with ceil(N/2^{sl}) <= N_max
+    for (int L = 0;; ++L) {
+        int64_t q = N;  // ceil(ceil(a/2)/2) = ceil(a/4): repeated ceiling-halving is ceil(N/2^{sL})
+        for (int i = 0; i < s * L; ++i) q = (q + 1) / 2;
+        if (q <= N_max) return L;
+    }
+}
+
+struct Tree {
+    int64_t N = 0;
+    int s = 0, L = 0;
+    std::vector<int64_t> perm;                       // tree order -> original index (T4)
+    std::vector<int64_t> level_off;                  // global id offset of each level (L+2 entries)
+    std::vector<int64_t> box_start, box_count;       // per global box id, range in tree order
+    std::vector<double> lo, hi, ctr, rad;            // per global box: 3,3,3,1 (T6); empty boxes: NaN-free zeros, count 0
+};
+
+void split_rec(const double* pos, std::vector<int64_t>& ids, int d, int dmax, const std::vector<int64_t>& nd,
+               std::vector<std::vector<int64_t>>& leaves) {
+    if (d == dmax) {
+        std::sort(ids.begin(), ids.end());  // T4 / PAPER.md:220
+        leaves.push_back(ids);
+        return;
+    }
+    const int64_t c = (int64_t)ids.size();
+    int axis = 0;
+    if (c > 0) {  // T3: tight bbox, extent in fp64, longest axis, ties -> lowest axis index
+        double e[3];
+        for (int a = 0; a < 3; ++a) {
+            double mn = pos[3 * ids[0] + a], mx = mn;
+            for (int64_t i : ids) { mn = std::min(mn, pos[3 * i + a]); mx = std::max(mx, pos[3 * i + a]); }
+            e[a] = mx - mn;
+        }
+        if (e[1] > e[axis]) axis = 1;
+        if (e[2] > e[axis]) axis = 2;
+    }
+    // order by (coordinate on axis, original index)  (S4)
+    std::sort(ids.begin(), ids.end(), [&](int64_t a, int64_t b) {
+        const double xa = pos[3 * a + axis], xb = pos[3 * b + axis];
+        if (xa < xb) return true;
+        if (xb < xa) return false;
+        return a < b;
+    });
+    // upper child gets the last floor(n_d/2), lower child the rest (T3; Listing 2)
+    int64_t n_up = nd[d] / 2;
+    if (n_up > c) n_up = c;
+    std::vector<int64_t> lower(ids.begin(), ids.end() - n_up), upper(ids.end() - n_up, ids.end());
+    split_rec(pos, lower, d + 1, dmax, nd, leaves);
+    split_rec(pos, upper, d + 1, dmax, nd, leaves);
+}
+
+void build_tree(const double* pos, int64_t N, int N_max, int s, Tree& T) {
+    T.N = N; T.s = s; T.L = tree_depth(N, N_max, s);
+    const int dmax = s * T.L;
+    std::vector<int64_t> nd(dmax + 1);
+    nd[0] = N;
+    for (int d = 0; d < dmax; ++d) nd[d + 1] = (nd[d] + 1) / 2;  // padded row length of Listing 2
+    std::vector<int64_t> ids(N);
+    for (int64_t i = 0; i < N; ++i) ids[i] = i;
+    std::vector<std::vector<int64_t>> leaves;
+    split_rec(pos, ids, 0, dmax, nd, leaves);
+    T.perm.clear();
+    const int64_t n_leaves = (int64_t)1 << dmax;
+    std::vector<int64_t> leaf_start(n_leaves + 1, 0);
+    for (int64_t b = 0; b < n_leaves; ++b) {
+        for (int64_t i : leaves[b]) T.perm.push_back(i);
+        leaf_start[b + 1] = (int64_t)T.perm.size();
+    }
+    T.level_off.assign(T.L + 2, 0);
+    for (int l = 0; l <= T.L; ++l) T.level_off[l + 1] = T.level_off[l] + ((int64_t)1 << (s * l));
+    const int64_t nb = T.level_off[T.L + 1];
+    T.box_start.assign(nb, 0); T.box_count.assign(nb, 0);
+    T.lo.assign(3 * nb, 0.0); T.hi.assign(3 * nb, 0.0); T.ctr.assign(3 * nb, 0.0); T.rad.assign(nb, 0.0);
+    for (int l = 0; l <= T.L; ++l) {
+        const int64_t nbl = (int64_t)1 << (s * l);
+        const int64_t leaves_per_box = n_leaves / nbl;  // T2: box b at level l = leaves [b*lpb, (b+1)*lpb)
+        for (int64_t b = 0; b < nbl; ++b) {
+            const int64_t g = T.level_off[l] + b;
+            const int64_t st = leaf_start[b * leaves_per_box], en = leaf_start[(b + 1) * leaves_per_box];
+            T.box_start[g] = st; T.box_count[g] = en - st;
+            if (en == st) continue;  // T5
+            for (int a = 0; a < 3; ++a) {
+                double mn = pos[3 * T.perm[st] + a], mx = mn;
+                for (int64_t k = st; k < en; ++k) { mn = std::min(mn, pos[3 * T.perm[k] + a]); mx = std::max(mx, pos[3 * T.perm[k] + a]); }
+                T.lo[3 * g + a] = mn; T.hi[3 * g + a] = mx;
+                T.ctr[3 * g + a] = 0.5 * (mn + mx);  // T6/T7
+            }
+            const double dx = T.hi[3 * g] - T.lo[3 * g], dy = T.hi[3 * g + 1] - T.lo[3 * g + 1], dz = T.hi[3 * g + 2] - T.lo[3 * g + 2];
+            T.rad[g] = 0.5 * std::sqrt((dx * dx + dy * dy) + dz * dz);  // T6, summed x->y->z
+        }
+    }
+}
+
+// eq. (4), rule L1: R + theta r < theta d, strict.
+bool admissible(const Tree& T, int64_t ga, int64_t gb, double theta) {
+    const double ra = T.rad[ga], rb = T.rad[gb];
+    const double R = std::max(ra, rb), r = std::min(ra, rb);
+    const double dx = T.ctr[3 * ga] - T.ctr[3 * gb], dy = T.ctr[3 * ga + 1] - T.ctr[3 * gb + 1], dz = T.ctr[3 * ga + 2] - T.ctr[3 * gb + 2];
+    const double d = std::sqrt((dx * dx + dy * dy) + dz * dz);
+    return R + theta * r < theta * d;
+}
+
+struct Lists {
+    // CSR by target global box id (L4); sources are global ids, ascending within a row.
+    std::vector<int64_t> weak_off; std::vector<int64_t> weak_src;
+    // CSR by target leaf (index within leaf level); sources are leaf indices, ascending.
+    std::vector<int64_t> strong_off; std::vector<int64_t> strong_src;
+};
+
+// PAPER.md:72-74, rules L2-L5.
+void build_lists(const Tree& T, double theta, Lists& Ls) {
+    const int s = T.s, L = T.L;
+    const int64_t nch = (int64_t)1 << s;
+    const int64_t nb = T.level_off[L + 1];
+    std::vector<std::vector<int64_t>> weak_rows(nb);
+    const int64_t n_leaves = (int64_t)1 << (s * L);
+    std::vector<std::vector<int64_t>> strong_rows(n_leaves);
+    std::vector<std::pair<int64_t, int64_t>> cand, fail;
+    cand.push_back({0, 0});  // (root, root), level-local indices
+    for (int l = 0; l <= L; ++l) {
+        fail.clear();
+        for (auto& pr : cand) {
+            const int64_t ga = T.level_off[l] + pr.first, gb = T.level_off[l] + pr.second;
+            if (admissible(T, ga, gb, theta)) weak_rows[ga].push_back(gb);
+            else fail.push_back(pr);
+        }
+        if (l == L) break;
+        cand.clear();
+        for (auto& pr : fail)
+            for (int64_t i = 0; i < nch; ++i)
+                for (int64_t j = 0; j < nch; ++j) {
+                    const int64_t a = pr.first * nch + i, b = pr.second * nch + j;
+                    if (T.box_count[T.level_off[l + 1] + a] == 0 || T.box_count[T.level_off[l + 1] + b] == 0) continue;  // T5
+                    cand.push_back({a, b});
+                }
+    }
+    for (auto& pr : fail) strong_rows[pr.first].push_back(pr.second);  // L3, includes (t,t)
+    Ls.weak_off.assign(nb + 1, 0); Ls.weak_src.clear();
+    for (int64_t g = 0; g < nb; ++g) {
+        std::sort(weak_rows[g].begin(), weak_rows[g].end());
+        for (int64_t v : weak_rows[g]) Ls.weak_src.push_back(v);
+        Ls.weak_off[g + 1] = (int64_t)Ls.weak_src.size();
+    }
+    Ls.strong_off.assign(n_leaves + 1, 0); Ls.strong_src.clear();
+    for (int64_t t = 0; t < n_leaves; ++t) {
+        std::sort(strong_rows[t].begin(), strong_rows[t].end());
+        for (int64_t v : strong_rows[t]) Ls.strong_src.push_back(v);
+        Ls.strong_off[t + 1] = (int64_t)Ls.strong_src.size();
+    }
+}
+
+struct Plan {
+    int p = 0; double theta = 0.77;
+    std::vector<double> pos;  // copy of input positions (N x 3)
+    Tree T; Lists Ls;
+};
+
+// -------------------------------------------------------------------------------------
+// Evaluate, stage order PAPER.md:251; steps E1-E7 of DESIGN.md.  If leaf_mask != nullptr only
+// the leaves with mask != 0 get results (all other outputs are left untouched): local
+// expansions are then computed only for those leaves and their ancestors, with the
+// same arithmetic and order as the full run, so sampled outputs equal the full ones.
+// -------------------------------------------------------------------------------------
+void evaluate(const Plan& P, const double* q, const uint8_t* leaf_mask, double* pot, double* field) {
+    const Tree& T = P.T; const Lists& Ls = P.Ls;
+    const int p = P.p, K = (p + 1) * (p + 1), s = T.s, L = T.L;
+    const int64_t nb = T.level_off[L + 1], n_leaves = (int64_t)1 << (s * L), nch = (int64_t)1 << s;
+    const int64_t leaf0 = T.level_off[L];
+    const double* pos = P.pos.data();
+    std::vector<double> C((size_t)nb * K, 0.0), D((size_t)nb * K, 0.0);
+    std::vector<uint8_t> need(nb, leaf_mask ? 0 : 1);
+    if (leaf_mask) {
+        for (int64_t t = 0; t < n_leaves; ++t) if (leaf_mask[t]) need[leaf0 + t] = 1;
+        for (int l = L; l >= 1; --l)
+            for (int64_t b = 0; b < ((int64_t)1 << (s * l)); ++b)
+                if (need[T.level_off[l] + b]) need[T.level_off[l - 1] + b / nch] = 1;
+    }
+    // E1: P2M at leaves, eq. (13)
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < n_leaves; ++t) {
+        const int64_t g = leaf0 + t;
+        std::vector<double> R(K);
+        for (int64_t k = T.box_start[g]; k < T.box_start[g] + T.box_count[g]; ++k) {
+            const int64_t i = T.perm[k];
+            regular_basis(p, pos[3 * i] - T.ctr[3 * g], pos[3 * i + 1] - T.ctr[3 * g + 1], pos[3 * i + 2] - T.ctr[3 * g + 2], R.data());
+            for (int c = 0; c < K; ++c) C[(size_t)g * K + c] += q[i] * R[c];
+        }
+    }
+    // E2: M2M, l = L..1, children in ascending order; b = child centre - parent centre
+    for (int l = L; l >= 1; --l) {
+        const int64_t nbp = (int64_t)1 << (s * (l - 1));
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t bp = 0; bp < nbp; ++bp) {
+            const int64_t gp = T.level_off[l - 1] + bp;
+            std::vector<double> tmp(K);
+            for (int64_t j = 0; j < nch; ++j) {
+                const int64_t gc = T.level_off[l] + bp * nch + j;
+                if (T.box_count[gc] == 0) continue;
+                const double b[3] = {T.ctr[3 * gc] - T.ctr[3 * gp], T.ctr[3 * gc + 1] - T.ctr[3 * gp + 1], T.ctr[3 * gc + 2] - T.ctr[3 * gp + 2]};
+                translate(0, p, &C[(size_t)gc * K], b, tmp.data());
+                for (int c = 0; c < K; ++c) C[(size_t)gp * K + c] += tmp[c];
+            }
+        }
+    }
+    // E3: M2L over the weak list, all levels; b = source centre - target centre
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t gt = 0; gt < nb; ++gt) {
+        if (!need[gt]) continue;
+        std::vector<double> tmp(K);
+        for (int64_t e = Ls.weak_off[gt]; e < Ls.weak_off[gt + 1]; ++e) {
+            const int64_t gs = Ls.weak_src[e];
+            const double b[3] = {T.ctr[3 * gs] - T.ctr[3 * gt], T.ctr[3 * gs + 1] - T.ctr[3 * gt + 1], T.ctr[3 * gs + 2] - T.ctr[3 * gt + 2]};
+            translate(1, p, &C[(size_t)gs * K], b, tmp.data());
+            for (int c = 0; c < K; ++c) D[(size_t)gt * K + c] += tmp[c];
+        }
+    }
+    // E4: L2L, l = 1..L; b = parent centre - child centre
+    for (int l = 1; l <= L; ++l) {
+        const int64_t nbl = (int64_t)1 << (s * l);
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t bc = 0; bc < nbl; ++bc) {
+            const int64_t gc = T.level_off[l] + bc, gp = T.level_off[l - 1] + bc / nch;
+            if (!need[gc] || T.box_count[gc] == 0) continue;
+            std::vector<double> tmp(K);
+            const double b[3] = {T.ctr[3 * gp] - T.ctr[3 * gc], T.ctr[3 * gp + 1] - T.ctr[3 * gc + 1], T.ctr[3 * gp + 2] - T.ctr[3 * gc + 2]};
+            translate(2, p, &D[(size_t)gp * K], b, tmp.data());
+            for (int c = 0; c < K; ++c) D[(size_t)gc * K + c] += tmp[c];
+        }
+    }
+    // E5 L2P (eq. 14, gradient App. A.3), E6 P2P, E7 scaling and scatter
+    const double inv4pi = 1.0 / (4.0 * M_PI);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t t = 0; t < n_leaves; ++t) {
+        if (leaf_mask && !leaf_mask[t]) continue;
+        const int64_t g = leaf0 + t;
+        std::vector<double> R(K), G(3 * K);
+        for (int64_t k = T.box_start[g]; k < T.box_start[g] + T.box_count[g]; ++k) {
+            const int64_t i = T.perm[k];
+            const double x = pos[3 * i] - T.ctr[3 * g], y = pos[3 * i + 1] - T.ctr[3 * g + 1], z = pos[3 * i + 2] - T.ctr[3 * g + 2];
+            regular_basis(p, x, y, z, R.data());
+            regular_grad(p, x, y, z, R.data(), G.data());
+            double phi_far = 0.0, gfar[3] = {0, 0, 0};
+            for (int n = 0; n <= p; ++n)
+                for (int m = -n; m <= n; ++m) {
+                    const double w = ((m == 0) ? 1.0 : 2.0) * sgn(m) * D[(size_t)g * K + IDX(n, m)];
+                    phi_far += w * R[IDX(n, m)];
+                    for (int c = 0; c < 3; ++c) gfar[c] += w * G[3 * IDX(n, m) + c];
+                }
+            double phi_near = 0.0, gnear[3] = {0, 0, 0};
+            for (int64_t e = Ls.strong_off[t]; e < Ls.strong_off[t + 1]; ++e) {
+                const int64_t gs = leaf0 + Ls.strong_src[e];
+                for (int64_t kk = T.box_start[gs]; kk < T.box_start[gs] + T.box_count[gs]; ++kk) {
+                    const int64_t j = T.perm[kk];
+                    if (j == i) continue;  // S3
+                    const double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 == 0.0) continue;  // S3: coincident points contribute nothing
+                    const double r = std::sqrt(r2);
+                    phi_near += q[j] / r;
+                    const double f = q[j] / (r2 * r);
+                    gnear[0] -= f * dx; gnear[1] -= f * dy; gnear[2] -= f * dz;
+                }
+            }
+            if (pot) pot[i] = -(phi_far + phi_near) * inv4pi;  // eqs. (2),(9),(14)
+            if (field) for (int c = 0; c < 3; ++c) field[3 * i + c] = (gfar[c] + gnear[c]) * inv4pi;  // field = -grad u (S2)
+        }
+    }
+}
+
+}  // namespace
+
+// =====================================================================================
+// C interface for ctypes (tests, smoke, bench cpu_baseline).  All pointers are host.
+// =====================================================================================
+extern "C" {
+
+void orc_regular_basis(int p, double x, double y, double z, double* R) { regular_basis(p, x, y, z, R); }
+void orc_singular_basis(int p, double x, double y, double z, double* S) { singular_basis(p, x, y, z, S); }
+void orc_regular_grad(int p, double x, double y, double z, double* G) {
+    std::vector<double> R((p + 1) * (p + 1));
+    regular_basis(p, x, y, z, R.data());
+    regular_grad(p, x, y, z, R.data(), G);
+}
+double orc_wigner_d(int j, int mp, int m, double beta) { return wigner_d(j, mp, m, beta); }
+void orc_rot_azimuthal(int p, int local_type, const double* in, double dphi, double* out) { rot_azimuthal(p, local_type, in, dphi, out); }
+void orc_rot_polar(int p, int local_type, const double* in, double dtheta, double* out) { rot_polar(p, local_type, in, dtheta, out); }
+void orc_shift(int kind, int p, const double* in, double r, double* out) {
+    if (kind == 0) shift_m2m(p, in, r, out); else if (kind == 1) shift_m2l(p, in, r, out); else shift_l2l(p, in, r, out);
+}
+void orc_translate(int kind, int p, const double* in, const double* b, double* out) { translate(kind, p, in, b, out); }
+int orc_tree_depth(int64_t N, int N_max, int s) { return tree_depth(N, N_max, s); }
+
+void* orc_plan_create(const double* pos, int64_t N, int p, int N_max, int s, double theta) {
+    Plan* P = new Plan();
+    P->p = p; P->theta = theta;
+    P->pos.assign(pos, pos + 3 * N);
+    build_tree(P->pos.data(), N, N_max, s, P->T);
+    build_lists(P->T, theta, P->Ls);
+    return P;
+}
+void orc_plan_destroy(void* h) { delete (Plan*)h; }
+void orc_plan_info(void* h, int* L, int64_t* n_boxes, int64_t* n_leaves, int64_t* n_weak, int64_t* n_strong, int64_t* n_p2p_pairs) {
+    Plan* P = (Plan*)h;
+    *L = P->T.L; *n_boxes = P->T.level_off[P->T.L + 1]; *n_leaves = (int64_t)1 << (P->T.s * P->T.L);
+    *n_weak = (int64_t)P->Ls.weak_src.size(); *n_strong = (int64_t)P->Ls.strong_src.size();
+    int64_t pairs = 0;
+    const int64_t leaf0 = P->T.level_off[P->T.L];
+    for (int64_t t = 0; t < *n_leaves; ++t)
+        for (int64_t e = P->Ls.strong_off[t]; e < P->Ls.strong_off[t + 1]; ++e)
+            pairs += P->T.box_count[leaf0 + t] * P->T.box_count[leaf0 + P->Ls.strong_src[e]];
+    *n_p2p_pairs = pairs;
+}
+void orc_plan_copy_tree(void* h, int64_t* perm, int64_t* box_start, int64_t* box_count, double* lo, double* hi, double* ctr, double* rad) {
+    Plan* P = (Plan*)h; const Tree& T = P->T;
+    const int64_t nb = T.level_off[T.L + 1];
+    if (perm) std::copy(T.perm.begin(), T.perm.end(), perm);
+    if (box_start) std::copy(T.box_start.begin(), T.box_start.end(), box_start);
+    if (box_count) std::copy(T.box_count.begin(), T.box_count.end(), box_count);
+    if (lo) std::copy(T.lo.begin(), T.lo.begin() + 3 * nb, lo);
+    if (hi) std::copy(T.hi.begin(), T.hi.begin() + 3 * nb, hi);
+    if (ctr) std::copy(T.ctr.begin(), T.ctr.begin() + 3 * nb, ctr);
+    if (rad) std::copy(T.rad.begin(), T.rad.begin() + nb, rad);
+}
+void orc_plan_copy_lists(void* h, int64_t* weak_off, int64_t* weak_src, int64_t* strong_off, int64_t* strong_src) {
+    Plan* P = (Plan*)h; const Lists& Ls = P->Ls;
+    if (weak_off) std::copy(Ls.weak_off.begin(), Ls.weak_off.end(), weak_off);
+    if (weak_src) std::copy(Ls.weak_src.begin(), Ls.weak_src.end(), weak_src);
+    if (strong_off) std::copy(Ls.strong_off.begin(), Ls.strong_off.end(), strong_off);
+    if (strong_src) std::copy(Ls.strong_src.begin(), Ls.strong_src.end(), strong_src);
+}
+// lists from hand-made geometry (pin PAPER.md:80): boxes given by ctr/rad, tree shape (s, L) complete
+void orc_lists_from_geometry(int s, int L, const double* ctr, const double* rad, double theta,
+                             int64_t* n_weak_per_box, int64_t* n_strong_per_leaf) {
+    Tree T; T.s = s; T.L = L;
+    T.level_off.assign(L + 2, 0);
+    for (int l = 0; l <= L; ++l) T.level_off[l + 1] = T.level_off[l] + ((int64_t)1 << (s * l));
+    const int64_t nb = T.level_off[L + 1];
+    T.ctr.assign(ctr, ctr + 3 * nb); T.rad.assign(rad, rad + nb);
+    T.box_count.assign(nb, 1); T.box_start.assign(nb, 0);
+    Lists Ls; build_lists(T, theta, Ls);
+    for (int64_t g = 0; g < nb; ++g) n_weak_per_box[g] = Ls.weak_off[g + 1] - Ls.weak_off[g];
+    const int64_t nl = (int64_t)1 << (s * L);
+    for (int64_t t = 0; t < nl; ++t) n_strong_per_leaf[t] = Ls.strong_off[t + 1] - Ls.strong_off[t];
+}
+void orc_evaluate(void* h, const double* q, const uint8_t* leaf_mask, double* pot, double* field) {
+    evaluate(*(Plan*)h, q, leaf_mask, pot, field);
+}
+// plain definition, eqs. (1)-(3) PAPER.md:19-28: u_i = -(1/4pi) sum_{j != i} q_j/|r_i - r_j|, field = -grad u;
+// evaluated at the targets listed in tgt (indices into pos), against all N sources.
+void orc_direct(const double* pos, const double* q, int64_t N, const int64_t* tgt, int64_t n_tgt, double* pot, double* field) {
+    const double inv4pi = 1.0 / (4.0 * M_PI);
+#pragma omp parallel for schedule(static)
+    for (int64_t a = 0; a < n_tgt; ++a) {
+        const int64_t i = tgt[a];
+        double ph = 0.0, g[3] = {0, 0, 0};
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            const double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 == 0.0) continue;
+            const double r = std::sqrt(r2);
+            ph += q[j] / r;
+            const double f = q[j] / (r2 * r);
+            g[0] -= f * dx; g[1] -= f * dy; g[2] -= f * dz;
+        }
+        if (pot) pot[a] = -ph * inv4pi;
+        if (field) for (int c = 0; c < 3; ++c) field[3 * a + c] = g[c] * inv4pi;
+    }
+}
+int orc_num_threads() {
+    int n = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp single
+        n = omp_get_num_threads();
+    }
+#endif
+    return n;
+}
+
+}  // extern "C"
