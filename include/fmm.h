@@ -1,0 +1,123 @@
+/* fmm.h -- C-ABI boundary of the B200-native adaptive Laplace FMM (arXiv 2511.15269, "jaxFMM").
+ *
+ * The paper's interface is two calls, gen_hierarchy(pts, p, theta, ...) -> hier and
+ * eval_potential(chrgs, **hier) (Listing 1), the hierarchy being reusable for new
+ * charges.  Here: fmm_plan_create builds the hierarchy and the interaction lists on
+ * the device, fmm_evaluate runs P2M -> M2M -> M2L -> L2L -> L2P + P2P (stage order PAPER.md:251).
+ *
+ * Result definition (eqs. (1)-(3)):
+ *     potential_i = -(1/4pi) * sum_{j != i} q_j / |r_i - r_j|        field_i = -grad potential (r_i)
+ * approximated by a p-th order FMM (eqs. (9)-(14)); pairs at zero distance
+ * contribute nothing.
+ *
+ * Conventions
+ *  - "DEVICE" pointers are CUDA device pointers of the current device; "HOST" pointers are ordinary
+ *    host memory.  The caller owns every buffer it passes; the plan copies what it needs and never
+ *    keeps caller pointers.  The plan owns all of its internal device memory.
+ *  - dtype selects the arithmetic AND the element type of positions/charges/outputs (float or double).
+ *    Geometric decisions (box centres, radii, admissibility) are always taken in IEEE fp64.
+ *  - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - fmm_plan_create and the fmm_plan_copy_* / fmm_plan_info calls synchronise the stream before
+ *    returning; fmm_evaluate only enqueues work on the stream (asynchronous).  Evaluations on one plan
+ *    must be serialised by stream order (the plan owns the coefficient scratch arrays).
+ *  - Outputs are in INPUT order.
+ *  - No exception or abort crosses this boundary: every failure is a status code, *out_plan is NULL on
+ *    failure, fmm_last_error() returns a thread-local message.
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns FMM_ERR_CUDA.
+ */
+#ifndef PAPER_2511_15269_FMM_H
+#define PAPER_2511_15269_FMM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fmm_plan fmm_plan; /* opaque */
+
+typedef enum {
+    FMM_OK = 0,
+    FMM_ERR_INVALID_ARG = 1, /* NULL pointer, N<1, p<0 or p>FMM_P_MAX, N_max<1, s<1, theta not in (0,1), non-finite position */
+    FMM_ERR_ALLOC = 2,       /* device or host allocation failed */
+    FMM_ERR_CUDA = 3,        /* any other CUDA runtime error (message in fmm_last_error) */
+    FMM_ERR_UNSUPPORTED = 4  /* cross_level != 0, or a tree too deep for 31-bit box ids */
+} fmm_status;
+
+typedef enum { FMM_F32 = 0, FMM_F64 = 1 } fmm_dtype;
+
+#define FMM_P_MAX 16
+
+/* Admissibility parameters of eq. (4):  R + theta*r < theta*d. */
+typedef struct {
+    double theta;    /* 0 < theta < 1; the paper's default is 0.77 */
+    int cross_level; /* 0 = same-level lists.  1 (level marching) is reserved. */
+} fmm_admissibility;
+
+/* Build hierarchy + lists for N charges (Listing 2; lists PAPER.md:72-74).
+ *   d_positions : DEVICE, N x 3 row-major (x,y,z), element type = dtype.  Read only during this call.
+ *   p           : expansion order, 0..FMM_P_MAX (eqs. (9),(11)).
+ *   N_max       : leaves hold at most N_max charges.   s : splits per level, 2^s children.
+ *   adm         : HOST pointer; NULL selects theta = 0.77, same-level lists.
+ * Tree depth L is the smallest l with ceil(N / 2^(s*l)) <= N_max.  Synchronises the stream. */
+fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max, int s,
+                           const fmm_admissibility* adm, fmm_dtype dtype, void* cuda_stream, fmm_plan** out_plan);
+
+/* Evaluate potential and/or field for new charges on an existing plan.
+ *   d_charges   : DEVICE, N, input order, dtype.
+ *   d_potential : DEVICE, N, input order, dtype; may be NULL.
+ *   d_field     : DEVICE, N x 3 row-major, input order, dtype; may be NULL.
+ * Asynchronous on cuda_stream. */
+fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream);
+
+/* Same operation with HOST buffers: copies charges host->device, evaluates, copies the results back and
+ * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
+fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);
+
+/* Frees all device memory of the plan.  NULL is allowed. */
+fmm_status fmm_plan_destroy(fmm_plan* plan);
+
+/* Introspection (HOST outputs, any may be NULL): tree depth L, number of boxes on all levels 0..L, number of
+ * leaf boxes 2^(s*L), number of weak (M2L) pairs over all levels, number of strong leaf pairs (including (t,t)),
+ * number of particle pairs the P2P stage visits (sum over strong leaf pairs of n_t * n_s). */
+fmm_status fmm_plan_info(const fmm_plan* plan, int* L, int64_t* n_boxes, int64_t* n_leaves, int64_t* n_weak,
+                         int64_t* n_strong, int64_t* n_p2p_pairs);
+
+/* Copy the hierarchy to HOST buffers (any may be NULL).  Boxes are numbered level by level, level l holding
+ * 2^(s*l) boxes, children of box b being b*2^s + j (lower half first at every sub-split).
+ *   h_perm      : N int32, tree order -> input index (leaves in box order, ascending input index inside a leaf).
+ *   h_box_start : n_boxes int32, first tree-order slot of the box;  h_box_count : n_boxes int32.
+ *   h_box_lo/hi : n_boxes x 3, dtype, tight particle bounding box (zeros for empty boxes).
+ *   h_box_ctr   : n_boxes x 3 double, 0.5*(lo+hi);  h_box_rad : n_boxes double, half diagonal (fp64, no FMA). */
+fmm_status fmm_plan_copy_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_box_start, int32_t* h_box_count,
+                              void* h_box_lo, void* h_box_hi, double* h_box_ctr, double* h_box_rad);
+
+/* Copy the interaction lists to HOST buffers (any may be NULL), canonical form: CSR by target, sources ascending.
+ *   h_weak_off   : n_boxes+1 int64 (row = target global box id);  h_weak_src : n_weak int32 global box ids.
+ *   h_strong_off : n_leaves+1 int64 (row = target leaf index);    h_strong_src : n_strong int32 leaf indices. */
+fmm_status fmm_plan_copy_lists(const fmm_plan* plan, int64_t* h_weak_off, int32_t* h_weak_src,
+                               int64_t* h_strong_off, int32_t* h_strong_src);
+
+/* Per-stage device times of the most recent fmm_evaluate_profiled call, in milliseconds (HOST out, 8 doubles):
+ * [0] permute, [1] P2M, [2] M2M, [3] M2L, [4] L2L, [5] L2P, [6] P2P, [7] total.  fmm_evaluate_profiled is
+ * fmm_evaluate with CUDA events between the stages (it synchronises the stream). */
+fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field,
+                                 void* cuda_stream, double* h_stage_ms);
+
+/* Plan-phase device times in ms (HOST out, 4 doubles): [0] sort keys, [1] tree rounds, [2] lists, [3] total. */
+fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
+
+/* Selects the M2L implementation used by subsequent fmm_evaluate calls on this plan:
+ * 0 = automatic (unrolled register kernel when available for (p, dtype), else generic), 1 = force generic. */
+fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
+
+/* Thread-local, NUL-terminated description of the last failure on the calling thread ("" if none). */
+const char* fmm_last_error(void);
+
+/* Library version string. */
+const char* fmm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_2511_15269_FMM_H */

@@ -1,0 +1,230 @@
+// api.cu -- the extern "C" boundary declared in include/fmm.h.  Argument checking, plan lifetime, host-buffer
+// convenience path; every computation is a kernel launched from plan.cu / evaluate.cu / m2l_fast.cu.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "internal.cuh"
+
+namespace fmm {
+namespace {
+thread_local std::string g_err;
+}
+void set_error(const std::string& msg) { g_err = msg; }
+}  // namespace fmm
+
+struct fmm_plan {
+    fmm::Plan P;
+};
+
+using namespace fmm;
+
+namespace {
+
+template <typename F>
+fmm_status guarded(F&& f) {
+    try {
+        return f();
+    } catch (CudaFail& c) {
+        cudaGetLastError();  // clear the sticky-less error state
+        return c.st;
+    } catch (std::bad_alloc&) {
+        set_error("host allocation failed");
+        return FMM_ERR_ALLOC;
+    } catch (...) {
+        set_error("unexpected exception");
+        return FMM_ERR_CUDA;
+    }
+}
+
+size_t esize(fmm_dtype d) { return d == FMM_F32 ? 4 : 8; }
+
+}  // namespace
+
+extern "C" {
+
+const char* fmm_last_error(void) { return g_err.c_str(); }
+const char* fmm_version(void) { return "paper_2511_15269_b200 0.1 (sm_100a)"; }
+
+fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max, int s, const fmm_admissibility* adm, fmm_dtype dtype,
+                           void* cuda_stream, fmm_plan** out_plan) {
+    if (out_plan) *out_plan = nullptr;
+    return guarded([&]() -> fmm_status {
+        g_err.clear();
+        if (!out_plan || !d_positions) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (N < 1 || N > 0x7fffff00ll) { set_error("N must be in [1, 2^31)"); return FMM_ERR_INVALID_ARG; }
+        if (p < 0 || p > PMAX) { set_error("p must be in [0, FMM_P_MAX]"); return FMM_ERR_INVALID_ARG; }
+        if (N_max < 1 || s < 1) { set_error("N_max and s must be >= 1"); return FMM_ERR_INVALID_ARG; }
+        if (dtype != FMM_F32 && dtype != FMM_F64) { set_error("unknown dtype"); return FMM_ERR_INVALID_ARG; }
+        double theta = 0.77;
+        if (adm) {
+            theta = adm->theta;
+            if (!(theta > 0.0 && theta < 1.0)) { set_error("theta must be in (0,1)"); return FMM_ERR_INVALID_ARG; }
+            if (adm->cross_level != 0) { set_error("cross_level lists are not implemented"); return FMM_ERR_UNSUPPORTED; }
+        }
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+            cudaGetLastError();
+            set_error("no CUDA device: this library has no CPU fallback");
+            return FMM_ERR_CUDA;
+        }
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        fmm_plan* h = new fmm_plan();
+        Plan& P = h->P;
+        try {
+            P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta;
+            P.K = (p + 1) * (p + 1);
+            P.Kp = (P.K + 3) & ~3;
+            int L = 0;  // smallest L with ceil(N / 2^(sL)) <= N_max
+            for (;; ++L) {
+                int64_t q = N;
+                for (int i = 0; i < s * L; ++i) q = (q + 1) / 2;
+                if (q <= N_max) break;
+            }
+            if ((int64_t)s * L > 30) { set_error("tree too deep: s*L > 30"); delete h; return FMM_ERR_UNSUPPORTED; }
+            P.L = L;
+            P.level_off.assign(L + 2, 0);
+            for (int l = 0; l <= L; ++l) P.level_off[l + 1] = P.level_off[l] + ((int64_t)1 << (s * l));
+            P.n_boxes = P.level_off[L + 1];
+            P.n_leaves = (int64_t)1 << (s * L);
+            if (P.n_boxes > 0x7fffff00ll) { set_error("too many boxes"); delete h; return FMM_ERR_UNSUPPORTED; }
+            tables();
+            cudaEvent_t e0, e1;
+            FMM_CUDA_CHECK(cudaEventCreate(&e0));
+            FMM_CUDA_CHECK(cudaEventCreate(&e1));
+            FMM_CUDA_CHECK(cudaEventRecord(e0, st));
+            build_tree(P, d_positions, st);
+            build_lists(P, st);
+            const size_t es = esize(dtype);
+            P.pq.alloc((size_t)N * 4 * es);
+            P.far.alloc((size_t)N * 4 * es);
+            P.Mc.alloc((size_t)P.n_boxes * P.Kp * es);
+            P.Lc.alloc((size_t)P.n_boxes * P.Kp * es);
+            FMM_CUDA_CHECK(cudaMemsetAsync(P.Mc.p, 0, P.Mc.n, st));
+            FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+            FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+            float ms = 0;
+            cudaEventElapsedTime(&ms, e0, e1);
+            P.plan_ms[3] = ms;
+            cudaEventDestroy(e0);
+            cudaEventDestroy(e1);
+        } catch (...) {
+            delete h;
+            throw;
+        }
+        *out_plan = h;
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_destroy(fmm_plan* plan) {
+    delete plan;
+    return FMM_OK;
+}
+
+fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !d_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        run_evaluate(plan->P, d_charges, d_potential, d_field, (cudaStream_t)cuda_stream, nullptr);
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream,
+                                 double* h_stage_ms) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !d_charges || !h_stage_ms) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        cudaEvent_t ev[8];
+        for (auto& e : ev) FMM_CUDA_CHECK(cudaEventCreate(&e));
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        run_evaluate(plan->P, d_charges, d_potential, d_field, st, ev);
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        for (int i = 0; i < 7; ++i) {
+            float ms = 0;
+            cudaEventElapsedTime(&ms, ev[i], ev[i + 1]);
+            h_stage_ms[i] = ms;
+        }
+        float tot = 0;
+        cudaEventElapsedTime(&tot, ev[0], ev[7]);
+        h_stage_ms[7] = tot;
+        for (auto& e : ev) cudaEventDestroy(e);
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !h_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        Plan& P = const_cast<Plan&>(plan->P);
+        const size_t es = esize(P.dtype);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        if (!P.h2d_q.p) P.h2d_q.alloc((size_t)P.N * es);
+        if (!P.d2h_out.p) P.d2h_out.alloc((size_t)P.N * 4 * es);
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.h2d_q.p, h_charges, (size_t)P.N * es, cudaMemcpyHostToDevice, st));
+        char* dpot = h_potential ? P.d2h_out.p : nullptr;
+        char* dfld = h_field ? P.d2h_out.p + (size_t)P.N * es : nullptr;
+        run_evaluate(P, P.h2d_q.p, dpot, dfld, st, nullptr);
+        if (h_potential) FMM_CUDA_CHECK(cudaMemcpyAsync(h_potential, dpot, (size_t)P.N * es, cudaMemcpyDeviceToHost, st));
+        if (h_field) FMM_CUDA_CHECK(cudaMemcpyAsync(h_field, dfld, (size_t)P.N * 3 * es, cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_info(const fmm_plan* plan, int* L, int64_t* n_boxes, int64_t* n_leaves, int64_t* n_weak, int64_t* n_strong,
+                         int64_t* n_p2p_pairs) {
+    if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+    const Plan& P = plan->P;
+    if (L) *L = P.L;
+    if (n_boxes) *n_boxes = P.n_boxes;
+    if (n_leaves) *n_leaves = P.n_leaves;
+    if (n_weak) *n_weak = P.n_weak;
+    if (n_strong) *n_strong = P.n_strong;
+    if (n_p2p_pairs) *n_p2p_pairs = P.n_p2p_pairs;
+    return FMM_OK;
+}
+
+fmm_status fmm_plan_copy_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_box_start, int32_t* h_box_count, void* h_box_lo,
+                              void* h_box_hi, double* h_box_ctr, double* h_box_rad) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        const Plan& P = plan->P;
+        const size_t es = esize(P.dtype);
+        FMM_CUDA_CHECK(cudaDeviceSynchronize());
+        if (h_perm) FMM_CUDA_CHECK(cudaMemcpy(h_perm, P.perm.p, P.N * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (h_box_start) FMM_CUDA_CHECK(cudaMemcpy(h_box_start, P.box_start.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (h_box_count) FMM_CUDA_CHECK(cudaMemcpy(h_box_count, P.box_count.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (h_box_lo) FMM_CUDA_CHECK(cudaMemcpy(h_box_lo, P.box_lo.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
+        if (h_box_hi) FMM_CUDA_CHECK(cudaMemcpy(h_box_hi, P.box_hi.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
+        if (h_box_ctr) FMM_CUDA_CHECK(cudaMemcpy(h_box_ctr, P.box_ctr.p, P.n_boxes * 3 * sizeof(double), cudaMemcpyDeviceToHost));
+        if (h_box_rad) FMM_CUDA_CHECK(cudaMemcpy(h_box_rad, P.box_rad.p, P.n_boxes * sizeof(double), cudaMemcpyDeviceToHost));
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_copy_lists(const fmm_plan* plan, int64_t* h_weak_off, int32_t* h_weak_src, int64_t* h_strong_off, int32_t* h_strong_src) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        const Plan& P = plan->P;
+        FMM_CUDA_CHECK(cudaDeviceSynchronize());
+        if (h_weak_off) FMM_CUDA_CHECK(cudaMemcpy(h_weak_off, P.weak_off.p, (P.n_boxes + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost));
+        if (h_weak_src && P.n_weak) FMM_CUDA_CHECK(cudaMemcpy(h_weak_src, P.weak_src.p, P.n_weak * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (h_strong_off) FMM_CUDA_CHECK(cudaMemcpy(h_strong_off, P.strong_off.p, (P.n_leaves + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost));
+        if (h_strong_src && P.n_strong) FMM_CUDA_CHECK(cudaMemcpy(h_strong_src, P.strong_src.p, P.n_strong * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms) {
+    if (!plan || !h_ms) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+    for (int i = 0; i < 4; ++i) h_ms[i] = plan->P.plan_ms[i];
+    return FMM_OK;
+}
+
+fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {
+    if (!plan || variant < 0 || variant > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    plan->P.m2l_variant = variant;
+    return FMM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,576 @@
+// evaluate.cu -- the evaluate pipeline (stage order PAPER.md:251):
+//   permute charges -> P2M (eq. 13) -> M2M (App. B) -> M2L (App. B) -> L2L -> L2P (eq. 14, App. A.3) -> P2P
+// All coefficient arrays use the normalised, length-scaled representation described in tables.cu / DESIGN.md.
+// This file holds the kernels that work for every order p <= FMM_P_MAX and both dtypes; the unrolled register
+// M2L kernels live in m2l_fast.cu.
+#include "internal.cuh"
+
+namespace fmm {
+namespace {
+
+__constant__ double c_g[KMAX];   // g_n^m, double
+__constant__ float c_gf[KMAX];   // g_n^m, float
+
+template <typename T> struct V4;
+template <> struct V4<float> { using type = float4; };
+template <> struct V4<double> { using type = double4; };
+template <typename T> __device__ inline typename V4<T>::type make4(T a, T b, T c, T d);
+template <> __device__ inline float4 make4<float>(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
+template <> __device__ inline double4 make4<double>(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
+
+template <typename T> __device__ inline T gnorm(int idx);
+template <> __device__ inline float gnorm<float>(int idx) { return c_gf[idx]; }
+template <> __device__ inline double gnorm<double>(int idx) { return c_g[idx]; }
+
+template <typename T> __device__ inline T rsqrt_t(T x);
+template <> __device__ inline float rsqrt_t<float>(float x) { return rsqrtf(x); }
+template <> __device__ inline double rsqrt_t<double>(double x) { return rsqrt(x); }
+
+inline unsigned nblocks(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
+
+// ------------------------------------------------------------------------------------------------ permute (a3)
+template <typename T>
+__global__ void permute_k(const T* __restrict__ pos_tree, const T* __restrict__ q, const int32_t* __restrict__ perm,
+                          typename V4<T>::type* __restrict__ pq, int64_t N) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    pq[k] = make4<T>(pos_tree[3 * k], pos_tree[3 * k + 1], pos_tree[3 * k + 2], q[perm[k]]);
+}
+
+// ------------------------------------------------------------------------------------------------ basis recursions
+// App. A.1 on scaled coordinates, degree by degree, two rotating degree slots indexed [n&1][m+P].
+// emit(n, m, R^_n^m) is called for every (n,m), n ascending, with compile-time n, m after unrolling.
+template <int P, typename T, typename F>
+__device__ __forceinline__ void regular_rec(T x, T y, T z, F&& emit) {
+    T R[2][2 * P + 1];
+    const T r2 = x * x + y * y + z * z;
+    R[0][P] = T(1);
+    emit(0, 0, R[0][P]);
+#pragma unroll
+    for (int n = 1; n <= P; ++n) {
+        const int c = n & 1, q = c ^ 1;
+        // inner orders first (they read slot c = degree n-2 and slot q = degree n-1), then +-(n-1), then +-n
+#pragma unroll
+        for (int m = -(n - 2); m <= n - 2; ++m) {
+            const int am = m < 0 ? -m : m;
+            R[c][P + m] = (T(2 * n - 1) * z * R[q][P + m] - r2 * R[c][P + m]) * (T(1) / T((n - am) * (n + am)));
+        }
+        if (n == 1) {
+            R[c][P] = z * R[q][P];
+            R[c][P + 1] = x * T(0.5);
+            R[c][P - 1] = -y * T(0.5);
+        } else {
+            const T dp = R[q][P + n - 1], dm = R[q][P - (n - 1)];
+            R[c][P + n - 1] = z * dp;
+            R[c][P - (n - 1)] = z * dm;
+            R[c][P + n] = (x * dp + y * dm) * (T(1) / T(2 * n));
+            R[c][P - n] = (x * dm - y * dp) * (T(1) / T(2 * n));
+        }
+#pragma unroll
+        for (int m = -n; m <= n; ++m) emit(n, m, R[c][P + m]);
+    }
+}
+
+// App. A.1 + A.3 (with reading G1: no leading minus at PAPER.md:419).
+template <int P, typename T, typename F>
+__device__ __forceinline__ void regular_grad_rec(T x, T y, T z, F&& emit) {
+    T R[2][2 * P + 1], GX[2][2 * P + 1], GY[2][2 * P + 1], GZ[2][2 * P + 1];
+    const T r2 = x * x + y * y + z * z;
+    R[0][P] = T(1); GX[0][P] = T(0); GY[0][P] = T(0); GZ[0][P] = T(0);
+    emit(0, 0, R[0][P], GX[0][P], GY[0][P], GZ[0][P]);
+#pragma unroll
+    for (int n = 1; n <= P; ++n) {
+        const int c = n & 1, q = c ^ 1;
+#pragma unroll
+        for (int m = -(n - 2); m <= n - 2; ++m) {
+            const int am = m < 0 ? -m : m;
+            const T inv = T(1) / T((n - am) * (n + am));
+            const T w = T(2 * n - 1);
+            const T r1 = R[q][P + m], r0 = R[c][P + m];
+            GX[c][P + m] = (w * z * GX[q][P + m] - r2 * GX[c][P + m] - T(2) * r0 * x) * inv;
+            GY[c][P + m] = (w * z * GY[q][P + m] - r2 * GY[c][P + m] - T(2) * r0 * y) * inv;
+            GZ[c][P + m] = (w * (z * GZ[q][P + m] + r1) - r2 * GZ[c][P + m] - T(2) * r0 * z) * inv;
+            R[c][P + m] = (w * z * r1 - r2 * r0) * inv;
+        }
+        if (n == 1) {
+            R[c][P] = z * R[q][P]; GX[c][P] = T(0); GY[c][P] = T(0); GZ[c][P] = R[q][P];
+            R[c][P + 1] = x * T(0.5); GX[c][P + 1] = T(0.5); GY[c][P + 1] = T(0); GZ[c][P + 1] = T(0);
+            R[c][P - 1] = -y * T(0.5); GX[c][P - 1] = T(0); GY[c][P - 1] = T(-0.5); GZ[c][P - 1] = T(0);
+        } else {
+            const int a = P + n - 1, b = P - (n - 1);
+            const T dp = R[q][a], dm = R[q][b];
+            const T dpx = GX[q][a], dpy = GY[q][a], dpz = GZ[q][a], dmx = GX[q][b], dmy = GY[q][b], dmz = GZ[q][b];
+            const T h = T(1) / T(2 * n);
+            R[c][a] = z * dp; GX[c][a] = z * dpx; GY[c][a] = z * dpy; GZ[c][a] = z * dpz + dp;
+            R[c][b] = z * dm; GX[c][b] = z * dmx; GY[c][b] = z * dmy; GZ[c][b] = z * dmz + dm;
+            R[c][P + n] = (x * dp + y * dm) * h;
+            GX[c][P + n] = (x * dpx + y * dmx + dp) * h;
+            GY[c][P + n] = (x * dpy + y * dmy + dm) * h;
+            GZ[c][P + n] = (x * dpz + y * dmz) * h;
+            R[c][P - n] = (x * dm - y * dp) * h;
+            GX[c][P - n] = (x * dmx - y * dpx + dm) * h;
+            GY[c][P - n] = (x * dmy - y * dpy - dp) * h;
+            GZ[c][P - n] = (x * dmz - y * dpz) * h;
+        }
+#pragma unroll
+        for (int m = -n; m <= n; ++m) emit(n, m, R[c][P + m], GX[c][P + m], GY[c][P + m], GZ[c][P + m]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ P2M (a4), warp per leaf
+constexpr int WARPS_PER_BLOCK = 4;
+
+template <typename T, int P>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
+                                                              const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
+                                                              const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves, int Kp,
+                                                              T* __restrict__ Mc) {
+    constexpr int K = (P + 1) * (P + 1);
+    constexpr int NJ = (K + 31) / 32;
+    const int lane = threadIdx.x & 31;
+    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
+    if (leaf >= n_leaves) return;
+    const int64_t g = leaf0 + leaf;
+    const int st = box_start[g], cnt = box_count[g];
+    const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
+    const T inva = T(1) / scale[g];
+    T acc[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) acc[j] = T(0);
+    for (int base = 0; base < cnt; base += 32) {
+        const int i = base + lane;
+        T x = 0, y = 0, z = 0, q = 0;
+        if (i < cnt) {
+            const typename V4<T>::type v = pq[st + i];
+            x = (T)((double)v.x - cx) * inva;
+            y = (T)((double)v.y - cy) * inva;
+            z = (T)((double)v.z - cz) * inva;
+            q = v.w;
+        }
+        regular_rec<P, T>(x, y, z, [&](int n, int m, T val) {
+            const int idx = n * n + n + m;
+            T v = q * val * gnorm<T>(idx);
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            if (lane == (idx & 31)) acc[idx >> 5] += v;
+        });
+    }
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+        const int idx = lane + 32 * j;
+        if (idx < K) Mc[g * Kp + idx] = acc[j];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ L2P (a8), warp per leaf
+template <typename T, int P>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
+                                                              const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
+                                                              const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves, int Kp,
+                                                              const T* __restrict__ Lc, typename V4<T>::type* __restrict__ far) {
+    constexpr int K = (P + 1) * (P + 1);
+    __shared__ T sL[WARPS_PER_BLOCK][K];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
+    if (leaf >= n_leaves) return;
+    const int64_t g = leaf0 + leaf;
+    const int st = box_start[g], cnt = box_count[g];
+    const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
+    const T inva = T(1) / scale[g];
+    for (int idx = lane; idx < K; idx += 32) sL[w][idx] = Lc[g * Kp + idx] * gnorm<T>(idx);
+    __syncwarp();
+    for (int base = 0; base < cnt; base += 32) {
+        const int i = base + lane;
+        if (i < cnt) {
+            const typename V4<T>::type v = pq[st + i];
+            const T x = (T)((double)v.x - cx) * inva, y = (T)((double)v.y - cy) * inva, z = (T)((double)v.z - cz) * inva;
+            T phi = 0, gx = 0, gy = 0, gz = 0;
+            regular_grad_rec<P, T>(x, y, z, [&](int n, int m, T R, T GX, T GY, T GZ) {
+                const T l = sL[w][n * n + n + m];
+                phi += l * R; gx += l * GX; gy += l * GY; gz += l * GZ;
+            });
+            far[st + i] = make4<T>(phi, gx * inva, gy * inva, gz * inva);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ generic translations
+// One warp per translation; state vectors in shared memory; rotation = Z(-phi) B Z(-theta) B^T [shift] B Z(theta) B^T Z(phi).
+template <typename T>
+struct WarpScratch {
+    T v[KMAX], u[KMAX];
+    T cph[PMAX + 1], sph[PMAX + 1], cth[PMAX + 1], sth[PMAX + 1], pw1[PMAX + 1], pw2[PMAX + 1];
+};
+
+struct TabPtrs {
+    const void* B;  // T-typed rotation blocks
+    const double *H, *A;
+};
+
+__device__ inline void idx_to_nm(int idx, int& n, int& m) {
+    n = (int)sqrtf((float)idx);
+    while (n * n > idx) --n;
+    while ((n + 1) * (n + 1) <= idx) ++n;
+    m = idx - n * n - n;
+}
+
+template <typename T>
+__device__ inline void az_step(int K, const T* in, T* out, const T* c, const T* s, T sign, int lane) {
+    for (int idx = lane; idx < K; idx += 32) {
+        int n, m;
+        idx_to_nm(idx, n, m);
+        const int am = m < 0 ? -m : m;
+        T ss = sign * s[am];
+        if (m < 0) ss = -ss;
+        out[idx] = in[idx] * c[am] - in[idx - 2 * m] * ss;
+    }
+}
+
+template <typename T>
+__device__ inline void b_step(int K, const T* in, T* out, const T* Btab, bool transpose, int lane) {
+    for (int idx = lane; idx < K; idx += 32) {
+        int n, m;
+        idx_to_nm(idx, n, m);
+        const int w = 2 * n + 1, i = m + n;
+        const T* Bn = Btab + boff(n);
+        const T* vin = in + n * n;
+        T acc = 0;
+        if (transpose) for (int j = 0; j < w; ++j) acc += Bn[j * w + i] * vin[j];
+        else for (int j = 0; j < w; ++j) acc += Bn[i * w + j] * vin[j];
+        out[idx] = acc;
+    }
+}
+
+// kind 0 = M2M (b = child - parent), 1 = M2L (b = source - target), 2 = L2L (b = parent - child)   [reading G3]
+// a_old / a_new: length scales of the box the input / the output expansion belongs to.  Result in ws.u.
+template <typename T>
+__device__ inline void translate_warp(int kind, int p, const T* __restrict__ src, double bxd, double byd, double bzd, T a_old, T a_new,
+                                      WarpScratch<T>& ws, TabPtrs tp, int lane) {
+    const int K = (p + 1) * (p + 1);
+    const int P1 = PMAX + 1;
+    const T bx = (T)bxd, by = (T)byd, bz = (T)bzd;
+    const T r = sqrt(bx * bx + by * by + bz * bz);
+    const T rxy = sqrt(bx * bx + by * by);
+    const T ct = r > 0 ? bz / r : T(1), st = r > 0 ? rxy / r : T(0);
+    const T cp = rxy > 0 ? bx / rxy : T(1), sp = rxy > 0 ? by / rxy : T(0);
+    for (int idx = lane; idx < K; idx += 32) ws.v[idx] = src[idx];
+    if (lane <= p) {
+        T c = 1, s = 0, c2 = 1, s2 = 0, x1, x2, p1 = 1, p2 = 1;
+        if (kind == 0) { x1 = r / a_new; x2 = a_old / a_new; }
+        else if (kind == 1) { x1 = a_new / r; x2 = a_old / r; }
+        else { x1 = -r / a_old; x2 = a_new / a_old; }
+        for (int i = 0; i < lane; ++i) {
+            T t = c * cp - s * sp; s = s * cp + c * sp; c = t;
+            t = c2 * ct - s2 * st; s2 = s2 * ct + c2 * st; c2 = t;
+            p1 *= x1; p2 *= x2;
+        }
+        ws.cph[lane] = c; ws.sph[lane] = s; ws.cth[lane] = c2; ws.sth[lane] = s2; ws.pw1[lane] = p1; ws.pw2[lane] = p2;
+    }
+    __syncwarp();
+    const T* Btab = (const T*)tp.B;
+    az_step<T>(K, ws.v, ws.u, ws.cph, ws.sph, T(1), lane); __syncwarp();
+    b_step<T>(K, ws.u, ws.v, Btab, true, lane); __syncwarp();
+    az_step<T>(K, ws.v, ws.u, ws.cth, ws.sth, T(1), lane); __syncwarp();
+    b_step<T>(K, ws.u, ws.v, Btab, false, lane); __syncwarp();
+    // z-shift (App. B.3) in the normalised, scaled representation
+    for (int idx = lane; idx < K; idx += 32) {
+        int n, m;
+        idx_to_nm(idx, n, m);
+        const int am = m < 0 ? -m : m;
+        T acc = 0;
+        if (kind == 0) {
+            for (int k = am; k <= n; ++k) acc += (T)tp.A[(am * P1 + n) * P1 + k] * ws.pw1[n - k] * ws.pw2[k] * ws.v[k * k + k + m];
+        } else if (kind == 1) {
+            for (int k = am; k <= p; ++k) acc += (T)tp.H[(am * P1 + n) * P1 + k] * ws.pw2[k] * ws.v[k * k + k + m];
+            acc *= ws.pw1[n] / r;
+        } else {
+            for (int k = n; k <= p; ++k) acc += (T)tp.A[(am * P1 + k) * P1 + n] * ws.pw1[k - n] * ws.v[k * k + k + m];
+            acc *= ws.pw2[n];
+        }
+        ws.u[idx] = acc;
+    }
+    __syncwarp();
+    b_step<T>(K, ws.u, ws.v, Btab, true, lane); __syncwarp();
+    az_step<T>(K, ws.v, ws.u, ws.cth, ws.sth, T(-1), lane); __syncwarp();
+    b_step<T>(K, ws.u, ws.v, Btab, false, lane); __syncwarp();
+    az_step<T>(K, ws.v, ws.u, ws.cph, ws.sph, T(-1), lane); __syncwarp();
+}
+
+constexpr int NJMAX = (KMAX + 31) / 32;
+
+// M2M (a5): warp per parent box of level l-1, children in ascending order
+template <typename T>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) m2m_k(int p, int s, int64_t off_parent, int64_t off_child, int64_t nb_parent,
+                                                              const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
+                                                              const T* __restrict__ scale, int Kp, T* __restrict__ Mc, TabPtrs tp) {
+    __shared__ WarpScratch<T> wsm[WARPS_PER_BLOCK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t bp = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
+    if (bp >= nb_parent) return;
+    const int K = (p + 1) * (p + 1);
+    const int64_t gp = off_parent + bp;
+    T acc[NJMAX];
+#pragma unroll
+    for (int j = 0; j < NJMAX; ++j) acc[j] = 0;
+    for (int j = 0; j < (1 << s); ++j) {
+        const int64_t gc = off_child + (bp << s) + j;
+        if (box_count[gc] == 0) continue;
+        translate_warp<T>(0, p, Mc + gc * Kp, ctr[3 * gc] - ctr[3 * gp], ctr[3 * gc + 1] - ctr[3 * gp + 1], ctr[3 * gc + 2] - ctr[3 * gp + 2],
+                          scale[gc], scale[gp], wsm[w], tp, lane);
+#pragma unroll
+        for (int jj = 0; jj < NJMAX; ++jj) {
+            const int idx = lane + 32 * jj;
+            if (idx < K) acc[jj] += wsm[w].u[idx];
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int jj = 0; jj < NJMAX; ++jj) {
+        const int idx = lane + 32 * jj;
+        if (idx < K) Mc[gp * Kp + idx] = acc[jj];
+    }
+}
+
+// M2L (a6), generic: warp per target box, loop over its row of the weak list (CSR by target)
+template <typename T>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) m2l_generic_k(int p, int64_t n_boxes, const int64_t* __restrict__ weak_off,
+                                                                      const int32_t* __restrict__ weak_src, const double* __restrict__ ctr,
+                                                                      const T* __restrict__ scale, int Kp, const T* __restrict__ Mc,
+                                                                      T* __restrict__ Lc, TabPtrs tp) {
+    __shared__ WarpScratch<T> wsm[WARPS_PER_BLOCK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t gt = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
+    if (gt >= n_boxes) return;
+    const int64_t e0 = weak_off[gt], e1 = weak_off[gt + 1];
+    if (e0 == e1) return;
+    const int K = (p + 1) * (p + 1);
+    T acc[NJMAX];
+#pragma unroll
+    for (int j = 0; j < NJMAX; ++j) acc[j] = 0;
+    const double tx = ctr[3 * gt], ty = ctr[3 * gt + 1], tz = ctr[3 * gt + 2];
+    const T at = scale[gt];
+    for (int64_t e = e0; e < e1; ++e) {
+        const int64_t gs = weak_src[e];
+        translate_warp<T>(1, p, Mc + gs * Kp, ctr[3 * gs] - tx, ctr[3 * gs + 1] - ty, ctr[3 * gs + 2] - tz, scale[gs], at, wsm[w], tp, lane);
+#pragma unroll
+        for (int jj = 0; jj < NJMAX; ++jj) {
+            const int idx = lane + 32 * jj;
+            if (idx < K) acc[jj] += wsm[w].u[idx];
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int jj = 0; jj < NJMAX; ++jj) {
+        const int idx = lane + 32 * jj;
+        if (idx < K) Lc[gt * Kp + idx] += acc[jj];
+    }
+}
+
+// L2L (a7): warp per child box of level l
+template <typename T>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2l_k(int p, int s, int64_t off_parent, int64_t off_child, int64_t nb_child,
+                                                              const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
+                                                              const T* __restrict__ scale, int Kp, T* __restrict__ Lc, TabPtrs tp) {
+    __shared__ WarpScratch<T> wsm[WARPS_PER_BLOCK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t bc = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
+    if (bc >= nb_child) return;
+    const int64_t gc = off_child + bc, gp = off_parent + (bc >> s);
+    if (box_count[gc] == 0) return;
+    const int K = (p + 1) * (p + 1);
+    translate_warp<T>(2, p, Lc + gp * Kp, ctr[3 * gp] - ctr[3 * gc], ctr[3 * gp + 1] - ctr[3 * gc + 1], ctr[3 * gp + 2] - ctr[3 * gc + 2],
+                      scale[gp], scale[gc], wsm[w], tp, lane);
+    for (int idx = lane; idx < K; idx += 32) Lc[gc * Kp + idx] += wsm[w].u[idx];
+}
+
+// ------------------------------------------------------------------------------------------------ P2P (a9) + finalize (a10)
+// One target leaf per CTA.  Threads are arranged as (target group, source slice): each thread keeps TPT targets in
+// registers and walks every nslices-th source of the shared-memory tile; partial sums are combined through shared memory.
+constexpr int P2P_THREADS = 128;
+constexpr int P2P_TPT = 4;
+constexpr int P2P_TILE = 512;
+
+template <typename T>
+__global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ leaf_start,
+                                                     const int32_t* __restrict__ leaf_cnt, const int64_t* __restrict__ strong_off,
+                                                     const int32_t* __restrict__ strong_src, const typename V4<T>::type* __restrict__ far,
+                                                     const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field) {
+    using T4 = typename V4<T>::type;
+    __shared__ T4 sh[P2P_TILE];
+    __shared__ T red[P2P_THREADS * P2P_TPT * 4];
+    const int tid = threadIdx.x;
+    const int64_t leaf = blockIdx.x;
+    const int tst = leaf_start[leaf], tcnt = leaf_cnt[leaf];
+    if (tcnt == 0) return;
+    const int64_t e0 = strong_off[leaf], e1 = strong_off[leaf + 1];
+    const T inv4pi = T(0.079577471545947667884441881686257);
+    for (int tbase = 0; tbase < tcnt; tbase += P2P_THREADS * P2P_TPT) {
+        const int tn = min(tcnt - tbase, P2P_THREADS * P2P_TPT);
+        int ntg = (tn + P2P_TPT - 1) / P2P_TPT, ntgp = 1;
+        while (ntgp < ntg) ntgp <<= 1;
+        const int nsl = P2P_THREADS / ntgp;
+        const int tg = tid & (ntgp - 1), sl = tid / ntgp;
+        T tx[P2P_TPT], ty[P2P_TPT], tz[P2P_TPT], ph[P2P_TPT], gx[P2P_TPT], gy[P2P_TPT], gz[P2P_TPT];
+#pragma unroll
+        for (int t = 0; t < P2P_TPT; ++t) {
+            const int ti = tg * P2P_TPT + t;
+            // out-of-range targets are parked far away with zero weight (their sums are discarded)
+            if (ti < tn) {
+                const T4 v = pq[tst + tbase + ti];
+                tx[t] = v.x; ty[t] = v.y; tz[t] = v.z;
+            } else {
+                tx[t] = T(1e18); ty[t] = T(1e18); tz[t] = T(1e18);
+            }
+            ph[t] = gx[t] = gy[t] = gz[t] = T(0);
+        }
+        int64_t e = e0;
+        int sub = 0;
+        for (;;) {
+            int tile_n = 0;
+            __syncthreads();
+            while (e < e1 && tile_n < P2P_TILE) {
+                const int sleaf = strong_src[e];
+                const int sst = leaf_start[sleaf], sc = leaf_cnt[sleaf];
+                const int take = min(sc - sub, P2P_TILE - tile_n);
+                for (int i = tid; i < take; i += P2P_THREADS) sh[tile_n + i] = pq[sst + sub + i];
+                tile_n += take;
+                sub += take;
+                if (sub >= sc) { ++e; sub = 0; }
+            }
+            if (tile_n == 0) break;
+            __syncthreads();
+#pragma unroll 2
+            for (int j = sl; j < tile_n; j += nsl) {
+                const T4 sv = sh[j];
+#pragma unroll
+                for (int t = 0; t < P2P_TPT; ++t) {
+                    const T dx = tx[t] - sv.x, dy = ty[t] - sv.y, dz = tz[t] - sv.z;
+                    const T r2 = dx * dx + dy * dy + dz * dz;
+                    T inv = rsqrt_t<T>(r2);
+                    inv = (r2 > T(0)) ? inv : T(0);  // S3: self / coincident pairs contribute nothing
+                    const T inv2 = inv * inv;
+                    const T q3 = sv.w * inv * inv2;
+                    ph[t] += sv.w * inv;
+                    gx[t] -= q3 * dx; gy[t] -= q3 * dy; gz[t] -= q3 * dz;
+                }
+            }
+        }
+        // combine the source slices
+        __syncthreads();
+#pragma unroll
+        for (int t = 0; t < P2P_TPT; ++t) {
+            T* r = red + ((sl * ntgp + tg) * P2P_TPT + t) * 4;
+            r[0] = ph[t]; r[1] = gx[t]; r[2] = gy[t]; r[3] = gz[t];
+        }
+        __syncthreads();
+        for (int ti = tid; ti < tn; ti += P2P_THREADS) {
+            const int g2 = ti / P2P_TPT, t2 = ti % P2P_TPT;
+            T a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+            for (int s2 = 0; s2 < nsl; ++s2) {
+                const T* r = red + ((s2 * ntgp + g2) * P2P_TPT + t2) * 4;
+                a0 += r[0]; a1 += r[1]; a2 += r[2]; a3 += r[3];
+            }
+            const int k = tst + tbase + ti;
+            const T4 f = far[k];
+            const int64_t i = perm[k];
+            if (pot) pot[i] = -(f.x + a0) * inv4pi;                 // eqs. (2), (9), (14)
+            if (field) {                                            // field = -grad u  (reading S2)
+                field[3 * i] = (f.y + a1) * inv4pi;
+                field[3 * i + 1] = (f.z + a2) * inv4pi;
+                field[3 * i + 2] = (f.w + a3) * inv4pi;
+            }
+        }
+    }
+}
+
+template <typename T, int P>
+void launch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
+    using T4 = typename V4<T>::type;
+    const int64_t leaf0 = Pl.level_off[Pl.L];
+    const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK);
+    if (!l2p)
+        p2m_k<T, P><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p,
+                                                           leaf0, Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p);
+    else
+        l2p_k<T, P><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p,
+                                                           leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p, (T4*)Pl.far.p);
+}
+
+template <typename T>
+void dispatch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
+    switch (Pl.p) {
+#define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, st); break;
+        FMM_CASE(0) FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
+        FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12) FMM_CASE(13) FMM_CASE(14) FMM_CASE(15) FMM_CASE(16)
+#undef FMM_CASE
+    }
+}
+
+bool g_const_uploaded = false;
+
+template <typename T>
+void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+    using T4 = typename V4<T>::type;
+    const Tables& tb = tables();
+    TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
+    const int p = Pl.p, s = Pl.s, L = Pl.L;
+    const int64_t N = Pl.N;
+    auto mark = [&](int i) { if (ev) FMM_CUDA_CHECK(cudaEventRecord(ev[i], st)); };
+    mark(0);
+    permute_k<T><<<nblocks(N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, st));
+    mark(1);
+    dispatch_p2m_l2p<T>(Pl, false, st);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(2);
+    for (int l = L; l >= 1; --l) {
+        const int64_t nbp = (int64_t)1 << (s * (l - 1));
+        m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbp, Pl.box_count.p,
+                                                                                Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Mc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(3);
+    if (Pl.n_weak > 0) {
+        if (Pl.m2l_variant == 0 && m2l_fast_available(p, Pl.dtype)) m2l_fast_launch(Pl, st);
+        else
+            m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(
+                p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(4);
+    for (int l = 1; l <= L; ++l) {
+        const int64_t nbc = (int64_t)1 << (s * l);
+        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
+                                                                                Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Lc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(5);
+    dispatch_p2m_l2p<T>(Pl, true, st);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(6);
+    const int64_t leaf0 = Pl.level_off[L];
+    p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
+                                                            Pl.strong_src.p, (const T4*)Pl.far.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(7);
+}
+
+}  // namespace
+
+void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+    if (!g_const_uploaded) {
+        const Tables& tb = tables();
+        std::vector<double> g(KMAX);
+        std::vector<float> gf(KMAX);
+        FMM_CUDA_CHECK(cudaMemcpy(g.data(), tb.d_g, KMAX * sizeof(double), cudaMemcpyDeviceToHost));
+        for (int i = 0; i < KMAX; ++i) gf[i] = (float)g[i];
+        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_g, g.data(), KMAX * sizeof(double)));
+        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
+        g_const_uploaded = true;
+    }
+    if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev);
+    else run_t<double>(P, d_q, d_pot, d_field, st, ev);
+}
+
+}  // namespace fmm

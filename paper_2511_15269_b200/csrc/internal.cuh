@@ -1,0 +1,110 @@
+// internal.cuh -- shared declarations of the CUDA path (plan struct, error helpers, device tables).
+// Not part of the public boundary (include/fmm.h) and not shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/fmm.h"
+
+namespace fmm {
+
+constexpr int PMAX = FMM_P_MAX;
+constexpr int KMAX = (PMAX + 1) * (PMAX + 1);
+
+void set_error(const std::string& msg);
+
+struct CudaFail {
+    fmm_status st;
+};
+
+#define FMM_CUDA_CHECK(expr)                                                                               \
+    do {                                                                                                   \
+        cudaError_t _e = (expr);                                                                           \
+        if (_e != cudaSuccess) {                                                                           \
+            ::fmm::set_error(std::string(#expr) + ": " + cudaGetErrorString(_e));                          \
+            throw ::fmm::CudaFail{_e == cudaErrorMemoryAllocation ? FMM_ERR_ALLOC : FMM_ERR_CUDA};         \
+        }                                                                                                  \
+    } while (0)
+
+// device buffer owned by the plan
+template <typename T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t n = 0;
+    void alloc(size_t count) {
+        release();
+        n = count;
+        if (count) FMM_CUDA_CHECK(cudaMalloc((void**)&p, count * sizeof(T)));
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+    ~DevBuf() { release(); }
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete;
+    DevBuf& operator=(const DevBuf&) = delete;
+};
+
+// Constant tables of the normalised operators (built once per process, host fp64 -> device):
+//   Bmat : per degree n a (2n+1)x(2n+1) row-major block at offset boff(n) = n(2n-1)(2n+1)/3;
+//          polar rotation Q_n(theta) = B_n Z_n(theta) B_n^T  (exact identity, B_n derived from d^n(pi/2))
+//   Hm2l : H[m][n][k] = (n+k)! / sqrt((n-m)!(n+m)!(k-m)!(k+m)!) * (-1)^(k+m)      (M2L z-shift weights)
+//   Am2m : A[m][n][k] = sqrt((n-m)!(n+m)!/((k-m)!(k+m)!)) / (n-k)!   for k<=n      (M2M; L2L uses A[m][k][n])
+//   gnorm: g[idx(n,m)] = sqrt((n-|m|)!(n+|m|)!) * (m ? sqrt2 : 1)
+struct Tables {
+    double* d_B = nullptr;   // sum_n (2n+1)^2 doubles
+    float* d_Bf = nullptr;   // same in fp32
+    double* d_H = nullptr;   // (PMAX+1)^3
+    double* d_A = nullptr;   // (PMAX+1)^3
+    double* d_g = nullptr;   // KMAX
+    std::vector<double> h_B; // host copy (used by the unrolled-kernel self check)
+};
+const Tables& tables();  // throws CudaFail
+__host__ __device__ inline int boff(int n) { return n * (2 * n - 1) * (2 * n + 1) / 3; }
+
+struct Plan {
+    int64_t N = 0;
+    int p = 0, N_max = 0, s = 0, L = 0;
+    fmm_dtype dtype = FMM_F32;
+    double theta = 0.77;
+    int K = 0, Kp = 0;  // (p+1)^2 and the padded row stride of coefficient arrays
+    int64_t n_boxes = 0, n_leaves = 0, n_weak = 0, n_strong = 0, n_p2p_pairs = 0;
+    std::vector<int64_t> level_off;  // L+2
+    std::vector<int64_t> weak_level_off;  // L+2: offsets of each level's pairs in the weak list
+    int m2l_variant = 0;
+    int max_leaf = 0;  // largest leaf population
+
+    DevBuf<int32_t> perm;                 // N: tree order -> input index
+    DevBuf<char> pos_tree;                // N x 3 dtype, tree order
+    DevBuf<int32_t> box_start, box_count; // n_boxes
+    DevBuf<char> box_lo, box_hi;          // n_boxes x 3 dtype
+    DevBuf<double> box_ctr, box_rad;      // n_boxes x 3, n_boxes  (fp64 always)
+    DevBuf<char> box_scale;               // n_boxes dtype: expansion length scale a_box
+    DevBuf<int64_t> weak_off;             // n_boxes+1
+    DevBuf<int32_t> weak_src, weak_tgt;   // n_weak (global ids)
+    DevBuf<int64_t> strong_off;           // n_leaves+1
+    DevBuf<int32_t> strong_src;           // n_strong (leaf indices)
+    // evaluate scratch
+    DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
+    DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
+    DevBuf<char> far;     // N x 4 dtype: (phi_far, grad phi_far) tree order
+    DevBuf<char> h2d_q, d2h_out;  // staging for fmm_evaluate_host
+    double plan_ms[4] = {0, 0, 0, 0};
+    double stage_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+// plan.cu
+void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
+void build_lists(Plan& P, cudaStream_t st);
+// evaluate.cu
+void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
+// m2l_fast.cu: returns false if no unrolled kernel exists for (p, dtype)
+bool m2l_fast_available(int p, fmm_dtype dt);
+void m2l_fast_launch(const Plan& P, cudaStream_t st);
+
+}  // namespace fmm

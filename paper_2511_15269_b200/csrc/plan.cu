@@ -1,0 +1,511 @@
+// plan.cu -- device-side hierarchy (median-split 2^s-tree) and interaction-list construction.
+//
+// Hierarchy: PAPER.md:40-43 and Listing 2.  The paper re-partitions every box with
+// argpartition at each of the s*L sub-splits; here each axis is radix-sorted ONCE by (coordinate, input index)
+// and the four orderings (x, y, z, index) are then stably partitioned per sub-split, so that
+//   * the tight bounding box of a node is read off the ends of its three sorted segments (no reduction pass),
+//   * the median is a direct lookup in the segment of the split axis,
+//   * ties are resolved by the total order (coordinate, input index) (reading S4),
+//   * leaves end up in ascending input index (final jnp.sort of Listing 2).
+// Which half receives the odd particle follows Listing 2's padding (DESIGN.md rule T3): with n_d the padded
+// row length at sub-depth d, the upper child takes the last floor(n_d/2) particles.
+//
+// Lists: PAPER.md:72-74 with criterion (4) PAPER.md:68-70, evaluated in non-contracted IEEE fp64.
+#include <algorithm>
+#include <climits>
+
+#include "primitives.cuh"
+
+namespace fmm {
+namespace {
+
+// ---------------------------------------------------------------------------------------------- keys
+__device__ inline uint32_t order_key(float x) {
+    if (x == 0.0f) x = 0.0f;  // -0 -> +0
+    const uint32_t b = __float_as_uint(x);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ inline uint64_t order_key(double x) {
+    if (x == 0.0) x = 0.0;
+    const uint64_t b = (uint64_t)__double_as_longlong(x);
+    return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+}
+
+template <typename T, typename KeyT>
+__global__ void make_keys_k(const T* pos, int64_t N, int axis, KeyT* keys, int32_t* vals, int* bad) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const T x = pos[3 * i + axis];
+    if (!isfinite(x)) *bad = 1;
+    keys[i] = order_key(x);
+    vals[i] = (int32_t)i;
+}
+
+__global__ void invert_perm_k(const int32_t* ord, int32_t* rank, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) rank[ord[i]] = (int32_t)i;
+}
+
+__global__ void iota_k(int32_t* a, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) a[i] = (int32_t)i;
+}
+
+// ---------------------------------------------------------------------------------------------- tree rounds
+struct OrdPtrs {
+    const int32_t* o[4];  // x, y, z, index orderings (particle ids, segmented by node)
+};
+
+// one thread per node of sub-depth d
+template <typename T>
+__global__ void node_k(const T* pos, OrdPtrs ord, const int32_t* rank0, const int32_t* rank1, const int32_t* rank2,
+                       const int32_t* nstart, const int32_t* ncnt, int64_t nnodes, int64_t n_d, int is_level, int is_last,
+                       int64_t box_off, int32_t* box_start, int32_t* box_count, T* box_lo, T* box_hi,
+                       int32_t* naxis, int32_t* npivot, int32_t* nstart2, int32_t* ncnt2) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nnodes) return;
+    const int32_t st = nstart[j], c = ncnt[j];
+    T lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    if (c > 0) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = pos[3 * (int64_t)ord.o[a][st] + a];
+            hi[a] = pos[3 * (int64_t)ord.o[a][st + c - 1] + a];
+        }
+    }
+    if (is_level) {
+        const int64_t g = box_off + j;
+        box_start[g] = st;
+        box_count[g] = c;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            box_lo[3 * g + a] = lo[a];
+            box_hi[3 * g + a] = hi[a];
+        }
+    }
+    if (is_last) return;
+    int32_t n_up = (int32_t)(n_d / 2);
+    if (n_up > c) n_up = c;
+    const int32_t n_lo = c - n_up;
+    int axis = 0;
+    if (c > 0) {  // longest extent in fp64, ties -> lowest axis (first maximum of jnp.argmax)
+        const double e0 = (double)hi[0] - (double)lo[0], e1 = (double)hi[1] - (double)lo[1], e2 = (double)hi[2] - (double)lo[2];
+        double eb = e0;
+        if (e1 > eb) { axis = 1; eb = e1; }
+        if (e2 > eb) { axis = 2; }
+    }
+    int32_t pivot = INT_MAX;
+    if (n_up > 0) {
+        const int32_t pt = ord.o[axis][st + n_lo];
+        pivot = (axis == 0 ? rank0 : axis == 1 ? rank1 : rank2)[pt];
+    }
+    naxis[j] = axis;
+    npivot[j] = pivot;
+    nstart2[2 * j] = st;
+    ncnt2[2 * j] = n_lo;
+    nstart2[2 * j + 1] = st + n_lo;
+    ncnt2[2 * j + 1] = n_up;
+}
+
+__global__ void pflag_k(const int32_t* pnode, const int32_t* rank0, const int32_t* rank1, const int32_t* rank2,
+                        const int32_t* naxis, const int32_t* npivot, uint8_t* pflag, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int32_t nd = pnode[i];
+    const int ax = naxis[nd];
+    const int32_t r = (ax == 0 ? rank0 : ax == 1 ? rank1 : rank2)[i];
+    pflag[i] = r >= npivot[nd] ? 1 : 0;
+}
+
+struct FlagLoad {
+    const uint8_t* pflag;
+    const int32_t* ord;
+    int64_t N;
+    __device__ int32_t operator()(int64_t i) const { return i < N ? (int32_t)pflag[ord[i]] : 0; }
+};
+
+__global__ void partition_k(const int32_t* ord_in, int32_t* ord_out, const int32_t* F, const uint8_t* pflag, const int32_t* pnode,
+                            const int32_t* nstart, const int32_t* nstart2, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int32_t pt = ord_in[i];
+    const int32_t nd = pnode[pt];
+    const int32_t s0 = nstart[nd];
+    const int32_t ups = F[i] - F[s0];  // flagged elements of this node before position i
+    int32_t dest;
+    if (pflag[pt]) dest = nstart2[2 * nd + 1] + ups;
+    else dest = nstart2[2 * nd] + ((int32_t)i - s0) - ups;
+    ord_out[dest] = pt;
+}
+
+__global__ void pnode_update_k(int32_t* pnode, const uint8_t* pflag, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) pnode[i] = 2 * pnode[i] + pflag[i];
+}
+
+// ---------------------------------------------------------------------------------------------- geometry (rule T6)
+template <typename T>
+__global__ void geometry_k(const T* lo, const T* hi, const int32_t* cnt, int64_t off, int64_t nb, int64_t off_parent, int s,
+                           double* ctr, double* rad, T* scale) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nb) return;
+    const int64_t g = off + b;
+    double d[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double l = (double)lo[3 * g + a], h = (double)hi[3 * g + a];
+        ctr[3 * g + a] = __dmul_rn(0.5, __dadd_rn(l, h));
+        d[a] = __dsub_rn(h, l);
+    }
+    const double r = __dmul_rn(0.5, __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]))));
+    rad[g] = r;
+    // expansion length scale: the radius, inherited from the parent for point-like boxes (any positive value is valid)
+    T sc = (T)r;
+    if (!(sc > (T)0)) sc = (off_parent >= 0) ? scale[off_parent + (b >> s)] : (T)1;
+    scale[g] = sc;
+    (void)cnt;
+}
+
+template <typename T>
+__global__ void gather_pos_k(const T* pos, const int32_t* perm, T* pos_tree, int64_t N) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int64_t i = perm[k];
+    pos_tree[3 * k] = pos[3 * i];
+    pos_tree[3 * k + 1] = pos[3 * i + 1];
+    pos_tree[3 * k + 2] = pos[3 * i + 2];
+}
+
+inline unsigned nblocks(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
+
+template <typename T, typename KeyT>
+void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
+    const int64_t N = P.N;
+    const int dmax = P.s * P.L;
+    const int64_t n_leaves = (int64_t)1 << dmax;
+    cudaEvent_t e0, e1, e2;
+    FMM_CUDA_CHECK(cudaEventCreate(&e0));
+    FMM_CUDA_CHECK(cudaEventCreate(&e1));
+    FMM_CUDA_CHECK(cudaEventCreate(&e2));
+    FMM_CUDA_CHECK(cudaEventRecord(e0, st));
+
+    DevBuf<KeyT> keys_a, keys_b;
+    DevBuf<int32_t> vals_b, hist, scan_scratch, rank[3], ordA[4], ordB[4], pnode, F;
+    DevBuf<uint8_t> pflag;
+    DevBuf<int> bad;
+    keys_a.alloc(N); keys_b.alloc(N); vals_b.alloc(N);
+    const int nblk = (int)((N + RS_TILE - 1) / RS_TILE);
+    hist.alloc((size_t)256 * nblk + 1);
+    scan_scratch.alloc((size_t)std::max(scan_scratch_elems((int64_t)256 * nblk), scan_scratch_elems(N + 1)));
+    for (int a = 0; a < 3; ++a) rank[a].alloc(N);
+    for (int a = 0; a < 4; ++a) { ordA[a].alloc(N); ordB[a].alloc(N); }
+    pnode.alloc(N); F.alloc(N + 1); pflag.alloc(N);
+    bad.alloc(1);
+    FMM_CUDA_CHECK(cudaMemsetAsync(bad.p, 0, sizeof(int), st));
+
+    // 1. three stable radix sorts by (coordinate, input index)
+    for (int a = 0; a < 3; ++a) {
+        make_keys_k<T, KeyT><<<nblocks(N, 256), 256, 0, st>>>(pos, N, a, keys_a.p, ordA[a].p, bad.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        const int where = radix_sort_pairs<KeyT>(keys_a.p, ordA[a].p, keys_b.p, vals_b.p, N, (int)sizeof(KeyT) * 8, hist.p, scan_scratch.p, st);
+        if (where == 1) FMM_CUDA_CHECK(cudaMemcpyAsync(ordA[a].p, vals_b.p, N * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        invert_perm_k<<<nblocks(N, 256), 256, 0, st>>>(ordA[a].p, rank[a].p, N);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    iota_k<<<nblocks(N, 256), 256, 0, st>>>(ordA[3].p, N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    int h_bad = 0;
+    FMM_CUDA_CHECK(cudaMemcpyAsync(&h_bad, bad.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    if (h_bad) {
+        set_error("positions contain non-finite values");
+        throw CudaFail{FMM_ERR_INVALID_ARG};
+    }
+    FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+
+    // 2. s*L rounds of stable partition
+    P.box_start.alloc(P.n_boxes); P.box_count.alloc(P.n_boxes);
+    P.box_lo.alloc(P.n_boxes * 3 * sizeof(T)); P.box_hi.alloc(P.n_boxes * 3 * sizeof(T));
+    DevBuf<int32_t> nstart[2], ncnt[2], naxis, npivot;
+    for (int k = 0; k < 2; ++k) { nstart[k].alloc(n_leaves); ncnt[k].alloc(n_leaves); }
+    naxis.alloc(n_leaves); npivot.alloc(n_leaves);
+    {
+        const int32_t z = 0, n32 = (int32_t)N;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(nstart[0].p, &z, 4, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(ncnt[0].p, &n32, 4, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaMemsetAsync(pnode.p, 0, N * sizeof(int32_t), st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    }
+    int32_t *oa[4], *ob[4];
+    for (int a = 0; a < 4; ++a) { oa[a] = ordA[a].p; ob[a] = ordB[a].p; }
+    int64_t n_d = N;
+    int cur = 0;
+    for (int d = 0; d <= dmax; ++d) {
+        const int64_t nnodes = (int64_t)1 << d;
+        const int is_level = (d % P.s == 0) ? 1 : 0;
+        const int is_last = (d == dmax) ? 1 : 0;
+        OrdPtrs op;
+        for (int a = 0; a < 4; ++a) op.o[a] = oa[a];
+        node_k<T><<<nblocks(nnodes, 128), 128, 0, st>>>(pos, op, rank[0].p, rank[1].p, rank[2].p, nstart[cur].p, ncnt[cur].p, nnodes, n_d,
+                                                        is_level, is_last, is_level ? P.level_off[d / P.s] : 0, P.box_start.p, P.box_count.p,
+                                                        (T*)P.box_lo.p, (T*)P.box_hi.p, naxis.p, npivot.p, nstart[cur ^ 1].p, ncnt[cur ^ 1].p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        if (is_last) break;
+        pflag_k<<<nblocks(N, 256), 256, 0, st>>>(pnode.p, rank[0].p, rank[1].p, rank[2].p, naxis.p, npivot.p, pflag.p, N);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        for (int a = 0; a < 4; ++a) {
+            exclusive_scan<int32_t, FlagLoad>(FlagLoad{pflag.p, oa[a], N}, F.p, N + 1, scan_scratch.p, st);
+            partition_k<<<nblocks(N, 256), 256, 0, st>>>(oa[a], ob[a], F.p, pflag.p, pnode.p, nstart[cur].p, nstart[cur ^ 1].p, N);
+            FMM_CUDA_CHECK(cudaGetLastError());
+            std::swap(oa[a], ob[a]);
+        }
+        pnode_update_k<<<nblocks(N, 256), 256, 0, st>>>(pnode.p, pflag.p, N);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        n_d = (n_d + 1) / 2;
+        cur ^= 1;
+    }
+    P.max_leaf = (int)n_d;
+    P.perm.alloc(N);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(P.perm.p, oa[3], N * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+
+    // 3. geometry, top-down (scale inherits from the parent)
+    P.box_ctr.alloc(P.n_boxes * 3); P.box_rad.alloc(P.n_boxes); P.box_scale.alloc(P.n_boxes * sizeof(T));
+    for (int l = 0; l <= P.L; ++l) {
+        const int64_t nb = (int64_t)1 << (P.s * l);
+        geometry_k<T><<<nblocks(nb, 128), 128, 0, st>>>((const T*)P.box_lo.p, (const T*)P.box_hi.p, P.box_count.p, P.level_off[l], nb,
+                                                        l > 0 ? P.level_off[l - 1] : -1, P.s, P.box_ctr.p, P.box_rad.p, (T*)P.box_scale.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    P.pos_tree.alloc(N * 3 * sizeof(T));
+    gather_pos_k<T><<<nblocks(N, 256), 256, 0, st>>>(pos, P.perm.p, (T*)P.pos_tree.p, N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    FMM_CUDA_CHECK(cudaEventRecord(e2, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    float ms1 = 0, ms2 = 0;
+    cudaEventElapsedTime(&ms1, e0, e1);
+    cudaEventElapsedTime(&ms2, e1, e2);
+    P.plan_ms[0] = ms1;
+    P.plan_ms[1] = ms2;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
+}
+
+// ---------------------------------------------------------------------------------------------- lists
+// eq. (4) PAPER.md:68-70 (rule L1): R + theta*r < theta*d, strict, IEEE fp64 without contraction.
+__device__ inline bool admissible(const double* ctr, const double* rad, int64_t ga, int64_t gb, double theta) {
+    const double ra = rad[ga], rb = rad[gb];
+    const double R = fmax(ra, rb), r = fmin(ra, rb);
+    const double dx = __dsub_rn(ctr[3 * ga], ctr[3 * gb]);
+    const double dy = __dsub_rn(ctr[3 * ga + 1], ctr[3 * gb + 1]);
+    const double dz = __dsub_rn(ctr[3 * ga + 2], ctr[3 * gb + 2]);
+    const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+    return __dadd_rn(R, __dmul_rn(theta, r)) < __dmul_rn(theta, d);
+}
+
+struct ExpandArgs {
+    const int32_t *ftgt, *fsrc;  // failing pairs of the parent level (level-local indices), sorted by (tgt, src)
+    const int64_t* foff;         // CSR offsets of the failing pairs by parent target
+    int64_t nfail;
+    int s;
+    int64_t off_child;           // global id offset of the child level
+    const int32_t* box_count;
+    const double *ctr, *rad;
+    double theta;
+};
+
+__device__ inline void expand_decode(const ExpandArgs& A, int64_t idx, int64_t& pos, int32_t& t, int32_t& sc) {
+    const int nch = 1 << A.s, nch2 = nch * nch;
+    const int64_t e = idx / nch2;
+    const int ij = (int)(idx - e * nch2);
+    const int i = ij >> A.s, j = ij & (nch - 1);
+    const int32_t a = A.ftgt[e], b = A.fsrc[e];
+    const int64_t row0 = A.foff[a], rowlen = A.foff[a + 1] - row0;
+    pos = row0 * nch2 + (int64_t)i * (rowlen * nch) + (e - row0) * nch + j;
+    t = a * nch + i;
+    sc = b * nch + j;
+}
+
+// codes: 0 = dropped (empty box), 1 = weak (admissible), 2 = fail (to be refined / strong)
+__global__ void expand_classify_k(ExpandArgs A, uint8_t* codes) {
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t total = A.nfail << (2 * A.s);
+    if (idx >= total) return;
+    int64_t pos; int32_t t, sc;
+    expand_decode(A, idx, pos, t, sc);
+    const int64_t gt = A.off_child + t, gs = A.off_child + sc;
+    uint8_t code = 0;
+    if (A.box_count[gt] > 0 && A.box_count[gs] > 0) code = admissible(A.ctr, A.rad, gt, gs, A.theta) ? 1 : 2;
+    codes[pos] = code;
+}
+
+struct CodeLoad {
+    const uint8_t* codes;
+    int64_t n;
+    __device__ unsigned long long operator()(int64_t i) const {
+        if (i >= n) return 0ull;
+        const uint8_t c = codes[i];
+        return c == 1 ? 1ull : (c == 2 ? (1ull << 32) : 0ull);
+    }
+};
+
+__global__ void expand_compact_k(ExpandArgs A, const uint8_t* codes, const unsigned long long* S, int32_t* wtgt, int32_t* wsrc,
+                                 int32_t* ftgt2, int32_t* fsrc2) {
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t total = A.nfail << (2 * A.s);
+    if (idx >= total) return;
+    int64_t pos; int32_t t, sc;
+    expand_decode(A, idx, pos, t, sc);
+    const uint8_t c = codes[pos];
+    const unsigned long long sv = S[pos];
+    if (c == 1) {
+        const int64_t o = (int64_t)(sv & 0xffffffffull);
+        wtgt[o] = (int32_t)(A.off_child + t);
+        wsrc[o] = (int32_t)(A.off_child + sc);
+    } else if (c == 2) {
+        const int64_t o = (int64_t)(sv >> 32);
+        ftgt2[o] = t;
+        fsrc2[o] = sc;
+    }
+}
+
+// row offsets of the child level: thread per child target (+1 for the end)
+__global__ void expand_offsets_k(ExpandArgs A, const unsigned long long* S, int64_t nb_child, int64_t total, int64_t weak_base,
+                                 int64_t* weak_off_global, int64_t* foff2) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > nb_child) return;
+    int64_t base;
+    if (t == nb_child) base = total;
+    else {
+        const int nch = 1 << A.s;
+        const int64_t a = t >> A.s;
+        const int i = (int)(t & (nch - 1));
+        const int64_t row0 = A.foff[a], rowlen = A.foff[a + 1] - row0;
+        base = row0 * nch * nch + (int64_t)i * rowlen * nch;
+    }
+    const unsigned long long sv = S[base];
+    weak_off_global[A.off_child + t] = weak_base + (int64_t)(sv & 0xffffffffull);
+    foff2[t] = (int64_t)(sv >> 32);
+}
+
+__global__ void count_p2p_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_cnt, int64_t n_leaves, unsigned long long* out) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long acc = 0;
+    if (t < n_leaves) {
+        unsigned long long ssum = 0;
+        for (int64_t e = soff[t]; e < soff[t + 1]; ++e) ssum += (unsigned long long)leaf_cnt[ssrc[e]];
+        acc = ssum * (unsigned long long)leaf_cnt[t];
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if ((threadIdx.x & 31) == 0 && acc) atomicAdd(out, acc);
+}
+
+}  // namespace
+
+void build_tree(Plan& P, const void* d_positions, cudaStream_t st) {
+    if (P.dtype == FMM_F32) build_tree_t<float, uint32_t>(P, (const float*)d_positions, st);
+    else build_tree_t<double, uint64_t>(P, (const double*)d_positions, st);
+}
+
+void build_lists(Plan& P, cudaStream_t st) {
+    cudaEvent_t e0, e1;
+    FMM_CUDA_CHECK(cudaEventCreate(&e0));
+    FMM_CUDA_CHECK(cudaEventCreate(&e1));
+    FMM_CUDA_CHECK(cudaEventRecord(e0, st));
+    const int s = P.s, L = P.L;
+    P.weak_off.alloc(P.n_boxes + 1);
+    FMM_CUDA_CHECK(cudaMemsetAsync(P.weak_off.p, 0, (P.n_boxes + 1) * sizeof(int64_t), st));
+    P.weak_level_off.assign(L + 2, 0);
+
+    // level 0: the pair (root, root) always fails eq. (4) (d = 0)
+    DevBuf<int32_t> ftgt, fsrc;
+    DevBuf<int64_t> foff;
+    ftgt.alloc(1); fsrc.alloc(1); foff.alloc(2);
+    {
+        const int32_t z = 0;
+        const int64_t o[2] = {0, 1};
+        FMM_CUDA_CHECK(cudaMemcpyAsync(ftgt.p, &z, 4, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(fsrc.p, &z, 4, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(foff.p, o, 16, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    }
+    int64_t nfail = 1;
+    std::vector<DevBuf<int32_t>> wt(L + 1), ws(L + 1);
+    std::vector<int64_t> wn(L + 1, 0);
+    int64_t weak_base = 0;
+    for (int l = 1; l <= L; ++l) {
+        const int64_t nb_child = (int64_t)1 << (s * l);
+        const int64_t total = nfail << (2 * s);
+        ExpandArgs A{ftgt.p, fsrc.p, foff.p, nfail, s, P.level_off[l], P.box_count.p, P.box_ctr.p, P.box_rad.p, P.theta};
+        DevBuf<uint8_t> codes;
+        DevBuf<unsigned long long> S, scr;
+        codes.alloc(total + 1);
+        S.alloc(total + 1);
+        scr.alloc(scan_scratch_elems(total + 1));
+        if (total > 0) {
+            expand_classify_k<<<nblocks(total, 256), 256, 0, st>>>(A, codes.p);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+        exclusive_scan<unsigned long long, CodeLoad>(CodeLoad{codes.p, total}, S.p, total + 1, scr.p, st);
+        unsigned long long tot = 0;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&tot, S.p + total, sizeof(tot), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        const int64_t nweak_l = (int64_t)(tot & 0xffffffffull), nfail2 = (int64_t)(tot >> 32);
+        if (nweak_l >= 0xffffffffll || nfail2 >= 0xffffffffll) {
+            set_error("interaction list of one level exceeds 2^32-1 pairs");
+            throw CudaFail{FMM_ERR_UNSUPPORTED};
+        }
+        wt[l].alloc(nweak_l); ws[l].alloc(nweak_l); wn[l] = nweak_l;
+        DevBuf<int32_t> ftgt2, fsrc2;
+        DevBuf<int64_t> foff2;
+        ftgt2.alloc(nfail2); fsrc2.alloc(nfail2); foff2.alloc(nb_child + 1);
+        if (total > 0) {
+            expand_compact_k<<<nblocks(total, 256), 256, 0, st>>>(A, codes.p, S.p, wt[l].p, ws[l].p, ftgt2.p, fsrc2.p);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+        expand_offsets_k<<<nblocks(nb_child + 1, 256), 256, 0, st>>>(A, S.p, nb_child, total, weak_base, P.weak_off.p, foff2.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        weak_base += nweak_l;
+        P.weak_level_off[l + 1] = weak_base;
+        std::swap(ftgt.p, ftgt2.p); std::swap(ftgt.n, ftgt2.n);
+        std::swap(fsrc.p, fsrc2.p); std::swap(fsrc.n, fsrc2.n);
+        std::swap(foff.p, foff2.p); std::swap(foff.n, foff2.n);
+        nfail = nfail2;
+    }
+    // the expand_offsets kernel wrote weak_off[off_l + t] for t = 0..nb_l (the entry t = nb_l is the next level's first row
+    // or the final end); level 0 rows are zero.  Make sure the final end is set when L == 0.
+    P.n_weak = weak_base;
+    if (L == 0) P.weak_level_off[1] = 0;
+    {
+        const int64_t endv = weak_base;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.weak_off.p + P.n_boxes, &endv, sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    }
+    P.weak_src.alloc(P.n_weak); P.weak_tgt.alloc(P.n_weak);
+    for (int l = 1; l <= L; ++l) {
+        if (!wn[l]) continue;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.weak_tgt.p + P.weak_level_off[l], wt[l].p, wn[l] * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.weak_src.p + P.weak_level_off[l], ws[l].p, wn[l] * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    }
+    // strong list = failing pairs of the leaf level (rule L3), already CSR by target leaf
+    P.n_strong = nfail;
+    P.strong_off.alloc(P.n_leaves + 1);
+    P.strong_src.alloc(nfail);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_off.p, foff.p, (P.n_leaves + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
+    FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_src.p, fsrc.p, nfail * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    DevBuf<unsigned long long> cnt;
+    cnt.alloc(1);
+    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 8, st));
+    count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], P.n_leaves, cnt.p);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    unsigned long long h = 0;
+    FMM_CUDA_CHECK(cudaMemcpyAsync(&h, cnt.p, 8, cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    P.n_p2p_pairs = (int64_t)h;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    P.plan_ms[2] = ms;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+}
+
+}  // namespace fmm

@@ -1,0 +1,212 @@
+"""Thin Python binding of include/fmm.h (argument marshalling only; every step runs in the CUDA library).
+
+Loads the in-tree library paper_2511_15269_b200/libfmm_b200.so and FAILS LOUDLY if it is missing -- there
+is no CPU or PyTorch fallback.  PyTorch is used only for device memory (tensor.data_ptr()) and streams.
+Function names mirror the C entry points; `Plan` is a small convenience wrapper around them.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfmm_b200.so")
+
+FMM_OK, FMM_ERR_INVALID_ARG, FMM_ERR_ALLOC, FMM_ERR_CUDA, FMM_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
+FMM_F32, FMM_F64 = 0, 1
+FMM_P_MAX = 16
+
+EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
+           "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_last_error",
+           "fmm_version"]
+
+
+class fmm_admissibility(C.Structure):
+    _fields_ = [("theta", C.c_double), ("cross_level", C.c_int)]
+
+
+class FmmError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("fmm status %d: %s" % (status, msg))
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises ImportError if the CUDA extension has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("CUDA library %s is missing: run `python -m paper_2511_15269_b200.build` (no fallback exists)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        vp, i64p, i32p, dp = C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32), C.POINTER(C.c_double)
+        L.fmm_plan_create.argtypes = [vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
+        L.fmm_evaluate.argtypes = [vp, vp, vp, vp, vp]
+        L.fmm_evaluate_host.argtypes = [vp, vp, vp, vp, vp]
+        L.fmm_evaluate_profiled.argtypes = [vp, vp, vp, vp, vp, dp]
+        L.fmm_plan_destroy.argtypes = [vp]
+        L.fmm_plan_info.argtypes = [vp, C.POINTER(C.c_int), i64p, i64p, i64p, i64p, i64p]
+        L.fmm_plan_copy_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
+        L.fmm_plan_copy_lists.argtypes = [vp, i64p, i32p, i64p, i32p]
+        L.fmm_plan_timings.argtypes = [vp, dp]
+        L.fmm_plan_set_m2l_variant.argtypes = [vp, C.c_int]
+        L.fmm_last_error.restype = C.c_char_p
+        L.fmm_version.restype = C.c_char_p
+        for name in EXPORTS:
+            if getattr(L, name).restype is C.c_int:
+                pass
+        _lib = L
+    return _lib
+
+
+def fmm_last_error():
+    return lib().fmm_last_error().decode()
+
+
+def fmm_version():
+    return lib().fmm_version().decode()
+
+
+def _check(st):
+    if st != FMM_OK:
+        raise FmmError(st, fmm_last_error())
+
+
+def _dtype_code(t):
+    import torch
+    if t.dtype == torch.float32:
+        return FMM_F32
+    if t.dtype == torch.float64:
+        return FMM_F64
+    raise TypeError("positions/charges must be float32 or float64")
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def fmm_plan_create(positions, p, N_max, s, theta=0.77, cross_level=0, stream=None):
+    """positions: CUDA tensor (N,3), contiguous, float32/float64.  Returns an opaque plan handle (c_void_p)."""
+    if not positions.is_cuda or not positions.is_contiguous() or positions.dim() != 2 or positions.shape[1] != 3:
+        raise ValueError("positions must be a contiguous CUDA tensor of shape (N,3)")
+    adm = fmm_admissibility(float(theta), int(cross_level))
+    h = C.c_void_p()
+    _check(lib().fmm_plan_create(C.c_void_p(positions.data_ptr()), positions.shape[0], int(p), int(N_max), int(s), C.byref(adm),
+                                 _dtype_code(positions), _stream_ptr(stream), C.byref(h)))
+    return h
+
+
+def fmm_plan_destroy(plan):
+    _check(lib().fmm_plan_destroy(plan))
+
+
+def fmm_evaluate(plan, charges, potential=None, field=None, stream=None):
+    """charges (N,), potential (N,) or None, field (N,3) or None: contiguous CUDA tensors of the plan's dtype."""
+    for t in (charges, potential, field):
+        if t is not None and (not t.is_cuda or not t.is_contiguous()):
+            raise ValueError("tensors must be contiguous CUDA tensors")
+    _check(lib().fmm_evaluate(plan, C.c_void_p(charges.data_ptr()), C.c_void_p(potential.data_ptr()) if potential is not None else None,
+                              C.c_void_p(field.data_ptr()) if field is not None else None, _stream_ptr(stream)))
+
+
+def fmm_evaluate_profiled(plan, charges, potential=None, field=None, stream=None):
+    ms = (C.c_double * 8)()
+    _check(lib().fmm_evaluate_profiled(plan, C.c_void_p(charges.data_ptr()), C.c_void_p(potential.data_ptr()) if potential is not None else None,
+                                       C.c_void_p(field.data_ptr()) if field is not None else None, _stream_ptr(stream), ms))
+    names = ["permute", "p2m", "m2m", "m2l", "l2l", "l2p", "p2p", "total"]
+    return dict(zip(names, list(ms)))
+
+
+def fmm_evaluate_host(plan, h_charges, h_potential=None, h_field=None, stream=None):
+    """Host-buffer path: numpy arrays or pinned CPU tensors; H2D and D2H copies happen inside the call."""
+    def ptr(a):
+        if a is None:
+            return None
+        if isinstance(a, np.ndarray):
+            return C.c_void_p(a.ctypes.data)
+        return C.c_void_p(a.data_ptr())
+    _check(lib().fmm_evaluate_host(plan, ptr(h_charges), ptr(h_potential), ptr(h_field), _stream_ptr(stream)))
+
+
+def fmm_plan_info(plan):
+    L = C.c_int()
+    v = [C.c_int64() for _ in range(5)]
+    _check(lib().fmm_plan_info(plan, C.byref(L), *[C.byref(x) for x in v]))
+    return dict(L=L.value, n_boxes=v[0].value, n_leaves=v[1].value, n_weak=v[2].value, n_strong=v[3].value, n_p2p_pairs=v[4].value)
+
+
+def fmm_plan_timings(plan):
+    ms = (C.c_double * 4)()
+    _check(lib().fmm_plan_timings(plan, ms))
+    return dict(sort=ms[0], tree=ms[1], lists=ms[2], total=ms[3])
+
+
+def fmm_plan_set_m2l_variant(plan, variant):
+    _check(lib().fmm_plan_set_m2l_variant(plan, int(variant)))
+
+
+def fmm_plan_copy_tree(plan, N, dtype):
+    info = fmm_plan_info(plan)
+    nb = info["n_boxes"]
+    fl = np.float32 if dtype == FMM_F32 else np.float64
+    t = dict(perm=np.empty(N, np.int32), box_start=np.empty(nb, np.int32), box_count=np.empty(nb, np.int32), lo=np.empty((nb, 3), fl),
+             hi=np.empty((nb, 3), fl), ctr=np.empty((nb, 3), np.float64), rad=np.empty(nb, np.float64))
+    i32p, dp = C.POINTER(C.c_int32), C.POINTER(C.c_double)
+    _check(lib().fmm_plan_copy_tree(plan, t["perm"].ctypes.data_as(i32p), t["box_start"].ctypes.data_as(i32p), t["box_count"].ctypes.data_as(i32p),
+                                    C.c_void_p(t["lo"].ctypes.data), C.c_void_p(t["hi"].ctypes.data), t["ctr"].ctypes.data_as(dp),
+                                    t["rad"].ctypes.data_as(dp)))
+    return t
+
+
+def fmm_plan_copy_lists(plan):
+    info = fmm_plan_info(plan)
+    ls = dict(weak_off=np.empty(info["n_boxes"] + 1, np.int64), weak_src=np.empty(info["n_weak"], np.int32),
+              strong_off=np.empty(info["n_leaves"] + 1, np.int64), strong_src=np.empty(info["n_strong"], np.int32))
+    i32p, i64p = C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    _check(lib().fmm_plan_copy_lists(plan, ls["weak_off"].ctypes.data_as(i64p), ls["weak_src"].ctypes.data_as(i32p),
+                                     ls["strong_off"].ctypes.data_as(i64p), ls["strong_src"].ctypes.data_as(i32p)))
+    return ls
+
+
+class Plan:
+    """gen_hierarchy(...) / eval_potential(...) of Listing 1 as an object: build once, evaluate many."""
+
+    def __init__(self, positions, p, N_max, s, theta=0.77, stream=None):
+        self.N = positions.shape[0]
+        self.dtype = _dtype_code(positions)
+        self.tdtype = positions.dtype
+        self.device = positions.device
+        self.p, self.N_max, self.s, self.theta = p, N_max, s, theta
+        self.handle = fmm_plan_create(positions, p, N_max, s, theta, 0, stream)
+        self.info = fmm_plan_info(self.handle)
+
+    def evaluate(self, charges, want_potential=True, want_field=True, stream=None):
+        import torch
+        pot = torch.empty(self.N, dtype=self.tdtype, device=self.device) if want_potential else None
+        fld = torch.empty((self.N, 3), dtype=self.tdtype, device=self.device) if want_field else None
+        fmm_evaluate(self.handle, charges, pot, fld, stream)
+        return pot, fld
+
+    def tree(self):
+        return fmm_plan_copy_tree(self.handle, self.N, self.dtype)
+
+    def lists(self):
+        return fmm_plan_copy_lists(self.handle)
+
+    def timings(self):
+        return fmm_plan_timings(self.handle)
+
+    def close(self):
+        if self.handle is not None:
+            fmm_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
