@@ -1,0 +1,244 @@
+"""GPU parity tests proper: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded inputs.
+
+Acceptance (BASELINE.json north_star): hierarchy and interaction lists bit-exact; rel-L2(GPU - oracle) <= 1e-5 (fp32) and
+<= 1e-11 (fp64) on potential and on field at equal p; error against the O(N^2) definition within 1.5x the oracle's own.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import api as O
+from paper_2511_15269_b200 import fmm, inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {np.float32: 1e-5, np.float64: 1e-11}  # north_star tolerances, rel-L2 GPU vs oracle
+
+
+def rel2(a, b):
+    return np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b)
+
+
+def gpu_plan(pos, p, N_max, s, theta=0.77):
+    tp = torch.from_numpy(np.ascontiguousarray(pos)).cuda()
+    return fmm.Plan(tp, p, N_max, s, theta)
+
+
+def gpu_eval(P, q):
+    tq = torch.from_numpy(np.ascontiguousarray(q)).cuda()
+    u, f = P.evaluate(tq)
+    torch.cuda.synchronize()
+    return u.cpu().numpy(), f.cpu().numpy()
+
+
+def assert_same_hierarchy(P, Po, dtype):
+    """bit-exact: permutation, box ranges, tight boxes, fp64 centres/radii, both lists in canonical CSR form."""
+    tg, to = P.tree(), Po.tree()
+    info = P.info
+    assert (info["L"], info["n_boxes"], info["n_leaves"]) == (Po.L, Po.n_boxes, Po.n_leaves)
+    assert np.array_equal(tg["perm"].astype(np.int64), to["perm"])
+    assert np.array_equal(tg["box_count"].astype(np.int64), to["box_count"])
+    ne = to["box_count"] > 0
+    assert np.array_equal(tg["box_start"].astype(np.int64)[ne], to["box_start"][ne])
+    assert np.array_equal(tg["lo"].astype(np.float64)[ne], to["lo"][ne])
+    assert np.array_equal(tg["hi"].astype(np.float64)[ne], to["hi"][ne])
+    assert np.array_equal(tg["ctr"][ne], to["ctr"][ne])  # fp64, no FMA contraction on either side (rule T6)
+    assert np.array_equal(tg["rad"][ne], to["rad"][ne])
+    lg, lo_ = P.lists(), Po.lists()
+    assert (info["n_weak"], info["n_strong"], info["n_p2p_pairs"]) == (Po.n_weak, Po.n_strong, Po.n_p2p_pairs)
+    assert np.array_equal(lg["weak_off"], lo_["weak_off"])
+    assert np.array_equal(lg["weak_src"].astype(np.int64), lo_["weak_src"])
+    assert np.array_equal(lg["strong_off"], lo_["strong_off"])
+    assert np.array_equal(lg["strong_src"].astype(np.int64), lo_["strong_src"])
+
+
+def run_case(pos, q, p, N_max, s, theta=0.77, direct=True):
+    dt = pos.dtype.type
+    P = gpu_plan(pos, p, N_max, s, theta)
+    Po = O.Plan(pos, p, N_max, s, theta)
+    assert_same_hierarchy(P, Po, dt)
+    u, f = gpu_eval(P, q)
+    uo, fo = Po.evaluate(q)
+    assert np.all(np.isfinite(u)) and np.all(np.isfinite(f))
+    eu, ef = rel2(u, uo), rel2(f, fo)
+    assert eu <= TOL[dt] and ef <= TOL[dt], (eu, ef)
+    if direct:
+        ud, fd = O.direct(pos, q)
+        assert rel2(u, ud) <= 1.5 * rel2(uo, ud) + 1e-14
+        assert rel2(f, fd) <= 1.5 * rel2(fo, fd) + 1e-14
+    P.close()
+    return eu, ef
+
+
+# ------------------------------------------------------------------------------------------- BASELINE config 1
+def test_config1_fp64():
+    pos, q, c = inputs.make("cfg1_cube4096_f64")
+    run_case(pos, q, c["p"], c["N_max"], c["s"], c["theta"])
+
+
+def test_config1_shape_fp32():
+    pos, q = inputs.uniform_cube(4096, 1, np.float32)
+    run_case(pos, q, 6, 64, 3)
+
+
+# ------------------------------------------------------------------------------------------- deep trees (M2M / L2L carry weight)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("N,N_max,s,p", [(1024, 16, 1, 6), (4096, 8, 3, 4), (3000, 20, 2, 8), (5000, 40, 1, 5)])
+def test_deep_trees(dtype, N, N_max, s, p):
+    pos, q = inputs.uniform_cube(N, 7, dtype)
+    run_case(pos, q, p, N_max, s)
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("p", [0, 1, 2, 3, 7, 10, 12])
+def test_orders(dtype, p):
+    pos, q = inputs.uniform_cube(2500, 11, dtype)
+    run_case(pos, q, p, 32, 2)
+
+
+@pytest.mark.parametrize("theta", [0.3, 0.5, 0.9])
+def test_theta(theta):
+    pos, q = inputs.uniform_cube(3000, 12, np.float64)
+    run_case(pos, q, 6, 24, 3, theta)
+
+
+# ------------------------------------------------------------------------------------------- other point distributions
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_sphere_surface(dtype):
+    pos, q = inputs.sphere_surface(6000, 21, dtype)
+    run_case(pos, q, 8, 32, 3)
+
+
+@pytest.mark.parametrize("dtype,s", [(np.float64, 3), (np.float32, 3), (np.float32, 1)])
+def test_clusters(dtype, s):
+    pos, q = inputs.gaussian_clusters(20000, 3, dtype)
+    run_case(pos, q, 8, 48, s)
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_thin_film_lattice_all_ties(dtype):
+    """config-4 shape at reduced size: every coordinate is tied many times (reading S4 decides the tree)."""
+    pos, q = inputs.thin_film(64, 48, 4, 4, dtype)
+    run_case(pos, q, 6, 16, 3)
+
+
+# ------------------------------------------------------------------------------------------- degenerate inputs
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("N,N_max,s", [(1, 4, 3), (2, 1, 1), (5, 8, 3), (7, 1, 3), (9, 1, 2), (100, 128, 3), (129, 128, 3), (1000, 1, 1)])
+def test_tiny_and_ragged(dtype, N, N_max, s):
+    """L = 0 (root only, all P2P), N < 2^(sL) (empty boxes, rule T5), one particle per leaf."""
+    pos, q = inputs.uniform_cube(N, 100 + N, dtype)
+    P = gpu_plan(pos, 4, N_max, s)
+    Po = O.Plan(pos, 4, N_max, s)
+    assert_same_hierarchy(P, Po, dtype)
+    u, f = gpu_eval(P, q)
+    uo, fo = Po.evaluate(q)
+    if N == 1:
+        assert u[0] == 0 and np.all(f == 0)
+    else:
+        assert rel2(u, uo) <= TOL[dtype] and rel2(f, fo) <= TOL[dtype]
+    P.close()
+
+
+def test_coincident_points_contribute_nothing():
+    """reading S3: zero-distance pairs are skipped (potential and field stay finite)."""
+    pos, q = inputs.uniform_cube(600, 5, np.float64)
+    pos[100:140] = pos[0:40]
+    run_case(pos, q, 5, 16, 2)
+
+
+def test_collinear_and_planar_points():
+    """boxes with zero extent along one or two axes; translations along +-z and in the xy-plane (reading S7)."""
+    rng = np.random.default_rng(9)
+    z = np.zeros((800, 3))
+    z[:, 2] = rng.random(800)
+    run_case(z, rng.uniform(-1, 1, 800), 6, 16, 1)
+    xy = rng.random((1500, 3))
+    xy[:, 2] = 0.25
+    run_case(xy, rng.uniform(-1, 1, 1500), 6, 16, 2)
+
+
+def test_small_and_large_length_scales_fp32():
+    """hard part 1 of DESIGN.md: unscaled fp32 coefficients would overflow/underflow; the scaled representation must not."""
+    for scale in (1e-4, 1.0, 1e4):
+        pos, q = inputs.uniform_cube(4000, 13, np.float64)
+        pos = (pos * scale).astype(np.float32)
+        run_case(pos, q.astype(np.float32), 8, 16, 3)
+
+
+def test_plan_reuse_and_linearity():
+    """one hierarchy, many charge vectors; the evaluate is linear in q."""
+    pos, q1 = inputs.uniform_cube(3000, 30, np.float64)
+    _, q2 = inputs.uniform_cube(3000, 31, np.float64)
+    P = gpu_plan(pos, 6, 32, 3)
+    u1, f1 = gpu_eval(P, q1)
+    u2, f2 = gpu_eval(P, q2)
+    u3, f3 = gpu_eval(P, 2.0 * q1 - 3.0 * q2)
+    assert rel2(u3, 2.0 * u1 - 3.0 * u2) < 1e-12 and rel2(f3, 2.0 * f1 - 3.0 * f2) < 1e-12
+    u1b, f1b = gpu_eval(P, q1)
+    assert np.array_equal(u1, u1b) and np.array_equal(f1, f1b)  # deterministic
+    P.close()
+
+
+def test_potential_only_and_field_only_and_host_path():
+    pos, q = inputs.uniform_cube(2000, 33, np.float32)
+    P = gpu_plan(pos, 5, 32, 3)
+    u, f = gpu_eval(P, q)
+    tq = torch.from_numpy(q).cuda()
+    u2, none = P.evaluate(tq, want_field=False)
+    none2, f2 = P.evaluate(tq, want_potential=False)
+    torch.cuda.synchronize()
+    assert none is None and none2 is None
+    assert np.array_equal(u2.cpu().numpy(), u) and np.array_equal(f2.cpu().numpy(), f)
+    hu, hf = np.empty_like(u), np.empty_like(f)
+    fmm.fmm_evaluate_host(P.handle, q, hu, hf)
+    assert np.array_equal(hu, u) and np.array_equal(hf, f)
+    P.close()
+
+
+def test_non_finite_positions_are_rejected():
+    pos, _ = inputs.uniform_cube(100, 1, np.float32)
+    pos[17, 1] = np.nan
+    with pytest.raises(fmm.FmmError) as e:
+        gpu_plan(pos, 4, 16, 2)
+    assert e.value.status == fmm.FMM_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------- full-size configs (sampled oracle)
+def sampled_case(name, n_sample_leaves=12, seed=0):
+    """BASELINE full-size configs in the configuration bench.py times: hierarchy/lists bit-exact on everything;
+    potential/field compared on the particles of a random sample of leaves (the oracle computes exactly those,
+    with the same arithmetic as a full run) and against the O(N^2) definition on the same particles."""
+    pos, q, c = inputs.make(name)
+    dt = pos.dtype.type
+    P = gpu_plan(pos, c["p"], c["N_max"], c["s"], c["theta"])
+    Po = O.Plan(pos, c["p"], c["N_max"], c["s"], c["theta"])
+    assert_same_hierarchy(P, Po, dt)
+    u, f = gpu_eval(P, q)
+    assert np.all(np.isfinite(u)) and np.all(np.isfinite(f))
+    rng = np.random.default_rng(seed)
+    mask = np.zeros(Po.n_leaves, np.uint8)
+    mask[rng.choice(Po.n_leaves, n_sample_leaves, replace=False)] = 1
+    uo, fo = Po.evaluate(q, leaf_mask=mask)
+    sel = np.flatnonzero(np.isfinite(uo))
+    assert sel.size > 0
+    eu, ef = rel2(u[sel], uo[sel]), rel2(f[sel], fo[sel])
+    assert eu <= TOL[dt] and ef <= TOL[dt], (eu, ef)
+    ud, fd = O.direct(pos, q, sel)
+    assert rel2(u[sel], ud) <= 1.5 * rel2(uo[sel], ud)
+    assert rel2(f[sel], fd) <= 1.5 * rel2(fo[sel], fd)
+    P.close()
+
+
+def test_config2_full_size_sampled():
+    sampled_case("cfg2_cube1M_f32")
+
+
+@pytest.mark.parametrize("name", ["cfg3_clusters1M_f32_s3", "cfg3_clusters1M_f32_s1"])
+def test_config3_full_size_sampled(name):
+    sampled_case(name, n_sample_leaves=8)
+
+
+def test_config4_full_size_sampled():
+    sampled_case("cfg4_film_f32", n_sample_leaves=24)
