@@ -111,6 +111,10 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
  * 0 = automatic (unrolled register kernel when available for (p, dtype), else generic), 1 = force generic. */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
+/* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M
+ * and one L2L per level, M2L (when the weak list is not empty), L2P, P2P.  cudaMemset nodes are not counted. */
+fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h_launches_per_evaluate);
+
 /* Thread-local, NUL-terminated description of the last failure on the calling thread ("" if none). */
 const char* fmm_last_error(void);
 

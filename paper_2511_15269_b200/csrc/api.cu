@@ -221,6 +221,12 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms) {
     return FMM_OK;
 }
 
+fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h) {
+    if (!plan || !h) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+    *h = evaluate_launches(plan->P);
+    return FMM_OK;
+}
+
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {
     if (!plan || variant < 0 || variant > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
     plan->P.m2l_variant = variant;

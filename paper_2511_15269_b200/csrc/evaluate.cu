@@ -558,6 +558,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
 
 }  // namespace
 
+int64_t evaluate_launches(const Plan& P) { return 4 + 2 * (int64_t)P.L + (P.n_weak > 0 ? 1 : 0); }
+
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
     if (!g_const_uploaded) {
         const Tables& tb = tables();

@@ -103,6 +103,7 @@ void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
 void build_lists(Plan& P, cudaStream_t st);
 // evaluate.cu
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
+int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evaluate
 // m2l_fast.cu: returns false if no unrolled kernel exists for (p, dtype)
 bool m2l_fast_available(int p, fmm_dtype dt);
 void m2l_fast_launch(const Plan& P, cudaStream_t st);
