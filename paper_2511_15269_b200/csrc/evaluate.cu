@@ -2,7 +2,7 @@
 //   permute charges -> P2M (eq. 13) -> M2M (App. B) -> M2L (App. B) -> L2L -> L2P (eq. 14, App. A.3) -> P2P
 // All coefficient arrays use the normalised, length-scaled representation described in tables.cu / DESIGN.md.
 // This file holds the kernels that work for every order p <= FMM_P_MAX and both dtypes; the unrolled register
-// M2L kernels live in m2l_fast.cu.
+// translation kernels (M2M, M2L, L2L) live in xlate_fast.cu.
 #include "internal.cuh"
 
 namespace fmm {
@@ -524,7 +524,11 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     dispatch_p2m_l2p<T>(Pl, false, st);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(2);
+    const bool fast = Pl.m2l_variant == 0 && xlate_fast_available(p, Pl.dtype);
+    if (fast && L > 0)  // the register kernels accumulate into the parents
+        FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), st));
     for (int l = L; l >= 1; --l) {
+        if (fast) { xlate_fast_launch(Pl, 0, l, st); continue; }
         const int64_t nbp = (int64_t)1 << (s * (l - 1));
         m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbp, Pl.box_count.p,
                                                                                 Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Mc.p, tp);
@@ -532,7 +536,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     }
     mark(3);
     if (Pl.n_weak > 0) {
-        if (Pl.m2l_variant == 0 && m2l_fast_available(p, Pl.dtype)) m2l_fast_launch(Pl, st);
+        if (fast) xlate_fast_launch(Pl, 1, 0, st);
         else
             m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(
                 p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
@@ -540,6 +544,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     }
     mark(4);
     for (int l = 1; l <= L; ++l) {
+        if (fast) { xlate_fast_launch(Pl, 2, l, st); continue; }
         const int64_t nbc = (int64_t)1 << (s * l);
         l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
                                                                                 Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Lc.p, tp);

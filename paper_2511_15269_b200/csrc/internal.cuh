@@ -104,8 +104,9 @@ void build_lists(Plan& P, cudaStream_t st);
 // evaluate.cu
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
 int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evaluate
-// m2l_fast.cu: returns false if no unrolled kernel exists for (p, dtype)
-bool m2l_fast_available(int p, fmm_dtype dt);
-void m2l_fast_launch(const Plan& P, cudaStream_t st);
+// xlate_fast.cu: register kernels (one thread per translation).  kind 0 = M2M into level-1 from `level`, 1 = M2L (all
+// levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
+bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
+void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st);
 
 }  // namespace fmm

@@ -1,0 +1,388 @@
+// xlate_fast.cu -- register ("fast") translation kernels: M2M (a5), M2L (a6) and L2L (a7) with ONE THREAD PER TRANSLATION.
+//
+// The operator is the paper's rotate / shift-along-z / rotate-back (App. B) in the
+// normalised, length-scaled representation of tables.cu, where rotations are orthogonal and the polar rotation factors
+// as Q(theta) = B Z(theta) B^T with constant matrices B (rot_tables.cuh).  One translation is
+//     Z(-phi) B Z(-theta) B^T  [z-shift]  B Z(theta) B^T Z(phi)
+// i.e. four azimuthal rotations (2 FP32 instructions per coefficient), four applications of the constant, 3/4-empty B
+// (247 MACs each at p=8) and one O(p^3) z-shift (489 MACs at p=8): about 2.3 k FP32 instructions at p=8.
+//
+// Why one thread per translation instead of the paper's / north_star's "one warp per interaction": every step is a
+// batch of small, ragged mat-vecs (block sizes 1..2p+1) with a different right-hand side per interaction, which maps
+// badly onto 32 lanes (K = 81 is 2.5 warps wide, rows have different lengths).  With one interaction per lane the whole
+// warp executes the same fully unrolled instruction stream, all matrix entries are immediates, the state vector lives
+// in registers, and there is no shuffle or shared-memory traffic inside the operator.  Shared memory is used only to
+// transpose: a warp loads its 32 source rows coalesced, each lane reads its own row with conflict-free LDS.128 (row
+// stride an odd number of 16-byte units), results go back the same way and are summed over runs of equal targets
+// (the lists are sorted by target) before one atomicAdd per coefficient and run.
+#include <type_traits>
+#include <utility>
+
+#include "internal.cuh"
+#include "rot_tables.cuh"
+
+namespace fmm {
+namespace {
+
+template <class F, int... I>
+__device__ __forceinline__ void sfor_impl(F&& f, std::integer_sequence<int, I...>) {
+    (f(std::integral_constant<int, I>{}), ...);
+}
+// compile-time loop: f(integral_constant<int, 0>) ... f(integral_constant<int, N-1>)
+template <int N, class F>
+__device__ __forceinline__ void sfor(F&& f) {
+    if constexpr (N > 0) sfor_impl(f, std::make_integer_sequence<int, N>{});
+}
+
+template <int n, bool TR>
+constexpr double bent(int i, int j) {
+    constexpr int w = 2 * n + 1;
+    return TR ? ct::kTab.B[ct::boff(n) + j * w + i] : ct::kTab.B[ct::boff(n) + i * w + j];
+}
+template <int n, bool TR>
+constexpr bool bfirst(int i, int j) {
+    for (int jj = 0; jj < j; ++jj)
+        if (bent<n, TR>(i, jj) != 0.0) return false;
+    return true;
+}
+
+// v[o .. o+2n] <- B_n v  (TR = false)  or  B_n^T v  (TR = true)
+template <typename T, int n, bool TR, int KV>
+__device__ __forceinline__ void apply_B(T (&v)[KV]) {
+    constexpr int w = 2 * n + 1, o = n * n;
+    T t[w];
+    sfor<w>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        T acc = T(0);
+        sfor<w>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            constexpr double b = bent<n, TR>(i, j);
+            if constexpr (b != 0.0) {
+                if constexpr (bfirst<n, TR>(i, j)) acc = T(b) * v[o + j];
+                else acc = fma(T(b), v[o + j], acc);
+            }
+        });
+        t[i] = acc;
+    });
+    sfor<w>([&](auto ic) { v[o + decltype(ic)::value] = t[decltype(ic)::value]; });
+}
+
+// azimuthal rotation of degree n (App. B.1 PAPER.md:441 in the normalised basis); SG = +1 forward, -1 inverse
+template <typename T, int n, int SG, int KV, int P1>
+__device__ __forceinline__ void apply_az(T (&v)[KV], const T (&c)[P1], const T (&s)[P1]) {
+    constexpr int o = n * n + n;
+    sfor<n>([&](auto mc) {
+        constexpr int m = decltype(mc)::value + 1;
+        const T a = v[o + m], b = v[o - m];
+        if constexpr (SG > 0) {
+            v[o + m] = fma(a, c[m], -(b * s[m]));
+            v[o - m] = fma(b, c[m], a * s[m]);
+        } else {
+            v[o + m] = fma(a, c[m], b * s[m]);
+            v[o - m] = fma(b, c[m], -(a * s[m]));
+        }
+    });
+}
+
+// cos(m x), sin(m x), m = 0..P, from cos x, sin x by the addition theorem
+template <typename T, int P1>
+__device__ __forceinline__ void trig_table(T c1, T s1, T (&c)[P1], T (&s)[P1]) {
+    c[0] = T(1);
+    s[0] = T(0);
+    sfor<P1 - 1>([&](auto mc) {
+        constexpr int m = decltype(mc)::value + 1;
+        c[m] = fma(c[m - 1], c1, -(s[m - 1] * s1));
+        s[m] = fma(s[m - 1], c1, c[m - 1] * s1);
+    });
+}
+
+// KIND 0 = M2M (b = child - parent), 1 = M2L (b = source - target), 2 = L2L (b = parent - child)   [DESIGN.md reading G3]
+// v: input coefficients of the old centre (length scale a_old) -> output coefficients about the new centre (a_new).
+template <typename T, int P, int KIND, int KV>
+__device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
+    constexpr int P1 = P + 1;
+    const T rxy2 = bx * bx + by * by;
+    const T r2 = rxy2 + bz * bz;
+    const T r = sqrt(r2), rxy = sqrt(rxy2);
+    const T rinv = r > T(0) ? T(1) / r : T(0);
+    const T rxyinv = rxy > T(0) ? T(1) / rxy : T(0);
+    const T ct_ = r > T(0) ? bz * rinv : T(1), st_ = rxy * rinv;
+    const T cp_ = rxy > T(0) ? bx * rxyinv : T(1), sp_ = by * rxyinv;
+    T x1, x2;
+    if constexpr (KIND == 0) { x1 = r / a_new; x2 = a_old / a_new; }
+    else if constexpr (KIND == 1) { x1 = a_new * rinv; x2 = a_old * rinv; }
+    else { x1 = -r / a_old; x2 = a_new / a_old; }
+
+    T cph[P1], sph[P1], cth[P1], sth[P1];
+    trig_table<T, P1>(cp_, sp_, cph, sph);
+    trig_table<T, P1>(ct_, st_, cth, sth);
+
+    // forward rotation, degree by degree; M2M / M2L fold the source scaling x2^k in
+    {
+        T pw = T(1);
+        sfor<P>([&](auto nc) {
+            constexpr int n = decltype(nc)::value + 1;
+            if constexpr (KIND != 2) {
+                pw *= x2;
+                sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
+            }
+            apply_az<T, n, +1>(v, cph, sph);
+            apply_B<T, n, true>(v);
+            apply_az<T, n, +1>(v, cth, sth);
+            apply_B<T, n, false>(v);
+        });
+    }
+
+    // z-shift (App. B.3), order by order; only equal m couple
+    if constexpr (KIND == 1) {
+        sfor<2 * P + 1>([&](auto mi) {
+            constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+            T t[cnt];
+            sfor<cnt>([&](auto ni) {
+                constexpr int n = am + decltype(ni)::value;
+                constexpr double h0 = ct::kTab.H[am][n][am];
+                T acc = T(h0) * v[am * am + am + m];
+                sfor<cnt - 1>([&](auto ki) {
+                    constexpr int k = am + 1 + decltype(ki)::value;
+                    constexpr double h = ct::kTab.H[am][n][k];
+                    acc = fma(T(h), v[k * k + k + m], acc);
+                });
+                t[decltype(ni)::value] = acc;
+            });
+            sfor<cnt>([&](auto ni) { v[(am + decltype(ni)::value) * (am + decltype(ni)::value + 1) + m] = t[decltype(ni)::value]; });
+        });
+        T pw = rinv;
+        sfor<P1>([&](auto nc) {
+            constexpr int n = decltype(nc)::value;
+            sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
+            pw *= x1;
+        });
+    } else {
+        T pw1[P1];
+        pw1[0] = T(1);
+        sfor<P>([&](auto jc) { pw1[decltype(jc)::value + 1] = pw1[decltype(jc)::value] * x1; });
+        if constexpr (KIND == 0) {
+            // out[n] = sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (v already scaled by x2^k): in place, n descending
+            sfor<2 * P + 1>([&](auto mi) {
+                constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+                sfor<cnt>([&](auto ni) {
+                    constexpr int n = P - decltype(ni)::value;
+                    T acc = v[n * n + n + m];  // A[m][n][n] = 1
+                    sfor<n - am>([&](auto ki) {
+                        constexpr int k = am + decltype(ki)::value;
+                        constexpr double aa = ct::kTab.A[am][n][k];
+                        acc = fma(T(aa) * pw1[n - k], v[k * k + k + m], acc);
+                    });
+                    v[n * n + n + m] = acc;
+                });
+            });
+        } else {
+            // out[n] = x2^n sum_{k=n..p} A[|m|][k][n] x1^(k-n) v[k]: in place, n ascending
+            T pw2[P1];
+            pw2[0] = T(1);
+            sfor<P>([&](auto jc) { pw2[decltype(jc)::value + 1] = pw2[decltype(jc)::value] * x2; });
+            sfor<2 * P + 1>([&](auto mi) {
+                constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+                sfor<cnt>([&](auto ni) {
+                    constexpr int n = am + decltype(ni)::value;
+                    T acc = v[n * n + n + m];
+                    sfor<P - n>([&](auto ki) {
+                        constexpr int k = n + 1 + decltype(ki)::value;
+                        constexpr double aa = ct::kTab.A[am][k][n];
+                        acc = fma(T(aa) * pw1[k - n], v[k * k + k + m], acc);
+                    });
+                    v[n * n + n + m] = acc * pw2[n];
+                });
+            });
+        }
+    }
+
+    // inverse rotation
+    sfor<P>([&](auto nc) {
+        constexpr int n = decltype(nc)::value + 1;
+        apply_B<T, n, true>(v);
+        apply_az<T, n, -1>(v, cth, sth);
+        apply_B<T, n, false>(v);
+        apply_az<T, n, -1>(v, cph, sph);
+    });
+}
+
+template <typename T> struct Vec16;
+template <> struct Vec16<float> { using type = float4; static constexpr int E = 4; };
+template <> struct Vec16<double> { using type = double2; static constexpr int E = 2; };
+
+template <typename T, int P>
+struct Geo {
+    static constexpr int K = (P + 1) * (P + 1);
+    static constexpr int E = Vec16<T>::E;
+    static constexpr int Kp = (K + 3) & ~3;            // row stride of the global coefficient arrays (elements)
+    static constexpr int CH = Kp / E;                  // 16-byte chunks per global row
+    static constexpr int KSB = (CH & 1) ? CH : CH + 1; // shared row stride in 16-byte units: odd => conflict-free LDS.128
+    static constexpr int KV = CH * E;                  // register vector length
+    static constexpr int NJ = (K + 31) / 32;
+};
+
+struct XArgs {
+    int64_t n;                    // number of translations
+    const int32_t *tgt, *src;     // KIND 1: global ids per pair
+    int64_t off_parent, off_child;
+    int s;
+    const int32_t* box_count;
+    const double* ctr;
+    const void* scale;
+    const void* in;
+    void* out;
+};
+
+constexpr int XW = 4;  // warps per CTA
+
+template <typename T, int P, int KIND>
+__global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
+    using G = Geo<T, P>;
+    using V = typename Vec16<T>::type;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    V* sm = reinterpret_cast<V*>(smraw) + (size_t)warp * 32 * G::KSB;
+    const int64_t e = ((int64_t)blockIdx.x * XW + warp) * 32 + lane;
+    int gs = -1, gt = -1;
+    if (e < a.n) {
+        if constexpr (KIND == 1) { gs = a.src[e]; gt = a.tgt[e]; }
+        else {
+            const int64_t gc = a.off_child + e, gp = a.off_parent + (e >> a.s);
+            if (a.box_count[gc] > 0) {
+                if constexpr (KIND == 0) { gs = (int)gc; gt = (int)gp; }
+                else { gs = (int)gp; gt = (int)gc; }
+            }
+        }
+    }
+    if (__ballot_sync(0xffffffffu, gs >= 0) == 0) return;
+
+    // coalesced load of the warp's 32 source rows into shared memory
+    const V* in16 = reinterpret_cast<const V*>(a.in);
+#pragma unroll
+    for (int it = 0; it < G::CH; ++it) {
+        const int idx = it * 32 + lane;
+        const int r = idx / G::CH, c = idx - r * G::CH;
+        const int g = __shfl_sync(0xffffffffu, gs, r);
+        if (g >= 0) sm[r * G::KSB + c] = in16[(int64_t)g * G::CH + c];
+    }
+    T bx = T(0), by = T(0), bz = T(1), a_old = T(1), a_new = T(1);
+    if (gs >= 0) {
+        const T* sc = reinterpret_cast<const T*>(a.scale);
+        bx = (T)(a.ctr[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
+        by = (T)(a.ctr[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
+        bz = (T)(a.ctr[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
+        a_old = sc[gs];
+        a_new = sc[gt];
+    }
+    __syncwarp();
+
+    T v[G::KV];
+    V* row = sm + lane * G::KSB;
+    if (gs >= 0) {
+        sfor<G::CH>([&](auto cc) {
+            constexpr int c = decltype(cc)::value;
+            const V x = row[c];
+            if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
+            else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
+        });
+        translate_reg<T, P, KIND>(v, bx, by, bz, a_old, a_new);
+        sfor<G::CH>([&](auto cc) {
+            constexpr int c = decltype(cc)::value;
+            V x;
+            if constexpr (G::E == 4) { x.x = v[4 * c]; x.y = v[4 * c + 1]; x.z = v[4 * c + 2]; x.w = v[4 * c + 3]; }
+            else { x.x = v[2 * c]; x.y = v[2 * c + 1]; }
+            row[c] = x;
+        });
+    }
+    __syncwarp();
+
+    // sum runs of equal targets (lists are sorted by target), one atomicAdd per coefficient and run
+    const T* smT = reinterpret_cast<const T*>(sm);
+    T* out = reinterpret_cast<T*>(a.out);
+    constexpr int RS = G::KSB * G::E;  // shared row stride in elements
+    T acc[G::NJ];
+#pragma unroll
+    for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
+    int cur = __shfl_sync(0xffffffffu, gt, 0);
+#pragma unroll 4
+    for (int r = 0; r < 32; ++r) {
+        const int t = __shfl_sync(0xffffffffu, gt, r);
+        if (t != cur) {
+            if (cur >= 0) {
+#pragma unroll
+                for (int j = 0; j < G::NJ; ++j)
+                    if (lane + 32 * j < G::K) atomicAdd(out + (int64_t)cur * G::Kp + lane + 32 * j, acc[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
+            cur = t;
+        }
+        if (t >= 0) {
+#pragma unroll
+            for (int j = 0; j < G::NJ; ++j)
+                if (lane + 32 * j < G::K) acc[j] += smT[r * RS + lane + 32 * j];
+        }
+    }
+    if (cur >= 0) {
+#pragma unroll
+        for (int j = 0; j < G::NJ; ++j)
+            if (lane + 32 * j < G::K) atomicAdd(out + (int64_t)cur * G::Kp + lane + 32 * j, acc[j]);
+    }
+}
+
+template <typename T, int P, int KIND>
+void launch(const XArgs& a, cudaStream_t st) {
+    using G = Geo<T, P>;
+    constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16;
+    static bool attr_set = false;
+    if (!attr_set) {
+        FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    const unsigned grid = (unsigned)((a.n + XW * 32 - 1) / (XW * 32));
+    xlate_fast_k<T, P, KIND><<<grid, XW * 32, smem, st>>>(a);
+}
+
+template <typename T, int KIND>
+bool dispatch(int p, const XArgs& a, cudaStream_t st) {
+    switch (p) {
+#define FMM_CASE(PP) case PP: launch<T, PP, KIND>(a, st); return true;
+        FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
+#undef FMM_CASE
+        default: return false;
+    }
+}
+
+}  // namespace
+
+bool xlate_fast_available(int p, fmm_dtype dt) { return dt == FMM_F32 && p >= 1 && p <= 8; }
+
+void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st) {
+    XArgs a{};
+    a.box_count = P.box_count.p;
+    a.ctr = P.box_ctr.p;
+    a.scale = P.box_scale.p;
+    a.s = P.s;
+    if (kind == 1) {
+        a.n = P.n_weak;
+        a.tgt = P.weak_tgt.p;
+        a.src = P.weak_src.p;
+        a.in = P.Mc.p;
+        a.out = P.Lc.p;
+    } else {
+        a.n = (int64_t)1 << (P.s * level);  // children on `level`
+        a.off_parent = P.level_off[level - 1];
+        a.off_child = P.level_off[level];
+        a.in = kind == 0 ? P.Mc.p : P.Lc.p;
+        a.out = kind == 0 ? P.Mc.p : P.Lc.p;
+    }
+    if (a.n == 0) return;
+    bool ok = false;
+    if (kind == 0) ok = dispatch<float, 0>(P.p, a, st);
+    else if (kind == 1) ok = dispatch<float, 1>(P.p, a, st);
+    else ok = dispatch<float, 2>(P.p, a, st);
+    if (!ok) { set_error("no register translation kernel for this order"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+}
+
+}  // namespace fmm
