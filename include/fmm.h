@@ -107,8 +107,9 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
 /* Plan-phase device times in ms (HOST out, 4 doubles): [0] sort keys, [1] tree rounds, [2] lists, [3] total. */
 fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
 
-/* Selects the M2L implementation used by subsequent fmm_evaluate calls on this plan:
- * 0 = automatic (unrolled register kernel when available for (p, dtype), else generic), 1 = force generic. */
+/* Selects the kernel family used by subsequent fmm_evaluate calls on this plan:
+ * 0 = automatic (register translation kernels and the packed-f32x2 P2P kernel when available for (p, dtype), else the
+ * generic kernels), 1 = force the generic kernels (any p <= FMM_P_MAX, both dtypes; used by the tests to cross-check). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
 /* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M

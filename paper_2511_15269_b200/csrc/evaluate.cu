@@ -555,7 +555,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(6);
     const int64_t leaf0 = Pl.level_off[L];
-    p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
+    if (sizeof(T) == 4 && Pl.m2l_variant == 0) p2p_fast_launch(Pl, d_pot, d_field, st);
+    else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
                                                             Pl.strong_src.p, (const T4*)Pl.far.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(7);

@@ -190,10 +190,11 @@ def test_potential_only_and_field_only_and_host_path():
     none2, f2 = P.evaluate(tq, want_potential=False)
     torch.cuda.synchronize()
     assert none is None and none2 is None
-    assert np.array_equal(u2.cpu().numpy(), u) and np.array_equal(f2.cpu().numpy(), f)
+    # the fp32 register translation kernels add partial sums with atomicAdd, so repeated runs agree to rounding only
+    assert rel2(u2.cpu().numpy(), u.astype(np.float64)) < 2e-6 and rel2(f2.cpu().numpy(), f.astype(np.float64)) < 2e-6
     hu, hf = np.empty_like(u), np.empty_like(f)
     fmm.fmm_evaluate_host(P.handle, q, hu, hf)
-    assert np.array_equal(hu, u) and np.array_equal(hf, f)
+    assert rel2(hu, u.astype(np.float64)) < 2e-6 and rel2(hf, f.astype(np.float64)) < 2e-6
     P.close()
 
 
