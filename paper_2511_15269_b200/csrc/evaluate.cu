@@ -31,10 +31,16 @@ inline unsigned nblocks(int64_t n, int t) { return (unsigned)((n + t - 1) / t); 
 // ------------------------------------------------------------------------------------------------ permute (a3)
 template <typename T>
 __global__ void permute_k(const T* __restrict__ pos_tree, const T* __restrict__ q, const int32_t* __restrict__ perm,
-                          typename V4<T>::type* __restrict__ pq, int64_t N) {
+                          typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ src_slot, float* __restrict__ srcg, int64_t N) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    pq[k] = make4<T>(pos_tree[3 * k], pos_tree[3 * k + 1], pos_tree[3 * k + 2], q[perm[k]]);
+    const T x = pos_tree[3 * k], y = pos_tree[3 * k + 1], z = pos_tree[3 * k + 2], qq = q[perm[k]];
+    pq[k] = make4<T>(x, y, z, qq);
+    if (srcg) {  // fp32 only: P2P source groups (-x[4], -y[4], -z[4], q[4]), see p2p_fast.cu
+        const int32_t sl = src_slot[k];
+        float* g = srcg + (int64_t)(sl >> 2) * 16 + (sl & 3);
+        g[0] = -(float)x; g[4] = -(float)y; g[8] = -(float)z; g[12] = (float)qq;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ basis recursions
@@ -517,7 +523,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const int64_t N = Pl.N;
     auto mark = [&](int i) { if (ev) FMM_CUDA_CHECK(cudaEventRecord(ev[i], st)); };
     mark(0);
-    permute_k<T><<<nblocks(N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, N);
+    permute_k<T><<<nblocks(N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, Pl.src_slot.p,
+                                                  sizeof(T) == 4 ? Pl.srcg.p : nullptr, N);
     FMM_CUDA_CHECK(cudaGetLastError());
     FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, st));
     mark(1);

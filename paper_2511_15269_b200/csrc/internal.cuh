@@ -93,6 +93,10 @@ struct Plan {
     DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> far;     // N x 4 dtype: (phi_far, grad phi_far) tree order
+    // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
+    DevBuf<float> srcg;
+    DevBuf<int32_t> src_slot;
+    int src_G = 0;
     DevBuf<char> h2d_q, d2h_out;  // staging for fmm_evaluate_host
     double plan_ms[4] = {0, 0, 0, 0};
     double stage_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};

@@ -5,8 +5,12 @@
 // Mapping (differs from north_star's "one target leaf per CTA": one target leaf per WARP):
 //   * a warp owns one target leaf (or a chunk of 32*TPT targets of a large leaf); lanes form ntgp target groups x nsl
 //     source slices, every lane keeps TPT targets in registers;
-//   * the warp stages the particles of its source leaves into its private shared-memory tile in SoA form
-//     (-x[], -y[], -z[], q[]), so one LDS.128 per array brings FOUR sources as two packed pairs;
+//   * sources are read from `srcg`, a per-evaluate copy of the particles in groups of four, (-x[4], -y[4], -z[4], q[4]) =
+//     64 bytes, every leaf padded to whole groups with zero charges (written by the permute kernel).  A warp copies the
+//     groups of its source leaves into its private, double-buffered shared-memory tiles with TMA bulk copies
+//     (cp.async.bulk + mbarrier: one copy per source leaf, issued by 32 lanes at once), so staging costs a handful of
+//     instructions per tile and overlaps with the arithmetic on the previous tile; one LDS.128 per component then brings
+//     FOUR sources as two packed pairs;
 //   * all FP32 arithmetic of a (target, source-pair) runs as packed f32x2 instructions (FADD2 / FMUL2 / FFMA2, new on
 //     sm_100): 13 packed instructions + 2 MUFU.RSQ + 2 (FSETP+FSEL) per two particle pairs.  The FMA pipe issues a packed
 //     instruction every other cycle, which leaves the issue slots in between for MUFU, the mask, LDS and the loop;
@@ -45,16 +49,39 @@ __device__ __forceinline__ float rsq(float x) {
     return r;
 }
 
-constexpr int PW = 4;      // warps per CTA (independent of one another)
-constexpr int TILE = 256;  // sources per warp tile (4 KB of shared memory per warp)
+constexpr int PW = 4;   // warps per CTA (independent of one another)
+constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two tiles per warp = 8 KB of shared memory
 
+// ---- TMA bulk copy (cp.async.bulk, SASS UBLKCP) + mbarrier, per-warp pipelines
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
+// the leaf population hold zeros (zero charge), so whole groups can be used without masks.
 template <int TPT>
-__global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const int32_t* __restrict__ leaf_start,
-                                                      const int32_t* __restrict__ leaf_cnt, const int64_t* __restrict__ strong_off,
-                                                      const int32_t* __restrict__ strong_src, const float4* __restrict__ far,
-                                                      const int32_t* __restrict__ perm, float* __restrict__ pot, float* __restrict__ field,
-                                                      int64_t n_items, int nchunk) {
-    __shared__ __align__(16) float sm[PW][4][TILE];
+__global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
+                                                      const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
+                                                      const int64_t* __restrict__ strong_off, const int32_t* __restrict__ strong_src,
+                                                      const float4* __restrict__ far, const int32_t* __restrict__ perm,
+                                                      float* __restrict__ pot, float* __restrict__ field, int64_t n_items, int nchunk) {
+    __shared__ __align__(128) float sm[PW][2][TG * 16];
+    __shared__ __align__(8) unsigned long long bars[PW][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t item = (int64_t)blockIdx.x * PW + warp;
     if (item >= n_items) return;
@@ -70,12 +97,15 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
     const int ntgp = 1 << lg, nsl = 32 >> lg;
     const int tg = lane & (ntgp - 1), sl = lane >> lg;
 
-    float* X = sm[warp][0];
-    float* Y = sm[warp][1];
-    float* Z = sm[warp][2];
-    float* Q = sm[warp][3];
+    const uint32_t bar0 = smem_u32(&bars[warp][0]), buf0 = smem_u32(&sm[warp][0][0]);
+    if (lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
 
-    // targets of this lane, each coordinate duplicated into both halves of a packed register
+    // targets of this lane (the compiler turns pk(v, v) into a broadcast operand of the packed instructions)
     u64 TX[TPT], TY[TPT], TZ[TPT], PH[TPT], GX[TPT], GY[TPT], GZ[TPT];
 #pragma unroll
     for (int k = 0; k < TPT; ++k) {
@@ -90,20 +120,23 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
 
     int64_t e = strong_off[leaf];
     const int64_t e1 = strong_off[leaf + 1];
-    int sub = 0;  // particles of entry e already consumed
-    while (e < e1) {
+    int sub = 0;  // groups of entry e already consumed
+
+    // producer: fill tile `b` with up to TG groups starting at the cursor (e, sub); every lane issues the bulk copy of "its" entry
+    auto produce = [&](int b) -> int {
         int fill = 0;
-        __syncwarp();  // the previous tile has been consumed by every lane
-        while (e < e1 && fill < TILE) {
-            // lanes look at the next (up to) 32 source leaves
+        uint32_t bytes = 0;
+        const uint32_t bar = bar0 + 8 * b, buf = buf0 + (uint32_t)b * (TG * 64);
+        while (e < e1 && fill < TG) {
             const int nb = (int)min((int64_t)32, e1 - e);
-            int st = 0, c = 0;
+            int c = 0;
+            int64_t g0 = 0;
             if (lane < nb) {
                 const int ent = strong_src[e + lane];
-                st = leaf_start[ent];
-                c = leaf_cnt[ent];
+                g0 = (int64_t)ent * G;
+                c = (leaf_cnt[ent] + 3) >> 2;
             }
-            if (lane == 0) { st += sub; c -= sub; }
+            if (lane == 0) { g0 += sub; c -= sub; }
             int incl = c;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
@@ -111,18 +144,11 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                 if (lane >= d) incl += t;
             }
             const int excl = incl - c;
-            const int room = TILE - fill;
-#pragma unroll 4
-            for (int i = 0; i < nb; ++i) {
-                const int oi = __shfl_sync(0xffffffffu, excl, i);
-                if (oi >= room) break;
-                const int si = __shfl_sync(0xffffffffu, st, i);
-                const int ni = min(__shfl_sync(0xffffffffu, c, i), room - oi);
-                for (int x = lane; x < ni; x += 32) {
-                    const float4 v = pq[si + x];
-                    const int d = fill + oi + x;
-                    X[d] = -v.x; Y[d] = -v.y; Z[d] = -v.z; Q[d] = v.w;
-                }
+            const int room = TG - fill;
+            const int ni = min(c, room - excl);
+            if (ni > 0) {
+                bulk_g2s(buf + (uint32_t)(fill + excl) * 64u, srcg + g0 * 16, (uint32_t)ni * 64u, bar);
+                bytes += (uint32_t)ni * 64u;
             }
             const int total = __shfl_sync(0xffffffffu, incl, 31);
             if (total <= room) {
@@ -135,23 +161,25 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                 const int ex = __shfl_sync(0xffffffffu, excl, idx);
                 sub = (idx == 0 ? sub : 0) + (room - ex);
                 e += idx;
-                fill = TILE;
+                fill = TG;
             }
         }
-        // pad to a multiple of four sources with zero charges
-        const int fp = (fill + 3) & ~3;
-        if (lane < fp - fill) {
-            const int d = fill + lane;
-            X[d] = 0.f; Y[d] = 0.f; Z[d] = 0.f; Q[d] = 0.f;
-        }
-        __syncwarp();
-        const int ng = fp >> 2;
-        const ulonglong2* X2 = reinterpret_cast<const ulonglong2*>(X);
-        const ulonglong2* Y2 = reinterpret_cast<const ulonglong2*>(Y);
-        const ulonglong2* Z2 = reinterpret_cast<const ulonglong2*>(Z);
-        const ulonglong2* Q2 = reinterpret_cast<const ulonglong2*>(Q);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, d);
+        if (lane == 0) mbar_expect_tx(bar, bytes);
+        return fill;
+    };
+
+    int ng_next = (e < e1) ? produce(0) : 0;
+    for (int t = 0; ng_next > 0; ++t) {
+        const int b = t & 1;
+        const int ng = ng_next;
+        __syncwarp();  // every lane has finished reading the other buffer (tile t-1)
+        ng_next = (e < e1) ? produce(b ^ 1) : 0;
+        mbar_wait(bar0 + 8 * b, (t >> 1) & 1);
+        const ulonglong2* T2 = reinterpret_cast<const ulonglong2*>(&sm[warp][b][0]);
         for (int j = sl; j < ng; j += nsl) {
-            const ulonglong2 xs = X2[j], ys = Y2[j], zs = Z2[j], qs = Q2[j];
+            const ulonglong2 xs = T2[4 * j], ys = T2[4 * j + 1], zs = T2[4 * j + 2], qs = T2[4 * j + 3];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const u64 sx = h ? xs.y : xs.x, sy = h ? ys.y : ys.x, sz = h ? zs.y : zs.x, sq = h ? qs.y : qs.x;
@@ -161,12 +189,12 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                     u64 r2 = mul2(dx, dx);
                     r2 = fma2(dy, dy, r2);
                     r2 = fma2(dz, dz, r2);
-                    float a, b;
-                    upk(r2, a, b);
-                    float ia = rsq(a), ib = rsq(b);
+                    float a, b2;
+                    upk(r2, a, b2);
+                    float ia = rsq(a), ib = rsq(b2);
                     // reading S3: coincident pairs contribute nothing (r^2 below FLT_MIN counts as coincident in fp32)
                     ia = a >= 1.17549435e-38f ? ia : 0.f;
-                    ib = b >= 1.17549435e-38f ? ib : 0.f;
+                    ib = b2 >= 1.17549435e-38f ? ib : 0.f;
                     const u64 inv = pk(ia, ib);
                     const u64 qi = mul2(sq, inv), inv2 = mul2(inv, inv);
                     const u64 q3 = mul2(qi, inv2);
@@ -225,8 +253,9 @@ void p2p_fast_launch(const Plan& P, void* d_pot, void* d_field, cudaStream_t st)
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
     const int64_t n_items = P.n_leaves * nchunk;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
-    p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, P.box_start.p + leaf0, P.box_count.p + leaf0, P.strong_off.p, P.strong_src.p,
-                                              (const float4*)P.far.p, P.perm.p, (float*)d_pot, (float*)d_field, n_items, nchunk);
+    p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
+                                              P.strong_off.p, P.strong_src.p, (const float4*)P.far.p, P.perm.p, (float*)d_pot, (float*)d_field,
+                                              n_items, nchunk);
 }
 
 }  // namespace fmm

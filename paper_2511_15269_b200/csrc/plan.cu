@@ -176,6 +176,14 @@ __global__ void gather_pos_k(const T* pos, const int32_t* perm, T* pos_tree, int
     pos_tree[3 * k + 2] = pos[3 * i + 2];
 }
 
+// P2P source-group slots (fp32): particle i of leaf l -> 4 * (l * G + i / 4) + (i & 3); one warp per leaf
+__global__ void src_slot_k(const int32_t* leaf_start, const int32_t* leaf_cnt, int64_t n_leaves, int G, int32_t* slot) {
+    const int64_t leaf = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (leaf >= n_leaves) return;
+    const int st = leaf_start[leaf], c = leaf_cnt[leaf];
+    for (int i = threadIdx.x & 31; i < c; i += 32) slot[st + i] = (int32_t)(4 * (leaf * G + (i >> 2)) + (i & 3));
+}
+
 inline unsigned nblocks(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
 
 template <typename T, typename KeyT>
@@ -274,6 +282,19 @@ void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
         const int64_t nb = (int64_t)1 << (P.s * l);
         geometry_k<T><<<nblocks(nb, 128), 128, 0, st>>>((const T*)P.box_lo.p, (const T*)P.box_hi.p, P.box_count.p, P.level_off[l], nb,
                                                         l > 0 ? P.level_off[l - 1] : -1, P.s, P.box_ctr.p, P.box_rad.p, (T*)P.box_scale.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    if (sizeof(T) == 4) {
+        P.src_G = (P.max_leaf + 3) / 4;
+        if (4 * (n_leaves * P.src_G + 1) > 0x7fffffffll) {
+            set_error("too many P2P source groups for 32-bit slots");
+            throw CudaFail{FMM_ERR_UNSUPPORTED};
+        }
+        P.src_slot.alloc(N);
+        P.srcg.alloc((size_t)n_leaves * P.src_G * 16);
+        FMM_CUDA_CHECK(cudaMemsetAsync(P.srcg.p, 0, P.srcg.n * sizeof(float), st));  // pad slots: zero charge, finite position
+        src_slot_k<<<nblocks(n_leaves * 32, 128), 128, 0, st>>>(P.box_start.p + P.level_off[P.L], P.box_count.p + P.level_off[P.L], n_leaves,
+                                                               P.src_G, P.src_slot.p);
         FMM_CUDA_CHECK(cudaGetLastError());
     }
     P.pos_tree.alloc(N * 3 * sizeof(T));
