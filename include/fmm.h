@@ -108,8 +108,9 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
 fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
 
 /* Selects the kernel family used by subsequent fmm_evaluate calls on this plan:
- * 0 = automatic (register translation kernels and the packed-f32x2 P2P kernel when available for (p, dtype), else the
- * generic kernels), 1 = force the generic kernels (any p <= FMM_P_MAX, both dtypes; used by the tests to cross-check). */
+ * 0 = automatic (register translation kernels, one translation per thread, and the packed-f32x2 P2P kernel when available
+ * for (p, dtype), else the generic kernels), 1 = force the generic kernels (any p <= FMM_P_MAX, both dtypes; used by the
+ * tests to cross-check), 2 = as 0 but M2L by the two-pairs-per-thread packed-f32x2 kernel (m2l_packed.cu). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
 /* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M

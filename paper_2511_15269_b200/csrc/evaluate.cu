@@ -531,7 +531,9 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     dispatch_p2m_l2p<T>(Pl, false, st);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(2);
-    const bool fast = Pl.m2l_variant == 0 && xlate_fast_available(p, Pl.dtype);
+    // m2l_variant: 0 = register kernels (one translation per thread), 1 = generic kernels, 2 = as 0 but M2L two pairs per thread (f32x2)
+    const bool fast = Pl.m2l_variant != 1 && xlate_fast_available(p, Pl.dtype);
+    const bool packed = Pl.m2l_variant == 2 && m2l_packed_available(p, Pl.dtype);
     if (fast && L > 0)  // the register kernels accumulate into the parents
         FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), st));
     for (int l = L; l >= 1; --l) {
@@ -543,7 +545,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     }
     mark(3);
     if (Pl.n_weak > 0) {
-        if (fast) xlate_fast_launch(Pl, 1, 0, st);
+        if (packed) m2l_packed_launch(Pl, st);
+        else if (fast) xlate_fast_launch(Pl, 1, 0, st);
         else
             m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(
                 p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
@@ -562,7 +565,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(6);
     const int64_t leaf0 = Pl.level_off[L];
-    if (sizeof(T) == 4 && Pl.m2l_variant == 0) p2p_fast_launch(Pl, d_pot, d_field, st);
+    if (sizeof(T) == 4 && Pl.m2l_variant != 1) p2p_fast_launch(Pl, d_pot, d_field, st);
     else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
                                                             Pl.strong_src.p, (const T4*)Pl.far.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
     FMM_CUDA_CHECK(cudaGetLastError());

@@ -112,6 +112,9 @@ int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evalua
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
 bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st);
+// m2l_packed.cu: fp32 M2L with two weak pairs per thread in packed f32x2 arithmetic (p <= 8); results are ADDED to Lc
+bool m2l_packed_available(int p, fmm_dtype dt);
+void m2l_packed_launch(const Plan& P, cudaStream_t st);
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
 void p2p_fast_launch(const Plan& P, void* d_pot, void* d_field, cudaStream_t st);
 

@@ -15,90 +15,19 @@
 // transpose: a warp loads its 32 source rows coalesced, each lane reads its own row with conflict-free LDS.128 (row
 // stride an odd number of 16-byte units), results go back the same way and are summed over runs of equal targets
 // (the lists are sorted by target) before one atomicAdd per coefficient and run.
-#include <type_traits>
-#include <utility>
-
-#include "internal.cuh"
-#include "rot_tables.cuh"
+#include "xlate_reg.cuh"
 
 namespace fmm {
 namespace {
 
-template <class F, int... I>
-__device__ __forceinline__ void sfor_impl(F&& f, std::integer_sequence<int, I...>) {
-    (f(std::integral_constant<int, I>{}), ...);
-}
-// compile-time loop: f(integral_constant<int, 0>) ... f(integral_constant<int, N-1>)
-template <int N, class F>
-__device__ __forceinline__ void sfor(F&& f) {
-    if constexpr (N > 0) sfor_impl(f, std::make_integer_sequence<int, N>{});
-}
+using namespace xr;
 
-template <int n, bool TR>
-constexpr double bent(int i, int j) {
-    constexpr int w = 2 * n + 1;
-    return TR ? ct::kTab.B[ct::boff(n) + j * w + i] : ct::kTab.B[ct::boff(n) + i * w + j];
-}
-template <int n, bool TR>
-constexpr bool bfirst(int i, int j) {
-    for (int jj = 0; jj < j; ++jj)
-        if (bent<n, TR>(i, jj) != 0.0) return false;
-    return true;
-}
-
-// v[o .. o+2n] <- B_n v  (TR = false)  or  B_n^T v  (TR = true)
-template <typename T, int n, bool TR, int KV>
-__device__ __forceinline__ void apply_B(T (&v)[KV]) {
-    constexpr int w = 2 * n + 1, o = n * n;
-    T t[w];
-    sfor<w>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        T acc = T(0);
-        sfor<w>([&](auto jc) {
-            constexpr int j = decltype(jc)::value;
-            constexpr double b = bent<n, TR>(i, j);
-            if constexpr (b != 0.0) {
-                if constexpr (bfirst<n, TR>(i, j)) acc = T(b) * v[o + j];
-                else acc = fma(T(b), v[o + j], acc);
-            }
-        });
-        t[i] = acc;
-    });
-    sfor<w>([&](auto ic) { v[o + decltype(ic)::value] = t[decltype(ic)::value]; });
-}
-
-// azimuthal rotation of degree n (App. B.1 PAPER.md:441 in the normalised basis); SG = +1 forward, -1 inverse
-template <typename T, int n, int SG, int KV, int P1>
-__device__ __forceinline__ void apply_az(T (&v)[KV], const T (&c)[P1], const T (&s)[P1]) {
-    constexpr int o = n * n + n;
-    sfor<n>([&](auto mc) {
-        constexpr int m = decltype(mc)::value + 1;
-        const T a = v[o + m], b = v[o - m];
-        if constexpr (SG > 0) {
-            v[o + m] = fma(a, c[m], -(b * s[m]));
-            v[o - m] = fma(b, c[m], a * s[m]);
-        } else {
-            v[o + m] = fma(a, c[m], b * s[m]);
-            v[o - m] = fma(b, c[m], -(a * s[m]));
-        }
-    });
-}
-
-// cos(m x), sin(m x), m = 0..P, from cos x, sin x by the addition theorem
-template <typename T, int P1>
-__device__ __forceinline__ void trig_table(T c1, T s1, T (&c)[P1], T (&s)[P1]) {
-    c[0] = T(1);
-    s[0] = T(0);
-    sfor<P1 - 1>([&](auto mc) {
-        constexpr int m = decltype(mc)::value + 1;
-        c[m] = fma(c[m - 1], c1, -(s[m - 1] * s1));
-        s[m] = fma(s[m - 1], c1, c[m - 1] * s1);
-    });
-}
 
 // KIND 0 = M2M (b = child - parent), 1 = M2L (b = source - target), 2 = L2L (b = parent - child)   [DESIGN.md reading G3]
 // v: input coefficients of the old centre (length scale a_old) -> output coefficients about the new centre (a_new).
-template <typename T, int P, int KIND, int KV>
+// SYNC: the warps of a CTA meet at a barrier after every phase, so that they walk the (large, straight-line) code in
+// lockstep and share instruction-cache lines.
+template <typename T, int P, int KIND, bool SYNC, int KV>
 __device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
     constexpr int P1 = P + 1;
     const T rxy2 = bx * bx + by * by;
@@ -130,6 +59,7 @@ __device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_
             apply_B<T, n, true>(v);
             apply_az<T, n, +1>(v, cth, sth);
             apply_B<T, n, false>(v);
+            if constexpr (SYNC && n >= 3) __syncthreads();
         });
     }
 
@@ -198,12 +128,14 @@ __device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_
     }
 
     // inverse rotation
+    if constexpr (SYNC) __syncthreads();
     sfor<P>([&](auto nc) {
         constexpr int n = decltype(nc)::value + 1;
         apply_B<T, n, true>(v);
         apply_az<T, n, -1>(v, cth, sth);
         apply_B<T, n, false>(v);
         apply_az<T, n, -1>(v, cph, sph);
+        if constexpr (SYNC && n >= 3) __syncthreads();
     });
 }
 
@@ -234,9 +166,8 @@ struct XArgs {
     void* out;
 };
 
-constexpr int XW = 4;  // warps per CTA
-
-template <typename T, int P, int KIND>
+// XW warps per CTA; SYNC = lockstep barriers (all warps then run the operator, also on padding lanes)
+template <typename T, int P, int KIND, int XW, bool SYNC>
 __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
@@ -255,7 +186,9 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
             }
         }
     }
-    if (__ballot_sync(0xffffffffu, gs >= 0) == 0) return;
+    if constexpr (!SYNC) {
+        if (__ballot_sync(0xffffffffu, gs >= 0) == 0) return;
+    }
 
     // coalesced load of the warp's 32 source rows into shared memory
     const V* in16 = reinterpret_cast<const V*>(a.in);
@@ -279,14 +212,14 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
 
     T v[G::KV];
     V* row = sm + lane * G::KSB;
-    if (gs >= 0) {
+    if (SYNC || gs >= 0) {
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             const V x = row[c];
             if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
             else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
         });
-        translate_reg<T, P, KIND>(v, bx, by, bz, a_old, a_new);
+        translate_reg<T, P, KIND, SYNC>(v, bx, by, bz, a_old, a_new);
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             V x;
@@ -331,17 +264,17 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
     }
 }
 
-template <typename T, int P, int KIND>
+template <typename T, int P, int KIND, int XW = 4, bool SYNC = false>
 void launch(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
     constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16;
     static bool attr_set = false;
     if (!attr_set) {
-        FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     const unsigned grid = (unsigned)((a.n + XW * 32 - 1) / (XW * 32));
-    xlate_fast_k<T, P, KIND><<<grid, XW * 32, smem, st>>>(a);
+    xlate_fast_k<T, P, KIND, XW, SYNC><<<grid, XW * 32, smem, st>>>(a);
 }
 
 template <typename T, int KIND>
