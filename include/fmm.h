@@ -99,7 +99,7 @@ fmm_status fmm_plan_copy_lists(const fmm_plan* plan, int64_t* h_weak_off, int32_
                                int64_t* h_strong_off, int32_t* h_strong_src);
 
 /* Per-stage device times of the most recent fmm_evaluate_profiled call, in milliseconds (HOST out, 8 doubles):
- * [0] permute, [1] P2M, [2] M2M, [3] M2L, [4] L2L, [5] L2P, [6] P2P, [7] total.  fmm_evaluate_profiled is
+ * [0] permute, [1] P2M, [2] M2M, [3] M2L, [4] L2L, [5] L2P, [6] P2P + finalize, [7] total.  fmm_evaluate_profiled is
  * fmm_evaluate with CUDA events between the stages (it synchronises the stream). */
 fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field,
                                  void* cuda_stream, double* h_stage_ms);
@@ -113,8 +113,17 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
  * tests to cross-check), 2 = as 0 but M2L by the two-pairs-per-thread packed-f32x2 kernel (m2l_packed.cu). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
+/* Schedule of subsequent fmm_evaluate / fmm_evaluate_host calls on this plan.  0 (default) = concurrent: the call forks
+ * three internal streams from cuda_stream and joins them back before it returns control of the stream -- the near field
+ * (P2P) runs beside the whole far-field chain and the M2M pass beside the leaf-level M2L; for the caller the call is
+ * still one asynchronous operation in cuda_stream order.  1 = serial: every kernel is launched on cuda_stream itself
+ * (what fmm_evaluate_profiled always does).  Both schedules run the same kernels on the same data; results agree to the
+ * order of the floating-point atomics. */
+fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial);
+
 /* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M
- * and one L2L per level, M2L (when the weak list is not empty), L2P, P2P.  cudaMemset nodes are not counted. */
+ * and one L2L per level, M2L (when the weak list is not empty; two launches -- leaf level and upper levels -- in the
+ * concurrent schedule with the register kernels), L2P, P2P, finalize.  cudaMemset nodes are not counted. */
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h_launches_per_evaluate);
 
 /* Thread-local, NUL-terminated description of the last failure on the calling thread ("" if none). */

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstring>
 #include <new>
+#include <utility>
 
 #include "internal.cuh"
 
@@ -97,6 +98,7 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
             build_lists(P, st);
             const size_t es = esize(dtype);
             P.pq.alloc((size_t)N * 4 * es);
+            P.near.alloc((size_t)N * 4 * es);
             P.far.alloc((size_t)N * 4 * es);
             P.Mc.alloc((size_t)P.n_boxes * P.Kp * es);
             P.Lc.alloc((size_t)P.n_boxes * P.Kp * es);
@@ -224,6 +226,12 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms) {
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h) {
     if (!plan || !h) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
     *h = evaluate_launches(plan->P);
+    return FMM_OK;
+}
+
+fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial) {
+    if (!plan || serial < 0 || serial > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    plan->P.serial = serial != 0;
     return FMM_OK;
 }
 

@@ -195,8 +195,27 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
                 const T l = sL[w][n * n + n + m];
                 phi += l * R; gx += l * GX; gy += l * GY; gz += l * GZ;
             });
-            far[st + i] = make4<T>(phi, gx * inva, gy * inva, gz * inva);
+            far[st + i] = make4<T>(phi, gx * inva, gy * inva, gz * inva);  // (phi_far, grad phi_far), tree order
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ finalize (a10)
+// u = -(phi_far + phi_near)/4pi (eqs. (2), (9), (14)), field = -grad u = (grad phi_far + grad phi_near)/4pi (reading S2),
+// scattered back to input order.  Separate from L2P and P2P so that those two never wait for one another.
+template <typename T>
+__global__ void finalize_k(const typename V4<T>::type* __restrict__ far, const typename V4<T>::type* __restrict__ near,
+                           const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field, int64_t N) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const typename V4<T>::type f = far[k], nr = near[k];
+    const T inv4pi = T(0.079577471545947667884441881686257);
+    const int64_t io = perm[k];
+    if (pot) pot[io] = -(f.x + nr.x) * inv4pi;
+    if (field) {
+        field[3 * io] = (f.y + nr.y) * inv4pi;
+        field[3 * io + 1] = (f.z + nr.z) * inv4pi;
+        field[3 * io + 2] = (f.w + nr.w) * inv4pi;
     }
 }
 
@@ -389,7 +408,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2l_k(int p, int s, int6
     for (int idx = lane; idx < K; idx += 32) Lc[gc * Kp + idx] += wsm[w].u[idx];
 }
 
-// ------------------------------------------------------------------------------------------------ P2P (a9) + finalize (a10)
+// ------------------------------------------------------------------------------------------------ P2P (a9)
 // One target leaf per CTA.  Threads are arranged as (target group, source slice): each thread keeps TPT targets in
 // registers and walks every nslices-th source of the shared-memory tile; partial sums are combined through shared memory.
 constexpr int P2P_THREADS = 128;
@@ -399,8 +418,7 @@ constexpr int P2P_TILE = 512;
 template <typename T>
 __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ leaf_start,
                                                      const int32_t* __restrict__ leaf_cnt, const int64_t* __restrict__ strong_off,
-                                                     const int32_t* __restrict__ strong_src, const typename V4<T>::type* __restrict__ far,
-                                                     const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field) {
+                                                     const int32_t* __restrict__ strong_src, typename V4<T>::type* __restrict__ near) {
     using T4 = typename V4<T>::type;
     __shared__ T4 sh[P2P_TILE];
     __shared__ T red[P2P_THREADS * P2P_TPT * 4];
@@ -409,7 +427,6 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
     const int tst = leaf_start[leaf], tcnt = leaf_cnt[leaf];
     if (tcnt == 0) return;
     const int64_t e0 = strong_off[leaf], e1 = strong_off[leaf + 1];
-    const T inv4pi = T(0.079577471545947667884441881686257);
     for (int tbase = 0; tbase < tcnt; tbase += P2P_THREADS * P2P_TPT) {
         const int tn = min(tcnt - tbase, P2P_THREADS * P2P_TPT);
         int ntg = (tn + P2P_TPT - 1) / P2P_TPT, ntgp = 1;
@@ -476,15 +493,7 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
                 const T* r = red + ((s2 * ntgp + g2) * P2P_TPT + t2) * 4;
                 a0 += r[0]; a1 += r[1]; a2 += r[2]; a3 += r[3];
             }
-            const int k = tst + tbase + ti;
-            const T4 f = far[k];
-            const int64_t i = perm[k];
-            if (pot) pot[i] = -(f.x + a0) * inv4pi;                 // eqs. (2), (9), (14)
-            if (field) {                                            // field = -grad u  (reading S2)
-                field[3 * i] = (f.y + a1) * inv4pi;
-                field[3 * i + 1] = (f.z + a2) * inv4pi;
-                field[3 * i + 2] = (f.w + a3) * inv4pi;
-            }
+            near[tst + tbase + ti] = make4<T>(a0, a1, a2, a3);  // (phi_near, grad phi_near), tree order
         }
     }
 }
@@ -514,6 +523,23 @@ void dispatch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
 
 bool g_const_uploaded = false;
 
+// Internal streams of a plan (created on first use).  s_far / s_up have the highest priority, s_near the lowest, so that
+// the latency-bound far-field kernels get SM resources as soon as they are launched and P2P fills whatever is left.
+void ensure_streams(const Plan& Pl) {
+    if (Pl.s_far) return;
+    int lo = 0, hi = 0;
+    FMM_CUDA_CHECK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    FMM_CUDA_CHECK(cudaStreamCreateWithPriority(&Pl.s_far, cudaStreamNonBlocking, hi));
+    FMM_CUDA_CHECK(cudaStreamCreateWithPriority(&Pl.s_up, cudaStreamNonBlocking, hi));
+    FMM_CUDA_CHECK(cudaStreamCreateWithPriority(&Pl.s_near, cudaStreamNonBlocking, lo));
+    for (cudaEvent_t* e : {&Pl.e_fork, &Pl.e_perm, &Pl.e_p2m, &Pl.e_up, &Pl.e_near, &Pl.e_done})
+        FMM_CUDA_CHECK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+}
+
+// One evaluate.  ev == nullptr: the production schedule -- three internal streams forked from / joined to the caller's
+// stream: far chain (permute, P2M, leaf-level M2L, L2L, L2P, finalize), upward chain (M2M levels, then the M2L of the upper
+// levels, concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and finalize).
+// ev != nullptr: the same kernels back to back on the caller's stream with an event after every stage (profiling).
 template <typename T>
 void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
     using T4 = typename V4<T>::type;
@@ -521,60 +547,106 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
     const int p = Pl.p, s = Pl.s, L = Pl.L;
     const int64_t N = Pl.N;
+    const bool serial = ev != nullptr || Pl.serial;
+    cudaStream_t sF = st, sU = st, sN = st;
+    if (!serial) {
+        ensure_streams(Pl);
+        sF = Pl.s_far; sU = Pl.s_up; sN = Pl.s_near;
+        FMM_CUDA_CHECK(cudaEventRecord(Pl.e_fork, st));
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(sF, Pl.e_fork, 0));
+    }
     auto mark = [&](int i) { if (ev) FMM_CUDA_CHECK(cudaEventRecord(ev[i], st)); };
-    mark(0);
-    permute_k<T><<<nblocks(N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, Pl.src_slot.p,
-                                                  sizeof(T) == 4 ? Pl.srcg.p : nullptr, N);
-    FMM_CUDA_CHECK(cudaGetLastError());
-    FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, st));
-    mark(1);
-    dispatch_p2m_l2p<T>(Pl, false, st);
-    FMM_CUDA_CHECK(cudaGetLastError());
-    mark(2);
+    auto after = [&](cudaStream_t waiter, cudaStream_t producer, cudaEvent_t e) {  // waiter continues after what producer has queued
+        if (serial) return;
+        FMM_CUDA_CHECK(cudaEventRecord(e, producer));
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(waiter, e, 0));
+    };
     // m2l_variant: 0 = register kernels (one translation per thread), 1 = generic kernels, 2 = as 0 but M2L two pairs per thread (f32x2)
     const bool fast = Pl.m2l_variant != 1 && xlate_fast_available(p, Pl.dtype);
     const bool packed = Pl.m2l_variant == 2 && m2l_packed_available(p, Pl.dtype);
+    const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
+    const int64_t leaf0 = Pl.level_off[L];
+    auto launch_p2p = [&](cudaStream_t q) {
+        if (fast_p2p) p2p_fast_launch(Pl, q);
+        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
+                                                                  Pl.strong_src.p, (T4*)Pl.near.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    };
+
+    mark(0);
+    permute_k<T><<<nblocks(N, 256), 256, 0, sF>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, Pl.src_slot.p,
+                                                  sizeof(T) == 4 ? Pl.srcg.p : nullptr, N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    after(sN, sF, Pl.e_perm);
+    if (!serial) launch_p2p(sN);
+    FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, sF));
+    mark(1);
+    dispatch_p2m_l2p<T>(Pl, false, sF);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(2);
     if (fast && L > 0)  // the register kernels accumulate into the parents
-        FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), st));
+        FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), sF));
+    // the M2L of the leaf level needs only the P2M output: with the register kernels it runs on sF while M2M and the upper
+    // levels' M2L run on sU (weak pairs are sorted by target id, hence by level; rows of different levels are disjoint)
+    const int64_t w_leaf = (int64_t)Pl.weak_level_off.size() > L ? Pl.weak_level_off[L] : 0;
+    const bool split = !serial && fast && L > 0;
+    if (split) after(sU, sF, Pl.e_p2m);
+    cudaStream_t sM = split ? sU : sF;
     for (int l = L; l >= 1; --l) {
-        if (fast) { xlate_fast_launch(Pl, 0, l, st); continue; }
+        if (fast) { xlate_fast_launch(Pl, 0, l, sM); continue; }
         const int64_t nbp = (int64_t)1 << (s * (l - 1));
-        m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbp, Pl.box_count.p,
+        m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sM>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbp, Pl.box_count.p,
                                                                                 Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Mc.p, tp);
         FMM_CUDA_CHECK(cudaGetLastError());
     }
     mark(3);
     if (Pl.n_weak > 0) {
-        if (packed) m2l_packed_launch(Pl, st);
-        else if (fast) xlate_fast_launch(Pl, 1, 0, st);
-        else
-            m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(
+        auto m2l_range = [&](int64_t e0, int64_t e1, cudaStream_t q) {
+            if (e1 <= e0) return;
+            if (packed) m2l_packed_launch(Pl, q, e0, e1);
+            else xlate_fast_launch(Pl, 1, 0, q, e0, e1);
+        };
+        if (split) {
+            m2l_range(w_leaf, Pl.n_weak, sF);
+            m2l_range(0, w_leaf, sU);
+        } else if (fast) {
+            m2l_range(0, Pl.n_weak, sF);
+        } else {
+            m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(
                 p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
+        }
         FMM_CUDA_CHECK(cudaGetLastError());
     }
+    if (split) after(sF, sU, Pl.e_up);
     mark(4);
     for (int l = 1; l <= L; ++l) {
-        if (fast) { xlate_fast_launch(Pl, 2, l, st); continue; }
+        if (fast) { xlate_fast_launch(Pl, 2, l, sF); continue; }
         const int64_t nbc = (int64_t)1 << (s * l);
-        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
+        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
                                                                                 Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Lc.p, tp);
         FMM_CUDA_CHECK(cudaGetLastError());
     }
     mark(5);
-    dispatch_p2m_l2p<T>(Pl, true, st);
+    dispatch_p2m_l2p<T>(Pl, true, sF);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(6);
-    const int64_t leaf0 = Pl.level_off[L];
-    if (sizeof(T) == 4 && Pl.m2l_variant != 1) p2p_fast_launch(Pl, d_pot, d_field, st);
-    else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
-                                                            Pl.strong_src.p, (const T4*)Pl.far.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
+    if (serial) launch_p2p(st);
+    else after(sF, sN, Pl.e_near);
+    finalize_k<T><<<nblocks(N, 256), 256, 0, sF>>>((const T4*)Pl.far.p, (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field, N);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(7);
+    after(st, sF, Pl.e_done);
 }
 
 }  // namespace
 
-int64_t evaluate_launches(const Plan& P) { return 4 + 2 * (int64_t)P.L + (P.n_weak > 0 ? 1 : 0); }
+int64_t evaluate_launches(const Plan& P) {
+    const bool fast = P.m2l_variant != 1 && xlate_fast_available(P.p, P.dtype);
+    const int64_t w_leaf = (int64_t)P.weak_level_off.size() > P.L ? P.weak_level_off[P.L] : 0;
+    int64_t m2l = P.n_weak > 0 ? 1 : 0;
+    if (fast && !P.serial && P.L > 0 && w_leaf > 0 && w_leaf < P.n_weak) m2l = 2;  // leaf level and upper levels on two streams
+    return 5 + 2 * (int64_t)P.L + m2l;  // permute, P2M, L2P, P2P, finalize + M2M/L2L per level + M2L
+}
 
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
     if (!g_const_uploaded) {

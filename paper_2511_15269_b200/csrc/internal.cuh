@@ -92,12 +92,24 @@ struct Plan {
     // evaluate scratch
     DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
-    DevBuf<char> far;     // N x 4 dtype: (phi_far, grad phi_far) tree order
+    DevBuf<char> far;     // N x 4 dtype: (phi_far, grad phi_far) tree order, L2P -> finalize
+    DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> finalize
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
     DevBuf<float> srcg;
     DevBuf<int32_t> src_slot;
     int src_G = 0;
     DevBuf<char> h2d_q, d2h_out;  // staging for fmm_evaluate_host
+    // internal streams / events of the concurrent evaluate schedule (evaluate.cu), created on first use
+    mutable cudaStream_t s_far = nullptr, s_up = nullptr, s_near = nullptr;
+    mutable cudaEvent_t e_fork = nullptr, e_perm = nullptr, e_p2m = nullptr, e_up = nullptr, e_near = nullptr, e_done = nullptr;
+    bool serial = false;  // true: every kernel on the caller's stream (fmm_plan_set_schedule)
+    ~Plan() {
+        for (cudaStream_t q : {s_far, s_up, s_near})
+            if (q) cudaStreamDestroy(q);
+        for (cudaEvent_t e : {e_fork, e_perm, e_p2m, e_up, e_near, e_done})
+            if (e) cudaEventDestroy(e);
+    }
+    Plan() = default;
     double plan_ms[4] = {0, 0, 0, 0};
     double stage_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
@@ -111,11 +123,11 @@ int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evalua
 // xlate_fast.cu: register kernels (one thread per translation).  kind 0 = M2M into level-1 from `level`, 1 = M2L (all
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
 bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
-void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st);
+void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0 = 0, int64_t e1 = -1);  // kind 1: weak pairs [e0, e1)
 // m2l_packed.cu: fp32 M2L with two weak pairs per thread in packed f32x2 arithmetic (p <= 8); results are ADDED to Lc
 bool m2l_packed_available(int p, fmm_dtype dt);
-void m2l_packed_launch(const Plan& P, cudaStream_t st);
+void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1);  // weak pairs [e0, e1)
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
-void p2p_fast_launch(const Plan& P, void* d_pot, void* d_field, cudaStream_t st);
+void p2p_fast_launch(const Plan& P, cudaStream_t st);
 
 }  // namespace fmm

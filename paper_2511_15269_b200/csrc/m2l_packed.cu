@@ -247,7 +247,7 @@ m2l_packed_k(int64_t n, const int32_t* __restrict__ wtgt, const int32_t* __restr
 }
 
 template <int P, int MW = 4, bool SYNC = false>
-void launch_packed(const Plan& Pl, cudaStream_t st) {
+void launch_packed(const Plan& Pl, cudaStream_t st, int64_t e0, int64_t e1) {
     using G = PGeo<P>;
     constexpr size_t smem = (size_t)MW * G::SMEM_WARP;
     static bool attr_set = false;
@@ -255,8 +255,8 @@ void launch_packed(const Plan& Pl, cudaStream_t st) {
         FMM_CUDA_CHECK(cudaFuncSetAttribute(m2l_packed_k<P, MW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    const unsigned grid = (unsigned)((Pl.n_weak + MW * 64 - 1) / (MW * 64));
-    m2l_packed_k<P, MW, SYNC><<<grid, MW * 32, smem, st>>>(Pl.n_weak, Pl.weak_tgt.p, Pl.weak_src.p, Pl.box_ctr.p, (const float*)Pl.box_scale.p,
+    const unsigned grid = (unsigned)((e1 - e0 + MW * 64 - 1) / (MW * 64));
+    m2l_packed_k<P, MW, SYNC><<<grid, MW * 32, smem, st>>>(e1 - e0, Pl.weak_tgt.p + e0, Pl.weak_src.p + e0, Pl.box_ctr.p, (const float*)Pl.box_scale.p,
                                                  (const float*)Pl.Mc.p, (float*)Pl.Lc.p);
 }
 
@@ -264,10 +264,10 @@ void launch_packed(const Plan& Pl, cudaStream_t st) {
 
 bool m2l_packed_available(int p, fmm_dtype dt) { return dt == FMM_F32 && p >= 1 && p <= 8; }
 
-void m2l_packed_launch(const Plan& P, cudaStream_t st) {
-    if (P.n_weak == 0) return;
+void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1) {
+    if (e1 <= e0) return;
     switch (P.p) {
-#define FMM_CASE(PP) case PP: launch_packed<PP>(P, st); break;
+#define FMM_CASE(PP) case PP: launch_packed<PP>(P, st, e0, e1); break;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
         default: set_error("no packed M2L kernel for this order"); throw CudaFail{FMM_ERR_UNSUPPORTED};

@@ -1,6 +1,7 @@
-// p2p_fast.cu -- fp32 near field (a9) + finalize (a10): direct sum over the strong leaf pairs (stage "evdir"
-// PAPER.md:251), fused with u = -(phi_far + phi_near)/4pi, field = (grad phi_far + grad phi_near)/4pi and the scatter
-// back to input order (eq. (2); readings S2, S3).
+// p2p_fast.cu -- fp32 near field (a9): direct sum over the strong leaf pairs (stage "evdir" PAPER.md:251;
+// DESIGN.md reading S3).  Writes (phi_near, grad phi_near) per particle in tree order; finalize_k (evaluate.cu) adds the far field,
+// scales and scatters to input order (a10).  The kernel depends only on the permuted particles, so run_evaluate launches it
+// on a second stream, concurrently with the whole far-field chain.
 //
 // Mapping (differs from north_star's "one target leaf per CTA": one target leaf per WARP):
 //   * a warp owns one target leaf (or a chunk of 32*TPT targets of a large leaf); lanes form ntgp target groups x nsl
@@ -16,6 +17,7 @@
 //     instruction every other cycle, which leaves the issue slots in between for MUFU, the mask, LDS and the loop;
 //   * slices are combined with warp shuffles (no block-level synchronisation anywhere in the kernel).
 #include "internal.cuh"
+#include "tma.cuh"
 
 namespace fmm {
 namespace {
@@ -52,34 +54,13 @@ __device__ __forceinline__ float rsq(float x) {
 constexpr int PW = 4;   // warps per CTA (independent of one another)
 constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two tiles per warp = 8 KB of shared memory
 
-// ---- TMA bulk copy (cp.async.bulk, SASS UBLKCP) + mbarrier, per-warp pipelines
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
 // the leaf population hold zeros (zero charge), so whole groups can be used without masks.
 template <int TPT>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
                                                       const int64_t* __restrict__ strong_off, const int32_t* __restrict__ strong_src,
-                                                      const float4* __restrict__ far, const int32_t* __restrict__ perm,
-                                                      float* __restrict__ pot, float* __restrict__ field, int64_t n_items, int nchunk) {
+                                                      float4* __restrict__ near, int64_t n_items, int nchunk) {
     __shared__ __align__(128) float sm[PW][2][TG * 16];
     __shared__ __align__(8) unsigned long long bars[PW][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -227,35 +208,24 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
         }
     }
     // every lane now holds the full sums of its group; slice sl writes the targets k with k mod nsl == sl
-    const float inv4pi = 0.079577471545947667884441881686257f;
 #pragma unroll
     for (int k = 0; k < TPT; ++k) {
         const int ti = tg * TPT + k;
-        if ((k & (nsl - 1)) == sl && ti < tn) {
-            const int kk = tst + t0 + ti;
-            const float4 f = far[kk];
-            const int64_t i = perm[kk];
-            if (pot) pot[i] = -(f.x + ph[k]) * inv4pi;  // eqs. (2), (9), (14)
-            if (field) {                                // field = -grad u (reading S2); G accumulates +q d / r^3 = -grad phi_near
-                field[3 * i] = (f.y - gx[k]) * inv4pi;
-                field[3 * i + 1] = (f.z - gy[k]) * inv4pi;
-                field[3 * i + 2] = (f.w - gz[k]) * inv4pi;
-            }
-        }
+        // G accumulates +q d / r^3 = -grad phi_near; stored: (phi_near, grad phi_near) in tree order for the L2P finalize
+        if ((k & (nsl - 1)) == sl && ti < tn) near[tst + t0 + ti] = make_float4(ph[k], -gx[k], -gy[k], -gz[k]);
     }
 }
 
 }  // namespace
 
-void p2p_fast_launch(const Plan& P, void* d_pot, void* d_field, cudaStream_t st) {
+void p2p_fast_launch(const Plan& P, cudaStream_t st) {
     constexpr int TPT = 4;
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
     const int64_t n_items = P.n_leaves * nchunk;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
-                                              P.strong_off.p, P.strong_src.p, (const float4*)P.far.p, P.perm.p, (float*)d_pot, (float*)d_field,
-                                              n_items, nchunk);
+                                              P.strong_off.p, P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
 
 }  // namespace fmm

@@ -11,10 +11,11 @@
 // batch of small, ragged mat-vecs (block sizes 1..2p+1) with a different right-hand side per interaction, which maps
 // badly onto 32 lanes (K = 81 is 2.5 warps wide, rows have different lengths).  With one interaction per lane the whole
 // warp executes the same fully unrolled instruction stream, all matrix entries are immediates, the state vector lives
-// in registers, and there is no shuffle or shared-memory traffic inside the operator.  Shared memory is used only to
-// transpose: a warp loads its 32 source rows coalesced, each lane reads its own row with conflict-free LDS.128 (row
-// stride an odd number of 16-byte units), results go back the same way and are summed over runs of equal targets
-// (the lists are sorted by target) before one atomicAdd per coefficient and run.
+// in registers, and there is no shuffle or shared-memory traffic inside the operator.  Shared memory is only the staging
+// area: every lane fetches its source row with one TMA bulk copy (cp.async.bulk + mbarrier) and reads it with conflict-free
+// LDS.128 (row stride an odd number of 16-byte units); results go back the same way and are summed over runs of equal
+// targets (the lists are sorted by target) before one atomicAdd per coefficient and run.
+#include "tma.cuh"
 #include "xlate_reg.cuh"
 
 namespace fmm {
@@ -186,19 +187,22 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
             }
         }
     }
+    const unsigned vmask = __ballot_sync(0xffffffffu, gs >= 0);
     if constexpr (!SYNC) {
-        if (__ballot_sync(0xffffffffu, gs >= 0) == 0) return;
+        if (vmask == 0) return;
     }
 
-    // coalesced load of the warp's 32 source rows into shared memory
-    const V* in16 = reinterpret_cast<const V*>(a.in);
-#pragma unroll
-    for (int it = 0; it < G::CH; ++it) {
-        const int idx = it * 32 + lane;
-        const int r = idx / G::CH, c = idx - r * G::CH;
-        const int g = __shfl_sync(0xffffffffu, gs, r);
-        if (g >= 0) sm[r * G::KSB + c] = in16[(int64_t)g * G::CH + c];
+    // every lane fetches its own source row (CH * 16 contiguous bytes) with one TMA bulk copy; all 32 copies of the warp
+    // complete on one mbarrier, so the whole batch is in flight at once while the geometry is being loaded
+    constexpr uint32_t ROWB = G::CH * 16;
+    const uint32_t bar = smem_u32(reinterpret_cast<unsigned long long*>(smraw + (size_t)XW * 32 * G::KSB * 16) + warp);
+    if (lane == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
     }
+    __syncwarp();
+    if (gs >= 0) bulk_g2s(smem_u32(sm + lane * G::KSB), reinterpret_cast<const char*>(a.in) + (int64_t)gs * ROWB, ROWB, bar);
+    if (lane == 0) mbar_expect_tx(bar, (uint32_t)__popc(vmask) * ROWB);
     T bx = T(0), by = T(0), bz = T(1), a_old = T(1), a_new = T(1);
     if (gs >= 0) {
         const T* sc = reinterpret_cast<const T*>(a.scale);
@@ -208,7 +212,7 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
         a_old = sc[gs];
         a_new = sc[gt];
     }
-    __syncwarp();
+    mbar_wait(bar, 0);
 
     T v[G::KV];
     V* row = sm + lane * G::KSB;
@@ -230,44 +234,38 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
     }
     __syncwarp();
 
-    // sum runs of equal targets (lists are sorted by target), one atomicAdd per coefficient and run
+    // sum runs of equal targets (lists are sorted by target), one atomicAdd per coefficient and run.  Run heads are found
+    // with one ballot; inside a run the row loop has warp-uniform bounds, so its loads are independent and pipeline.
     const T* smT = reinterpret_cast<const T*>(sm);
     T* out = reinterpret_cast<T*>(a.out);
     constexpr int RS = G::KSB * G::E;  // shared row stride in elements
-    T acc[G::NJ];
+    const int prev = __shfl_up_sync(0xffffffffu, gt, 1);
+    unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || gt != prev);
+    while (heads) {
+        const int r0 = __ffs(heads) - 1;
+        heads &= heads - 1;
+        const int r1 = heads ? __ffs(heads) - 1 : 32;
+        const int t = __shfl_sync(0xffffffffu, gt, r0);
+        if (t < 0) continue;  // padding lanes / empty boxes
+        T acc[G::NJ];
 #pragma unroll
-    for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
-    int cur = __shfl_sync(0xffffffffu, gt, 0);
-#pragma unroll 4
-    for (int r = 0; r < 32; ++r) {
-        const int t = __shfl_sync(0xffffffffu, gt, r);
-        if (t != cur) {
-            if (cur >= 0) {
-#pragma unroll
-                for (int j = 0; j < G::NJ; ++j)
-                    if (lane + 32 * j < G::K) atomicAdd(out + (int64_t)cur * G::Kp + lane + 32 * j, acc[j]);
-            }
-#pragma unroll
-            for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
-            cur = t;
-        }
-        if (t >= 0) {
+        for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
+#pragma unroll 8
+        for (int r = r0; r < r1; ++r) {
 #pragma unroll
             for (int j = 0; j < G::NJ; ++j)
                 if (lane + 32 * j < G::K) acc[j] += smT[r * RS + lane + 32 * j];
         }
-    }
-    if (cur >= 0) {
 #pragma unroll
         for (int j = 0; j < G::NJ; ++j)
-            if (lane + 32 * j < G::K) atomicAdd(out + (int64_t)cur * G::Kp + lane + 32 * j, acc[j]);
+            if (lane + 32 * j < G::K) atomicAdd(out + (int64_t)t * G::Kp + lane + 32 * j, acc[j]);
     }
 }
 
 template <typename T, int P, int KIND, int XW = 4, bool SYNC = false>
 void launch(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
-    constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16;
+    constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;  // rows + one mbarrier per warp
     static bool attr_set = false;
     if (!attr_set) {
         FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -291,16 +289,17 @@ bool dispatch(int p, const XArgs& a, cudaStream_t st) {
 
 bool xlate_fast_available(int p, fmm_dtype dt) { return dt == FMM_F32 && p >= 1 && p <= 8; }
 
-void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st) {
+void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     XArgs a{};
     a.box_count = P.box_count.p;
     a.ctr = P.box_ctr.p;
     a.scale = P.box_scale.p;
     a.s = P.s;
     if (kind == 1) {
-        a.n = P.n_weak;
-        a.tgt = P.weak_tgt.p;
-        a.src = P.weak_src.p;
+        if (e1 < 0) e1 = P.n_weak;
+        a.n = e1 - e0;
+        a.tgt = P.weak_tgt.p + e0;
+        a.src = P.weak_src.p + e0;
         a.in = P.Mc.p;
         a.out = P.Lc.p;
     } else {
@@ -310,7 +309,7 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st) {
         a.in = kind == 0 ? P.Mc.p : P.Lc.p;
         a.out = kind == 0 ? P.Mc.p : P.Lc.p;
     }
-    if (a.n == 0) return;
+    if (a.n <= 0) return;
     bool ok = false;
     if (kind == 0) ok = dispatch<float, 0>(P.p, a, st);
     else if (kind == 1) ok = dispatch<float, 1>(P.p, a, st);

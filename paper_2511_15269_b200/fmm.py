@@ -17,7 +17,7 @@ FMM_F32, FMM_F64 = 0, 1
 FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
-           "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_launches", "fmm_last_error",
+           "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
            "fmm_version"]
 
 
@@ -52,6 +52,7 @@ def lib():
         L.fmm_plan_copy_lists.argtypes = [vp, i64p, i32p, i64p, i32p]
         L.fmm_plan_timings.argtypes = [vp, dp]
         L.fmm_plan_set_m2l_variant.argtypes = [vp, C.c_int]
+        L.fmm_plan_set_schedule.argtypes = [vp, C.c_int]
         L.fmm_plan_launches.argtypes = [vp, i64p]
         L.fmm_last_error.restype = C.c_char_p
         L.fmm_version.restype = C.c_char_p
@@ -150,6 +151,10 @@ def fmm_plan_launches(plan):
     v = C.c_int64()
     _check(lib().fmm_plan_launches(plan, C.byref(v)))
     return v.value
+
+
+def fmm_plan_set_schedule(plan, serial):
+    _check(lib().fmm_plan_set_schedule(plan, int(serial)))
 
 
 def fmm_plan_set_m2l_variant(plan, variant):

@@ -196,6 +196,30 @@ def test_kernel_families_agree_with_the_oracle_fp32(N, N_max, s, p):
     P.close()
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_concurrent_and_serial_schedules_agree(dtype):
+    """fmm_plan_set_schedule: the forked-stream schedule (default) and the single-stream schedule run the same kernels;
+    both must meet the tolerance, repeatedly on one plan (stream joins must order consecutive evaluates), also on a side stream."""
+    pos, q = inputs.uniform_cube(20000, 12, dtype)
+    p = 8 if dtype == np.float32 else 6
+    Po = O.Plan(pos, p, 32, 3, 0.77)
+    uo, fo = Po.evaluate(q)
+    P = gpu_plan(pos, p, 32, 3)
+    for serial in (0, 1, 0):
+        fmm.fmm_plan_set_schedule(P.handle, serial)
+        for rep in range(3):
+            u, f = gpu_eval(P, q if rep != 1 else -q)
+            sgn = 1.0 if rep != 1 else -1.0
+            assert rel2(sgn * u, uo) <= TOL[dtype] and rel2(sgn * f, fo) <= TOL[dtype], (serial, rep)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        tq = torch.from_numpy(q).cuda()
+        u, f = P.evaluate(tq)
+    side.synchronize()
+    assert rel2(u.cpu().numpy(), uo) <= TOL[dtype]
+    P.close()
+
+
 def test_potential_only_and_field_only_and_host_path():
     pos, q = inputs.uniform_cube(2000, 33, np.float32)
     P = gpu_plan(pos, 5, 32, 3)
