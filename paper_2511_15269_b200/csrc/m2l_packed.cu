@@ -16,6 +16,7 @@
 // units, so the per-lane LDS.128 are conflict-free).  When both pairs of every lane have the same target the halves are
 // added in registers; rows are then summed over runs of equal targets and added to D with one atomicAdd per coefficient
 // and run.
+#include "tma.cuh"
 #include "xlate_reg.cuh"
 
 namespace fmm {
@@ -127,12 +128,6 @@ __device__ __forceinline__ void m2l_pair(f2 (&v)[KV], f2 ct, f2 st, f2 cp, f2 sp
     sync();
     az_all<P, -1>(v, cp, sp);
 }
-
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int P, int MW, bool SYNC>
 __global__ void __launch_bounds__(MW * 32, 8 / MW)

@@ -1,4 +1,4 @@
-// tma.cuh -- TMA bulk copies (cp.async.bulk, SASS UBLKCP) completing on an mbarrier; used per warp (one warp = one
+// tma.cuh -- asynchronous global->shared copies: TMA bulk copies (cp.async.bulk, SASS UBLKCP) completing on an mbarrier; used per warp (one warp = one
 // pipeline) by the P2P source staging and by the coefficient-row loads of the register translation kernels.
 #pragma once
 #include <stdint.h>
@@ -25,5 +25,12 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 
 __device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// Ampere-style 16-byte asynchronous copies (SASS LDGSTS), per thread
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 }  // namespace fmm

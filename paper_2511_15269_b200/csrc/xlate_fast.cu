@@ -192,8 +192,8 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
         if (vmask == 0) return;
     }
 
-    // every lane fetches its own source row (CH * 16 contiguous bytes) with one TMA bulk copy; all 32 copies of the warp
-    // complete on one mbarrier, so the whole batch is in flight at once while the geometry is being loaded
+    // source rows (CH * 16 contiguous bytes each) arrive by TMA bulk copies that complete on one mbarrier per warp, so the
+    // whole batch is in flight at once while the geometry is being loaded
     constexpr uint32_t ROWB = G::CH * 16;
     const uint32_t bar = smem_u32(reinterpret_cast<unsigned long long*>(smraw + (size_t)XW * 32 * G::KSB * 16) + warp);
     if (lane == 0) {
@@ -201,7 +201,18 @@ __global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
         mbar_fence_init();
     }
     __syncwarp();
-    if (gs >= 0) bulk_g2s(smem_u32(sm + lane * G::KSB), reinterpret_cast<const char*>(a.in) + (int64_t)gs * ROWB, ROWB, bar);
+    // consecutive lanes with consecutive source ids (siblings are numbered consecutively and the lists are sorted) read one
+    // contiguous piece of the coefficient array: the first lane of such a run copies the whole run (possible when the shared
+    // rows are contiguous too, KSB == CH); a bulk copy is issued by one elected lane at a time, so fewer copies matter
+    {
+        const int gprev = __shfl_up_sync(0xffffffffu, gs, 1);
+        const bool head = lane == 0 || gs < 0 || gprev < 0 || gs != gprev + 1 || G::KSB != G::CH;
+        const unsigned hm = __ballot_sync(0xffffffffu, head);
+        const unsigned above = lane == 31 ? 0u : (hm >> (lane + 1));
+        const int len = above ? __ffs(above) : 32 - lane;
+        if (head && gs >= 0)
+            bulk_g2s(smem_u32(sm + lane * G::KSB), reinterpret_cast<const char*>(a.in) + (int64_t)gs * ROWB, (uint32_t)len * ROWB, bar);
+    }
     if (lane == 0) mbar_expect_tx(bar, (uint32_t)__popc(vmask) * ROWB);
     T bx = T(0), by = T(0), bz = T(1), a_old = T(1), a_new = T(1);
     if (gs >= 0) {
