@@ -537,8 +537,8 @@ void ensure_streams(const Plan& Pl) {
 }
 
 // One evaluate.  ev == nullptr: the production schedule -- three internal streams forked from / joined to the caller's
-// stream: far chain (permute, P2M, leaf-level M2L, L2L, L2P, finalize), upward chain (M2M levels, then the M2L of the upper
-// levels, concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and finalize).
+// stream: far chain (permute, P2M, leaf-level M2L, L2P, finalize), tree chain (M2M levels, the M2L of the upper levels, then
+// the L2L levels, all concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and finalize).
 // ev != nullptr: the same kernels back to back on the caller's stream with an event after every stage (profiling).
 template <typename T>
 void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
@@ -617,15 +617,18 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
         }
         FMM_CUDA_CHECK(cudaGetLastError());
     }
-    if (split) after(sF, sU, Pl.e_up);
     mark(4);
+    // L2L (a7).  The register kernels ADD into the children with atomics, exactly like the M2L, so in the split schedule the
+    // whole downward pass runs on sU right behind the upper levels' M2L and beside the leaf-level M2L on sF.
+    cudaStream_t sL = split ? sU : sF;
     for (int l = 1; l <= L; ++l) {
-        if (fast) { xlate_fast_launch(Pl, 2, l, sF); continue; }
+        if (fast) { xlate_fast_launch(Pl, 2, l, sL); continue; }
         const int64_t nbc = (int64_t)1 << (s * l);
-        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
+        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sL>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
                                                                                 Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Lc.p, tp);
         FMM_CUDA_CHECK(cudaGetLastError());
     }
+    if (split) after(sF, sU, Pl.e_up);
     mark(5);
     dispatch_p2m_l2p<T>(Pl, true, sF);
     FMM_CUDA_CHECK(cudaGetLastError());

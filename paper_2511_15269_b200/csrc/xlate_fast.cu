@@ -169,7 +169,7 @@ struct XArgs {
 
 // XW warps per CTA; SYNC = lockstep barriers (all warps then run the operator, also on padding lanes)
 template <typename T, int P, int KIND, int XW, bool SYNC>
-__global__ void __launch_bounds__(XW * 32) xlate_fast_k(XArgs a) {
+__global__ void __launch_bounds__(XW * 32, XW == 8 ? 2 : (XW == 4 ? 4 : 1)) xlate_fast_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
