@@ -140,31 +140,67 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
     const int st = box_start[g], cnt = box_count[g];
     const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
     const T inva = T(1) / scale[g];
-    T acc[NJ];
+    if constexpr (NJ * 32 * sizeof(T) / 4 <= 128) {
+        // every lane accumulates all K coefficients of its own particles in registers; one recursive-halving reduce-scatter
+        // (K + K/2 + ... shuffles instead of 5 K) then leaves coefficients NJ*lane .. NJ*lane + NJ-1 on lane `lane`
+        constexpr int KP = NJ * 32;
+        T w[KP];
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) acc[j] = T(0);
-    for (int base = 0; base < cnt; base += 32) {
-        const int i = base + lane;
-        T x = 0, y = 0, z = 0, q = 0;
-        if (i < cnt) {
-            const typename V4<T>::type v = pq[st + i];
-            x = (T)((double)v.x - cx) * inva;
-            y = (T)((double)v.y - cy) * inva;
-            z = (T)((double)v.z - cz) * inva;
-            q = v.w;
+        for (int i = 0; i < KP; ++i) w[i] = T(0);
+        for (int base = 0; base < cnt; base += 32) {
+            const int i = base + lane;
+            T x = 0, y = 0, z = 0, q = 0;
+            if (i < cnt) {
+                const typename V4<T>::type v = pq[st + i];
+                x = (T)((double)v.x - cx) * inva;
+                y = (T)((double)v.y - cy) * inva;
+                z = (T)((double)v.z - cz) * inva;
+                q = v.w;
+            }
+            regular_rec<P, T>(x, y, z, [&](int n, int m, T val) { w[n * n + n + m] += q * val; });
         }
-        regular_rec<P, T>(x, y, z, [&](int n, int m, T val) {
-            const int idx = n * n + n + m;
-            T v = q * val * gnorm<T>(idx);
 #pragma unroll
-            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-            if (lane == (idx & 31)) acc[idx >> 5] += v;
-        });
-    }
+        for (int bit = 16, h = KP / 2; bit > 0; bit >>= 1, h >>= 1) {
+            const bool up = (lane & bit) != 0;
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-        const int idx = lane + 32 * j;
-        if (idx < K) Mc[g * Kp + idx] = acc[j];
+            for (int i = 0; i < h; ++i) {
+                const T send = up ? w[i] : w[i + h];
+                const T keep = up ? w[i + h] : w[i];
+                w[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int idx = NJ * lane + j;
+            if (idx < K) Mc[g * Kp + idx] = w[j] * gnorm<T>(idx);
+        }
+    } else {
+        T acc[NJ];
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) acc[j] = T(0);
+        for (int base = 0; base < cnt; base += 32) {
+            const int i = base + lane;
+            T x = 0, y = 0, z = 0, q = 0;
+            if (i < cnt) {
+                const typename V4<T>::type v = pq[st + i];
+                x = (T)((double)v.x - cx) * inva;
+                y = (T)((double)v.y - cy) * inva;
+                z = (T)((double)v.z - cz) * inva;
+                q = v.w;
+            }
+            regular_rec<P, T>(x, y, z, [&](int n, int m, T val) {
+                const int idx = n * n + n + m;
+                T v = q * val * gnorm<T>(idx);
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+                if (lane == (idx & 31)) acc[idx >> 5] += v;
+            });
+        }
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int idx = lane + 32 * j;
+            if (idx < K) Mc[g * Kp + idx] = acc[j];
+        }
     }
 }
 
