@@ -99,7 +99,7 @@ fmm_status fmm_plan_copy_lists(const fmm_plan* plan, int64_t* h_weak_off, int32_
                                int64_t* h_strong_off, int32_t* h_strong_src);
 
 /* Per-stage device times of the most recent fmm_evaluate_profiled call, in milliseconds (HOST out, 8 doubles):
- * [0] permute, [1] P2M, [2] M2M, [3] M2L, [4] L2L, [5] L2P, [6] P2P + finalize, [7] total.  fmm_evaluate_profiled is
+ * [0] permute, [1] P2M, [2] M2M, [3] M2L, [4] L2L, [5] L2P + finalize, [6] P2P, [7] total.  fmm_evaluate_profiled is
  * fmm_evaluate with CUDA events between the stages (it synchronises the stream). */
 fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field,
                                  void* cuda_stream, double* h_stage_ms);
@@ -123,7 +123,7 @@ fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial);
 
 /* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M
  * and one L2L per level, M2L (when the weak list is not empty; two launches -- leaf level and upper levels -- in the
- * concurrent schedule with the register kernels), L2P, P2P, finalize.  cudaMemset nodes are not counted. */
+ * concurrent schedule with the register kernels), P2P, L2P (which also finalizes).  cudaMemset nodes are not counted. */
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h_launches_per_evaluate);
 
 /* Thread-local, NUL-terminated description of the last failure on the calling thread ("" if none). */

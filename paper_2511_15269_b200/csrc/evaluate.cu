@@ -204,12 +204,13 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
     }
 }
 
-// ------------------------------------------------------------------------------------------------ L2P (a8), warp per leaf
+// ------------------------------------------------------------------------------------------------ L2P (a8) + finalize (a10), warp per leaf
 template <typename T, int P>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
                                                               const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
                                                               const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves, int Kp,
-                                                              const T* __restrict__ Lc, typename V4<T>::type* __restrict__ far) {
+                                                              const T* __restrict__ Lc, const typename V4<T>::type* __restrict__ near,
+                                                              const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field) {
     constexpr int K = (P + 1) * (P + 1);
     __shared__ T sL[WARPS_PER_BLOCK][K];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -231,27 +232,18 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
                 const T l = sL[w][n * n + n + m];
                 phi += l * R; gx += l * GX; gy += l * GY; gz += l * GZ;
             });
-            far[st + i] = make4<T>(phi, gx * inva, gy * inva, gz * inva);  // (phi_far, grad phi_far), tree order
+            // finalize (a10): add the near field written by P2P; u = -(phi_far + phi_near)/4pi (eqs. (2), (9), (14)),
+            // field = -grad u = (grad phi_far + grad phi_near)/4pi (reading S2); scatter back to input order
+            const typename V4<T>::type nr = near[st + i];
+            const T inv4pi = T(0.079577471545947667884441881686257);
+            const int64_t io = perm[st + i];
+            if (pot) pot[io] = -(phi + nr.x) * inv4pi;
+            if (field) {
+                field[3 * io] = (gx * inva + nr.y) * inv4pi;
+                field[3 * io + 1] = (gy * inva + nr.z) * inv4pi;
+                field[3 * io + 2] = (gz * inva + nr.w) * inv4pi;
+            }
         }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------ finalize (a10)
-// u = -(phi_far + phi_near)/4pi (eqs. (2), (9), (14)), field = -grad u = (grad phi_far + grad phi_near)/4pi (reading S2),
-// scattered back to input order.  Separate from L2P and P2P so that those two never wait for one another.
-template <typename T>
-__global__ void finalize_k(const typename V4<T>::type* __restrict__ far, const typename V4<T>::type* __restrict__ near,
-                           const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field, int64_t N) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= N) return;
-    const typename V4<T>::type f = far[k], nr = near[k];
-    const T inv4pi = T(0.079577471545947667884441881686257);
-    const int64_t io = perm[k];
-    if (pot) pot[io] = -(f.x + nr.x) * inv4pi;
-    if (field) {
-        field[3 * io] = (f.y + nr.y) * inv4pi;
-        field[3 * io + 1] = (f.z + nr.z) * inv4pi;
-        field[3 * io + 2] = (f.w + nr.w) * inv4pi;
     }
 }
 
@@ -535,7 +527,7 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
 }
 
 template <typename T, int P>
-void launch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
+void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
     using T4 = typename V4<T>::type;
     const int64_t leaf0 = Pl.level_off[Pl.L];
     const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK);
@@ -544,13 +536,13 @@ void launch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
                                                            leaf0, Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p);
     else
         l2p_k<T, P><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p,
-                                                           leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p, (T4*)Pl.far.p);
+                                                           leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p, (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
 }
 
 template <typename T>
-void dispatch_p2m_l2p(const Plan& Pl, bool l2p, cudaStream_t st) {
+void dispatch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
     switch (Pl.p) {
-#define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, st); break;
+#define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, d_pot, d_field, st); break;
         FMM_CASE(0) FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
         FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12) FMM_CASE(13) FMM_CASE(14) FMM_CASE(15) FMM_CASE(16)
 #undef FMM_CASE
@@ -573,8 +565,8 @@ void ensure_streams(const Plan& Pl) {
 }
 
 // One evaluate.  ev == nullptr: the production schedule -- three internal streams forked from / joined to the caller's
-// stream: far chain (permute, P2M, leaf-level M2L, L2P, finalize), tree chain (M2M levels, the M2L of the upper levels, then
-// the L2L levels, all concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and finalize).
+// stream: far chain (permute, P2M, leaf-level M2L, L2P + finalize), tree chain (M2M levels, the M2L of the upper levels, then
+// the L2L levels, all concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and L2P).
 // ev != nullptr: the same kernels back to back on the caller's stream with an event after every stage (profiling).
 template <typename T>
 void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
@@ -617,7 +609,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     if (!serial) launch_p2p(sN);
     FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, sF));
     mark(1);
-    dispatch_p2m_l2p<T>(Pl, false, sF);
+    dispatch_p2m_l2p<T>(Pl, false, nullptr, nullptr, sF);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(2);
     if (fast && L > 0)  // the register kernels accumulate into the parents
@@ -666,12 +658,10 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     }
     if (split) after(sF, sU, Pl.e_up);
     mark(5);
-    dispatch_p2m_l2p<T>(Pl, true, sF);
-    FMM_CUDA_CHECK(cudaGetLastError());
-    mark(6);
     if (serial) launch_p2p(st);
     else after(sF, sN, Pl.e_near);
-    finalize_k<T><<<nblocks(N, 256), 256, 0, sF>>>((const T4*)Pl.far.p, (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field, N);
+    mark(6);
+    dispatch_p2m_l2p<T>(Pl, true, d_pot, d_field, sF);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(7);
     after(st, sF, Pl.e_done);
@@ -684,7 +674,7 @@ int64_t evaluate_launches(const Plan& P) {
     const int64_t w_leaf = (int64_t)P.weak_level_off.size() > P.L ? P.weak_level_off[P.L] : 0;
     int64_t m2l = P.n_weak > 0 ? 1 : 0;
     if (fast && !P.serial && P.L > 0 && w_leaf > 0 && w_leaf < P.n_weak) m2l = 2;  // leaf level and upper levels on two streams
-    return 5 + 2 * (int64_t)P.L + m2l;  // permute, P2M, L2P, P2P, finalize + M2M/L2L per level + M2L
+    return 4 + 2 * (int64_t)P.L + m2l;  // permute, P2M, P2P, L2P(+finalize) + M2M/L2L per level + M2L
 }
 
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {

@@ -92,8 +92,7 @@ struct Plan {
     // evaluate scratch
     DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
-    DevBuf<char> far;     // N x 4 dtype: (phi_far, grad phi_far) tree order, L2P -> finalize
-    DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> finalize
+    DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
     DevBuf<float> srcg;
     DevBuf<int32_t> src_slot;

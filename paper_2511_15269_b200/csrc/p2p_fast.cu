@@ -1,5 +1,5 @@
 // p2p_fast.cu -- fp32 near field (a9): direct sum over the strong leaf pairs (stage "evdir" PAPER.md:251;
-// DESIGN.md reading S3).  Writes (phi_near, grad phi_near) per particle in tree order; finalize_k (evaluate.cu) adds the far field,
+// DESIGN.md reading S3).  Writes (phi_near, grad phi_near) per particle in tree order; the L2P kernel (evaluate.cu) adds the far field,
 // scales and scatters to input order (a10).  The kernel depends only on the permuted particles, so run_evaluate launches it
 // on a second stream, concurrently with the whole far-field chain.
 //
