@@ -6,7 +6,9 @@
 A "step" is one pass of the whole hot path (permute -> P2M -> M2M -> M2L -> L2L -> L2P -> P2P, SURVEY.md section 8(a) rows
 a3-a10) over one charge vector on an existing plan (the paper times eval_potential on a cached hierarchy).
 The workload is BASELINE config 2 (N=1M uniform cube, fp32, p=8, s=3, N_max=128, theta=0.77); plan time is reported
-separately in the JSON (`plan_ms`).  The L2 (126 MB) is flushed between timed steps by writing a 512 MiB buffer; each step
+separately in the JSON (`plan_ms`).  `value` times fmm_evaluate in its production (concurrent, forked-stream) schedule;
+`stages` and `roofline.launch_ms` come from fmm_evaluate_profiled (same kernels back to back on one stream, CUDA events
+between them), so the stage times add up to more than one step.  The L2 (126 MB) is flushed between timed steps by writing a 512 MiB buffer; each step
 is timed with its own CUDA event pair on the launching stream, the flush lying outside the pairs.
 
 N > 1 (torchrun): replicas only -- every rank evaluates its own independent problem of the same
@@ -58,6 +60,10 @@ def m2l_bytes(p, esize, n_weak, n_targets):
 
 
 P2P_FLOP_PER_PAIR = 20.0  # 3 sub, mul+2 FMA, rsqrt, 3 mul, 1+3 FMA, mask
+
+# dram__bytes_read.sum + dram__bytes_write.sum per evaluate of the named kernel, from the committed `ncu --set full` capture
+# profiles/r01_ncu_full_evaluate.md (M2L = leaf-level launch 71.27 MB + upper-levels launch 8.66 MB)
+NCU_DRAM_BYTES = {"cfg2_cube1M_f32": {"m2l": 79.93e6, "p2p": 36.84e6}}
 
 
 class ClockSampler:
@@ -300,9 +306,12 @@ def run_ours(args):
     stages["p2p_frac_fp32"] = stages["p2p_tflops"] / fp32_peak_tflops
     dom = "m2l" if stage_ms["m2l"] >= stage_ms["p2p"] else "p2p"
     roofline = dict(kernel=dom, bound="alu", achieved=stages[dom + "_tflops"], peak=fp32_peak_tflops, unit="TFLOP/s",
-                    frac=stages[dom + "_tflops"] / fp32_peak_tflops, traffic=None,
+                    frac=stages[dom + "_tflops"] / fp32_peak_tflops, traffic=NCU_DRAM_BYTES.get(args.workload, {}).get(dom),
+                    traffic_source="profiles/r01_ncu_full_evaluate.md (ncu --set full, dram bytes read+write of this kernel per evaluate)",
+                    algorithmic_bytes=m2l_b if dom == "m2l" else None,
                     peak_source="148 SM x 128 FP32 lanes x 2 x %.0f MHz (DESIGN.md; FFMA micro-benchmark reached 98%% of it)" % peaks["sm_max_mhz"],
                     launch_ms=stage_ms[dom], launches_per_step=1,
+                    launch_ms_source="CUDA events around the kernel in fmm_evaluate_profiled (serial schedule, one launch), mean of %d steps" % n_prof,
                     hbm_peak_gbs=peaks["hbm_gbs"], hbm_peak_source=peaks["source"])
 
     cpu_baseline = None
@@ -320,7 +329,8 @@ def run_ours(args):
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if esize == 4 else "f64", data="synthetic",
                 config=dict(workload=args.workload, N=N, p=c["p"], s=c["s"], N_max=c["N_max"], theta=c["theta"], outputs="potential+field",
                             L=info["L"], n_boxes=info["n_boxes"], n_weak=info["n_weak"], n_strong=info["n_strong"], n_p2p_pairs=info["n_p2p_pairs"],
-                            l2="flushed between timed steps (512 MiB memset outside the event pairs)", parallelism="replicas x%d" % world),
+                            l2="flushed between timed steps (512 MiB memset outside the event pairs)", parallelism="replicas x%d" % world,
+                            schedule="concurrent: P2P, the tree passes (M2M, upper-level M2L, L2L) and the leaf-level M2L on three forked streams"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
                 gpu_launches=launches * args.steps, gpu_launches_per_step=launches, roofline=roofline, stages=stages, plan_ms=plan_ms,
