@@ -11,11 +11,10 @@
 // Register budget: 84 packed state values (168 registers) + one cos/sin table (18 packed) or one block of B temporaries
 // (17 packed) at a time; the four trig tables are regenerated when needed (8 packed FMAs each) instead of kept alive.
 //
-// A warp owns 64 consecutive weak pairs (sorted by target); lane l holds pairs 2l (low half) and 2l+1 (high half).
-// Source rows arrive through shared memory (cp.async, coalesced 16-byte chunks; row stride an odd number of 16-byte
-// units, so the per-lane LDS.128 are conflict-free).  When both pairs of every lane have the same target the halves are
-// added in registers; rows are then summed over runs of equal targets and added to D with one atomicAdd per coefficient
-// and run.
+// A warp owns 64 consecutive weak pairs (sorted by target); lane l holds pairs l (low half) and 32 + l (high half).
+// Source rows arrive in shared memory by TMA bulk copies (one per run of consecutive source ids; row stride an odd number
+// of 16-byte units, so the per-lane LDS.128 are conflict-free); the 64 result rows are summed over runs of equal targets
+// and added to D with one atomicAdd per coefficient and run.
 #include "tma.cuh"
 #include "xlate_reg.cuh"
 
@@ -33,7 +32,7 @@ struct PGeo {
     static constexpr int KSB = (CH & 1) ? CH : CH + 1;  // shared row stride in 16-byte units (odd)
     static constexpr int KV = CH * 4;
     static constexpr int NJ = (K + 31) / 32;
-    static constexpr size_t SMEM_WARP = (size_t)64 * KSB * 16 + 64 * sizeof(int);
+    static constexpr size_t SMEM_WARP = (size_t)64 * KSB * 16 + 16;  // 64 rows + one mbarrier
 };
 
 struct PairGeo {
@@ -138,7 +137,7 @@ m2l_packed_k(int64_t n, const int32_t* __restrict__ wtgt, const int32_t* __restr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned char* wbase = smraw + (size_t)warp * G::SMEM_WARP;
     float4* sm = reinterpret_cast<float4*>(wbase);
-    int* sidx = reinterpret_cast<int*>(wbase + (size_t)64 * G::KSB * 16);
+    const uint32_t bar = smem_u32(wbase + (size_t)64 * G::KSB * 16);
     int64_t e0 = ((int64_t)blockIdx.x * MW + warp) * 64;
     if constexpr (SYNC) {
         if (e0 >= n) e0 = n;  // idle warps still walk the code (barriers); all their pairs are discarded
@@ -146,27 +145,35 @@ m2l_packed_k(int64_t n, const int32_t* __restrict__ wtgt, const int32_t* __restr
         if (e0 >= n) return;
     }
 
-    // pairs of this lane: 2*lane (low half) and 2*lane+1 (high half); out-of-range pairs repeat the last valid one and are discarded
-    const int64_t eA = e0 + 2 * lane, eB = eA + 1;
-    const int64_t lA = eA < n ? eA : n - 1, lB = eB < n ? eB : n - 1;
-    const int gsA = wsrc[lA], gsB = wsrc[lB];
-    const int gtA0 = wtgt[lA], gtB0 = wtgt[lB];
-    sidx[2 * lane] = gsA;
-    sidx[2 * lane + 1] = gsB;
+    // pairs of this lane: e0 + lane (low half, shared row `lane`) and e0 + 32 + lane (high half, shared row 32 + lane)
+    const int64_t eA = e0 + lane, eB = eA + 32;
+    int gsA = -1, gtA = -1, gsB = -1, gtB = -1;
+    if (eA < n) { gsA = wsrc[eA]; gtA = wtgt[eA]; }
+    if (eB < n) { gsB = wsrc[eB]; gtB = wtgt[eB]; }
+    if (lane == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
     __syncwarp();
 
-    // coalesced asynchronous copy of the 64 source rows; pair r goes to shared row (r >> 1) + 32 (r & 1)
-    const float4* in16 = reinterpret_cast<const float4*>(Mc);
-#pragma unroll
-    for (int it = 0; it < 2 * G::CH; ++it) {
-        const int idx = it * 32 + lane;
-        const int r = idx / G::CH, c = idx - r * G::CH;
-        const int g = sidx[r];
-        cp_async16(sm + ((r >> 1) + 32 * (r & 1)) * G::KSB + c, in16 + (int64_t)g * G::CH + c);
-    }
-    const PairGeo ga = pair_geometry(ctr, scale, gsA, gtA0), gb = pair_geometry(ctr, scale, gsB, gtB0);
-    cp_async_wait_all();
-    __syncwarp();
+    // source rows by TMA bulk copies, one per run of consecutive source ids (see xlate_fast.cu), all on one mbarrier
+    constexpr uint32_t ROWB = G::CH * 16;
+    auto fetch = [&](int gs, int rowbase) -> int {
+        const int gprev = __shfl_up_sync(0xffffffffu, gs, 1);
+        const bool head = lane == 0 || gs < 0 || gprev < 0 || gs != gprev + 1 || G::KSB != G::CH;
+        const unsigned hm = __ballot_sync(0xffffffffu, head);
+        const unsigned above = lane == 31 ? 0u : (hm >> (lane + 1));
+        const int len = above ? __ffs(above) : 32 - lane;
+        if (head && gs >= 0)
+            bulk_g2s(smem_u32(sm + (rowbase + lane) * G::KSB), reinterpret_cast<const char*>(Mc) + (int64_t)gs * ROWB, (uint32_t)len * ROWB, bar);
+        return __popc(__ballot_sync(0xffffffffu, gs >= 0));
+    };
+    const int nA = fetch(gsA, 0), nB = fetch(gsB, 32);
+    if (lane == 0) mbar_expect_tx(bar, (uint32_t)(nA + nB) * ROWB);
+    // padding pairs compute on whatever their shared rows hold (their results are discarded), with a harmless geometry
+    const PairGeo ga = pair_geometry(ctr, scale, gsA >= 0 ? gsA : 0, gsA >= 0 ? gtA : 1);
+    const PairGeo gb = pair_geometry(ctr, scale, gsB >= 0 ? gsB : 0, gsB >= 0 ? gtB : 1);
+    mbar_wait(bar, 0);
 
     f2 v[G::KV];
     {
@@ -186,17 +193,9 @@ m2l_packed_k(int64_t n, const int32_t* __restrict__ wtgt, const int32_t* __restr
     m2l_pair<P, SYNC>(v, f2(ga.ct, gb.ct), f2(ga.st, gb.st), f2(ga.cp, gb.cp), f2(ga.sp, gb.sp), f2(ga.x1, gb.x1), f2(ga.x2, gb.x2),
                 f2(ga.rinv, gb.rinv));
 
-    const int gtA = eA < n ? gtA0 : -1, gtB = eB < n ? gtB0 : -1;
-    const bool merged = __all_sync(0xffffffffu, gtA == gtB || gtA < 0);  // every lane's two pairs share their target
-    float4* rowA = sm + lane * G::KSB;
-    float4* rowB = sm + (32 + lane) * G::KSB;
-    if (merged) {
-        sfor<G::CH>([&](auto cc) {
-            constexpr int c = decltype(cc)::value;
-            rowA[c] = make_float4(v[4 * c].lo() + v[4 * c].hi(), v[4 * c + 1].lo() + v[4 * c + 1].hi(), v[4 * c + 2].lo() + v[4 * c + 2].hi(),
-                                  v[4 * c + 3].lo() + v[4 * c + 3].hi());
-        });
-    } else {
+    {
+        float4* rowA = sm + lane * G::KSB;
+        float4* rowB = sm + (32 + lane) * G::KSB;
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             rowA[c] = make_float4(v[4 * c].lo(), v[4 * c + 1].lo(), v[4 * c + 2].lo(), v[4 * c + 3].lo());
@@ -205,40 +204,34 @@ m2l_packed_k(int64_t n, const int32_t* __restrict__ wtgt, const int32_t* __restr
     }
     __syncwarp();
 
-    // sum runs of equal targets (the list is sorted by target); lane j owns coefficients j, j+32, j+64
+    // sum runs of equal targets over the 64 rows (the list is sorted by target): run heads by ballots, warp-uniform row
+    // loops, one atomicAdd per coefficient and run; lane j owns coefficients j, j+32, j+64
     const float* smT = reinterpret_cast<const float*>(sm);
     constexpr int RS = G::KSB * 4;  // shared row stride in floats
-    float acc[G::NJ];
-#pragma unroll
-    for (int j = 0; j < G::NJ; ++j) acc[j] = 0.f;
-    int cur = -1;
-    auto flush = [&]() {
-        if (cur >= 0) {
-#pragma unroll
-            for (int j = 0; j < G::NJ; ++j)
-                if (lane + 32 * j < G::K) atomicAdd(Lc + (int64_t)cur * G::Kp + lane + 32 * j, acc[j]);
-        }
+    const int pA = __shfl_up_sync(0xffffffffu, gtA, 1), lastA = __shfl_sync(0xffffffffu, gtA, 31);
+    const int pB = __shfl_up_sync(0xffffffffu, gtB, 1);
+    const unsigned hA = __ballot_sync(0xffffffffu, lane == 0 || gtA != pA);
+    const unsigned hB = __ballot_sync(0xffffffffu, lane == 0 ? gtB != lastA : gtB != pB);
+    unsigned long long heads = (unsigned long long)hA | ((unsigned long long)hB << 32);
+    while (heads) {
+        const int r0 = __ffsll((long long)heads) - 1;
+        heads &= heads - 1;
+        const int r1 = heads ? __ffsll((long long)heads) - 1 : 64;
+        const int t = r0 < 32 ? __shfl_sync(0xffffffffu, gtA, r0) : __shfl_sync(0xffffffffu, gtB, r0 - 32);
+        if (t < 0) continue;  // padding pairs
+        float acc[G::NJ];
 #pragma unroll
         for (int j = 0; j < G::NJ; ++j) acc[j] = 0.f;
-    };
-    const int nrows = merged ? 32 : 64;
-#pragma unroll 4
-    for (int r = 0; r < nrows; ++r) {
-        // merged: row r = lane r's sum; otherwise pair order r -> lane r >> 1, half r & 1, shared row (r >> 1) + 32 (r & 1)
-        const int srcl = merged ? r : (r >> 1);
-        const int tA = __shfl_sync(0xffffffffu, gtA, srcl), tB = __shfl_sync(0xffffffffu, gtB, srcl);
-        const int t = (merged || !(r & 1)) ? tA : tB;
-        const int row = merged ? r : (r >> 1) + 32 * (r & 1);
-        if (t < 0) continue;
-        if (t != cur) {
-            flush();
-            cur = t;
+#pragma unroll 8
+        for (int r = r0; r < r1; ++r) {
+#pragma unroll
+            for (int j = 0; j < G::NJ; ++j)
+                if (lane + 32 * j < G::K) acc[j] += smT[r * RS + lane + 32 * j];
         }
 #pragma unroll
         for (int j = 0; j < G::NJ; ++j)
-            if (lane + 32 * j < G::K) acc[j] += smT[row * RS + lane + 32 * j];
+            if (lane + 32 * j < G::K) atomicAdd(Lc + (int64_t)t * G::Kp + lane + 32 * j, acc[j]);
     }
-    flush();
 }
 
 template <int P, int MW = 4, bool SYNC = false>
