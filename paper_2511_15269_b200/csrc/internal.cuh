@@ -67,6 +67,13 @@ struct Tables {
 const Tables& tables();  // throws CudaFail
 __host__ __device__ inline int boff(int n) { return n * (2 * n - 1) * (2 * n + 1) / 3; }
 
+// P2P work item (plan.cu p2p_segments_k, p2p_fast.cu): one segment of the strong list of a target leaf
+struct P2PItem {
+    int32_t start, cnt;  // particle range of the target leaf (tree order)
+    int64_t e0, e1;      // entries [e0, e1) of strong_src; e1 < 0 encodes ~e1 and "the leaf has several segments": partial
+                         // sums are then combined with atomics
+};
+
 struct Plan {
     int64_t N = 0;
     int p = 0, N_max = 0, s = 0, L = 0;
@@ -94,6 +101,9 @@ struct Plan {
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
+    DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
+    int64_t n_p2p_items = 0;
+    bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
     DevBuf<float> srcg;
     DevBuf<int32_t> src_slot;
     int src_G = 0;

@@ -59,16 +59,18 @@ constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two
 template <int TPT>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
-                                                      const int64_t* __restrict__ strong_off, const int32_t* __restrict__ strong_src,
+                                                      const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
                                                       float4* __restrict__ near, int64_t n_items, int nchunk) {
     __shared__ __align__(128) float sm[PW][2][TG * 16];
     __shared__ __align__(8) unsigned long long bars[PW][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t item = (int64_t)blockIdx.x * PW + warp;
     if (item >= n_items) return;
-    const int64_t leaf = item / nchunk;
-    const int chunk = (int)(item - leaf * nchunk);
-    const int tst = leaf_start[leaf], tcnt = leaf_cnt[leaf];
+    const int64_t iw = item / nchunk;
+    const int chunk = (int)(item - iw * nchunk);
+    const P2PItem wi = items[iw];  // one segment of the strong list of one target leaf
+    const bool multi = wi.e1 < 0;
+    const int tst = wi.start, tcnt = wi.cnt;
     const int t0 = chunk * 32 * TPT;
     if (t0 >= tcnt) return;
     const int tn = min(tcnt - t0, 32 * TPT);
@@ -99,8 +101,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
         PH[k] = GX[k] = GY[k] = GZ[k] = 0ull;
     }
 
-    int64_t e = strong_off[leaf];
-    const int64_t e1 = strong_off[leaf + 1];
+    int64_t e = wi.e0;
+    const int64_t e1 = multi ? ~wi.e1 : wi.e1;
     int sub = 0;  // groups of entry e already consumed
 
     // producer: fill tile `b` with up to TG groups starting at the cursor (e, sub); every lane issues the bulk copy of "its" entry
@@ -212,7 +214,13 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
     for (int k = 0; k < TPT; ++k) {
         const int ti = tg * TPT + k;
         // G accumulates +q d / r^3 = -grad phi_near; stored: (phi_near, grad phi_near) in tree order for the L2P finalize
-        if ((k & (nsl - 1)) == sl && ti < tn) near[tst + t0 + ti] = make_float4(ph[k], -gx[k], -gy[k], -gz[k]);
+        if ((k & (nsl - 1)) == sl && ti < tn) {
+            if (!multi) near[tst + t0 + ti] = make_float4(ph[k], -gx[k], -gy[k], -gz[k]);
+            else {  // several segments per leaf: `near` was zeroed by run_evaluate
+                float* o = reinterpret_cast<float*>(near + tst + t0 + ti);
+                atomicAdd(o, ph[k]); atomicAdd(o + 1, -gx[k]); atomicAdd(o + 2, -gy[k]); atomicAdd(o + 3, -gz[k]);
+            }
+        }
     }
 }
 
@@ -222,10 +230,12 @@ void p2p_fast_launch(const Plan& P, cudaStream_t st) {
     constexpr int TPT = 4;
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
-    const int64_t n_items = P.n_leaves * nchunk;
+    const int64_t n_items = P.n_p2p_items * nchunk;
+    if (n_items == 0) return;
+    if (P.p2p_multi) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
-                                              P.strong_off.p, P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
 
 }  // namespace fmm

@@ -407,17 +407,57 @@ __global__ void expand_offsets_k(ExpandArgs A, const unsigned long long* S, int6
     foff2[t] = (int64_t)(sv >> 32);
 }
 
+// out[0] = number of particle pairs of the P2P stage, out[1] = sum over non-empty target leaves of their source particles
 __global__ void count_p2p_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_cnt, int64_t n_leaves, unsigned long long* out) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned long long acc = 0;
-    if (t < n_leaves) {
-        unsigned long long ssum = 0;
+    unsigned long long acc = 0, ssum = 0;
+    if (t < n_leaves && leaf_cnt[t] > 0) {
         for (int64_t e = soff[t]; e < soff[t + 1]; ++e) ssum += (unsigned long long)leaf_cnt[ssrc[e]];
         acc = ssum * (unsigned long long)leaf_cnt[t];
     }
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-    if ((threadIdx.x & 31) == 0 && acc) atomicAdd(out, acc);
+    for (int d = 16; d > 0; d >>= 1) {
+        acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        ssum += __shfl_xor_sync(0xffffffffu, ssum, d);
+    }
+    if ((threadIdx.x & 31) == 0 && acc) {
+        atomicAdd(out, acc);
+        atomicAdd(out + 1, ssum);
+    }
+}
+
+// P2P work items: the strong list of a target leaf is cut into segments of at most `budget` source particles (whole source
+// leaves; a segment closes as soon as it has reached the budget), so that one warp never owns more than about twice the
+// average work even when a few leaves have very long lists (clustered inputs).  Pass 1 (items == nullptr) counts the segments
+// of every leaf, pass 2 writes them at seg_off[leaf].
+struct SegLoad {
+    const int32_t* p;
+    int64_t n;
+    __device__ int64_t operator()(int64_t i) const { return i < n ? (int64_t)p[i] : 0; }
+};
+__global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_start, const int32_t* leaf_cnt, int64_t n_leaves, int64_t budget,
+                               int32_t* nseg, const int64_t* seg_off, P2PItem* items, int* any_multi) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_leaves) return;
+    int n = 0;
+    if (leaf_cnt[t] > 0) {
+        const int total = items ? nseg[t] : 0;
+        int64_t acc = 0, e0 = soff[t];
+        const int64_t eend = soff[t + 1];
+        for (int64_t e = e0; e < eend; ++e) {
+            acc += leaf_cnt[ssrc[e]];
+            if (acc >= budget || e + 1 == eend) {
+                if (items) items[seg_off[t] + n] = P2PItem{leaf_start[t], leaf_cnt[t], e0, total > 1 ? ~(e + 1) : e + 1};
+                ++n;
+                acc = 0;
+                e0 = e + 1;
+            }
+        }
+    }
+    if (!items) {
+        nseg[t] = n;
+        if (n > 1) *any_multi = 1;
+    }
 }
 
 }  // namespace
@@ -514,15 +554,46 @@ void build_lists(Plan& P, cudaStream_t st) {
     FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_off.p, foff.p, (P.n_leaves + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
     FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_src.p, fsrc.p, nfail * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     DevBuf<unsigned long long> cnt;
-    cnt.alloc(1);
-    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 8, st));
+    cnt.alloc(2);
+    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 16, st));
     count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], P.n_leaves, cnt.p);
     FMM_CUDA_CHECK(cudaGetLastError());
-    unsigned long long h = 0;
-    FMM_CUDA_CHECK(cudaMemcpyAsync(&h, cnt.p, 8, cudaMemcpyDeviceToHost, st));
+    unsigned long long h[2] = {0, 0};
+    FMM_CUDA_CHECK(cudaMemcpyAsync(h, cnt.p, 16, cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    P.n_p2p_pairs = (int64_t)h[0];
+    {
+        // work items of the P2P kernel: budget = twice the mean number of source particles per target leaf (at least 1024)
+        const int32_t* lcnt = P.box_count.p + P.level_off[L];
+        const int64_t mean_src = (int64_t)(h[1] / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
+        const int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
+        DevBuf<int32_t> nseg, any_multi;
+        DevBuf<int64_t> seg_off, scratch;
+        nseg.alloc(P.n_leaves);
+        any_multi.alloc(1);
+        FMM_CUDA_CHECK(cudaMemsetAsync(any_multi.p, 0, sizeof(int32_t), st));
+        seg_off.alloc(P.n_leaves + 1);
+        scratch.alloc(scan_scratch_elems(P.n_leaves + 1));
+        p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, nullptr, nullptr,
+                                                                 any_multi.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        exclusive_scan<int64_t>(SegLoad{nseg.p, P.n_leaves}, seg_off.p, P.n_leaves + 1, scratch.p, st);
+        int64_t n_items = 0;
+        int32_t multi = 0;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&n_items, seg_off.p + P.n_leaves, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&multi, any_multi.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        P.n_p2p_items = n_items;
+        P.p2p_multi = multi != 0;
+        P.p2p_items.alloc((size_t)n_items * sizeof(P2PItem));
+        if (n_items > 0) {
+            p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, seg_off.p,
+                                                                     reinterpret_cast<P2PItem*>(P.p2p_items.p), nullptr);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+    }
     FMM_CUDA_CHECK(cudaEventRecord(e1, st));
     FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-    P.n_p2p_pairs = (int64_t)h;
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     P.plan_ms[2] = ms;
