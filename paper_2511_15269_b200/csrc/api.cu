@@ -236,7 +236,7 @@ fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial) {
 }
 
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {
-    if (!plan || variant < 0 || variant > 2) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    if (!plan || variant < 0 || variant > 3) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
     plan->P.m2l_variant = variant;
     return FMM_OK;
 }

@@ -592,6 +592,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     // m2l_variant: 0 = register kernels (one translation per thread), 1 = generic kernels, 2 = as 0 but M2L two pairs per thread (f32x2)
     const bool fast = Pl.m2l_variant != 1 && xlate_fast_available(p, Pl.dtype);
     const bool packed = Pl.m2l_variant == 2 && m2l_packed_available(p, Pl.dtype);
+    const bool stream = Pl.m2l_variant == 3 && m2l_stream_available(p, Pl.dtype) && Pl.n_weak > 0;
+    if (stream && Pl.n_m2l_batches == 0) build_m2l_batches(const_cast<Plan&>(Pl), st);  // built on first use of variant 3
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
@@ -634,7 +636,12 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
             if (packed) m2l_packed_launch(Pl, q, e0, e1);
             else xlate_fast_launch(Pl, 1, 0, q, e0, e1);
         };
-        if (split) {
+        if (stream) {
+            if (split) {
+                m2l_stream_launch(Pl, sF, Pl.m2l_batch_leaf, Pl.n_m2l_batches);
+                m2l_stream_launch(Pl, sU, 0, Pl.m2l_batch_leaf);
+            } else m2l_stream_launch(Pl, sF, 0, Pl.n_m2l_batches);
+        } else if (split) {
             m2l_range(w_leaf, Pl.n_weak, sF);
             m2l_range(0, w_leaf, sU);
         } else if (fast) {

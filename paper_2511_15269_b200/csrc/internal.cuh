@@ -101,6 +101,9 @@ struct Plan {
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
+    // weak list in batches of 32 pairs that never straddle two targets (m2l_stream.cu): sources padded with -1, one target per batch
+    DevBuf<int32_t> wpad_src, wpad_tgt;
+    int64_t n_m2l_batches = 0, m2l_batch_leaf = 0;  // m2l_batch_leaf: first batch whose target is a leaf-level box
     DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
     int64_t n_p2p_items = 0;
     bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
@@ -126,6 +129,7 @@ struct Plan {
 // plan.cu
 void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
 void build_lists(Plan& P, cudaStream_t st);
+void build_m2l_batches(Plan& P, cudaStream_t st);  // after build_lists; called on the first evaluate with m2l_variant 3
 // evaluate.cu
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
 int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evaluate
@@ -136,6 +140,9 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
 // m2l_packed.cu: fp32 M2L with two weak pairs per thread in packed f32x2 arithmetic (p <= 8); results are ADDED to Lc
 bool m2l_packed_available(int p, fmm_dtype dt);
 void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1);  // weak pairs [e0, e1)
+// m2l_stream.cu: fp32 M2L, one pair per thread, software-pipelined over the batches [b0, b1) of the padded weak list
+bool m2l_stream_available(int p, fmm_dtype dt);
+void m2l_stream_launch(const Plan& P, cudaStream_t st, int64_t b0, int64_t b1);
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
 void p2p_fast_launch(const Plan& P, cudaStream_t st);
 

@@ -226,8 +226,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
 
 }  // namespace
 
-void p2p_fast_launch(const Plan& P, cudaStream_t st) {
-    constexpr int TPT = 4;
+template <int TPT>
+static void p2p_launch_t(const Plan& P, cudaStream_t st) {
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
     const int64_t n_items = P.n_p2p_items * nchunk;
@@ -237,5 +237,7 @@ void p2p_fast_launch(const Plan& P, cudaStream_t st) {
     p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
                                               reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
+
+void p2p_fast_launch(const Plan& P, cudaStream_t st) { p2p_launch_t<4>(P, st); }  // measured on B200: TPT 2 / 4 / 8 -> 0.50 / 0.49 / 0.49 ms (config 2)
 
 }  // namespace fmm

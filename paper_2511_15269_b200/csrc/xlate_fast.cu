@@ -24,122 +24,6 @@ namespace {
 using namespace xr;
 
 
-// KIND 0 = M2M (b = child - parent), 1 = M2L (b = source - target), 2 = L2L (b = parent - child)   [DESIGN.md reading G3]
-// v: input coefficients of the old centre (length scale a_old) -> output coefficients about the new centre (a_new).
-// SYNC: the warps of a CTA meet at a barrier after every phase, so that they walk the (large, straight-line) code in
-// lockstep and share instruction-cache lines.
-template <typename T, int P, int KIND, bool SYNC, int KV>
-__device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
-    constexpr int P1 = P + 1;
-    const T rxy2 = bx * bx + by * by;
-    const T r2 = rxy2 + bz * bz;
-    const T r = sqrt(r2), rxy = sqrt(rxy2);
-    const T rinv = r > T(0) ? T(1) / r : T(0);
-    const T rxyinv = rxy > T(0) ? T(1) / rxy : T(0);
-    const T ct_ = r > T(0) ? bz * rinv : T(1), st_ = rxy * rinv;
-    const T cp_ = rxy > T(0) ? bx * rxyinv : T(1), sp_ = by * rxyinv;
-    T x1, x2;
-    if constexpr (KIND == 0) { x1 = r / a_new; x2 = a_old / a_new; }
-    else if constexpr (KIND == 1) { x1 = a_new * rinv; x2 = a_old * rinv; }
-    else { x1 = -r / a_old; x2 = a_new / a_old; }
-
-    T cph[P1], sph[P1], cth[P1], sth[P1];
-    trig_table<T, P1>(cp_, sp_, cph, sph);
-    trig_table<T, P1>(ct_, st_, cth, sth);
-
-    // forward rotation, degree by degree; M2M / M2L fold the source scaling x2^k in
-    {
-        T pw = T(1);
-        sfor<P>([&](auto nc) {
-            constexpr int n = decltype(nc)::value + 1;
-            if constexpr (KIND != 2) {
-                pw *= x2;
-                sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
-            }
-            apply_az<T, n, +1>(v, cph, sph);
-            apply_B<T, n, true>(v);
-            apply_az<T, n, +1>(v, cth, sth);
-            apply_B<T, n, false>(v);
-            if constexpr (SYNC && n >= 3) __syncthreads();
-        });
-    }
-
-    // z-shift (App. B.3), order by order; only equal m couple
-    if constexpr (KIND == 1) {
-        sfor<2 * P + 1>([&](auto mi) {
-            constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-            T t[cnt];
-            sfor<cnt>([&](auto ni) {
-                constexpr int n = am + decltype(ni)::value;
-                constexpr double h0 = ct::kTab.H[am][n][am];
-                T acc = T(h0) * v[am * am + am + m];
-                sfor<cnt - 1>([&](auto ki) {
-                    constexpr int k = am + 1 + decltype(ki)::value;
-                    constexpr double h = ct::kTab.H[am][n][k];
-                    acc = fma(T(h), v[k * k + k + m], acc);
-                });
-                t[decltype(ni)::value] = acc;
-            });
-            sfor<cnt>([&](auto ni) { v[(am + decltype(ni)::value) * (am + decltype(ni)::value + 1) + m] = t[decltype(ni)::value]; });
-        });
-        T pw = rinv;
-        sfor<P1>([&](auto nc) {
-            constexpr int n = decltype(nc)::value;
-            sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
-            pw *= x1;
-        });
-    } else {
-        T pw1[P1];
-        pw1[0] = T(1);
-        sfor<P>([&](auto jc) { pw1[decltype(jc)::value + 1] = pw1[decltype(jc)::value] * x1; });
-        if constexpr (KIND == 0) {
-            // out[n] = sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (v already scaled by x2^k): in place, n descending
-            sfor<2 * P + 1>([&](auto mi) {
-                constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                sfor<cnt>([&](auto ni) {
-                    constexpr int n = P - decltype(ni)::value;
-                    T acc = v[n * n + n + m];  // A[m][n][n] = 1
-                    sfor<n - am>([&](auto ki) {
-                        constexpr int k = am + decltype(ki)::value;
-                        constexpr double aa = ct::kTab.A[am][n][k];
-                        acc = fma(T(aa) * pw1[n - k], v[k * k + k + m], acc);
-                    });
-                    v[n * n + n + m] = acc;
-                });
-            });
-        } else {
-            // out[n] = x2^n sum_{k=n..p} A[|m|][k][n] x1^(k-n) v[k]: in place, n ascending
-            T pw2[P1];
-            pw2[0] = T(1);
-            sfor<P>([&](auto jc) { pw2[decltype(jc)::value + 1] = pw2[decltype(jc)::value] * x2; });
-            sfor<2 * P + 1>([&](auto mi) {
-                constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                sfor<cnt>([&](auto ni) {
-                    constexpr int n = am + decltype(ni)::value;
-                    T acc = v[n * n + n + m];
-                    sfor<P - n>([&](auto ki) {
-                        constexpr int k = n + 1 + decltype(ki)::value;
-                        constexpr double aa = ct::kTab.A[am][k][n];
-                        acc = fma(T(aa) * pw1[k - n], v[k * k + k + m], acc);
-                    });
-                    v[n * n + n + m] = acc * pw2[n];
-                });
-            });
-        }
-    }
-
-    // inverse rotation
-    if constexpr (SYNC) __syncthreads();
-    sfor<P>([&](auto nc) {
-        constexpr int n = decltype(nc)::value + 1;
-        apply_B<T, n, true>(v);
-        apply_az<T, n, -1>(v, cth, sth);
-        apply_B<T, n, false>(v);
-        apply_az<T, n, -1>(v, cph, sph);
-        if constexpr (SYNC && n >= 3) __syncthreads();
-    });
-}
-
 template <typename T> struct Vec16;
 template <> struct Vec16<float> { using type = float4; static constexpr int E = 4; };
 template <> struct Vec16<double> { using type = double2; static constexpr int E = 2; };

@@ -189,7 +189,7 @@ def test_kernel_families_agree_with_the_oracle_fp32(N, N_max, s, p):
     Po = O.Plan(pos, p, N_max, s, 0.77)
     uo, fo = Po.evaluate(q)
     P = gpu_plan(pos, p, N_max, s)
-    for variant in (0, 1, 2):
+    for variant in (0, 1, 2, 3):
         fmm.fmm_plan_set_m2l_variant(P.handle, variant)
         u, f = gpu_eval(P, q)
         assert rel2(u, uo) <= 1e-5 and rel2(f, fo) <= 1e-5, (variant, rel2(u, uo), rel2(f, fo))
