@@ -77,52 +77,6 @@ __device__ __forceinline__ void regular_rec(T x, T y, T z, F&& emit) {
     }
 }
 
-// App. A.1 + A.3 (with reading G1: no leading minus at PAPER.md:419).
-template <int P, typename T, typename F>
-__device__ __forceinline__ void regular_grad_rec(T x, T y, T z, F&& emit) {
-    T R[2][2 * P + 1], GX[2][2 * P + 1], GY[2][2 * P + 1], GZ[2][2 * P + 1];
-    const T r2 = x * x + y * y + z * z;
-    R[0][P] = T(1); GX[0][P] = T(0); GY[0][P] = T(0); GZ[0][P] = T(0);
-    emit(0, 0, R[0][P], GX[0][P], GY[0][P], GZ[0][P]);
-#pragma unroll
-    for (int n = 1; n <= P; ++n) {
-        const int c = n & 1, q = c ^ 1;
-#pragma unroll
-        for (int m = -(n - 2); m <= n - 2; ++m) {
-            const int am = m < 0 ? -m : m;
-            const T inv = T(1) / T((n - am) * (n + am));
-            const T w = T(2 * n - 1);
-            const T r1 = R[q][P + m], r0 = R[c][P + m];
-            GX[c][P + m] = (w * z * GX[q][P + m] - r2 * GX[c][P + m] - T(2) * r0 * x) * inv;
-            GY[c][P + m] = (w * z * GY[q][P + m] - r2 * GY[c][P + m] - T(2) * r0 * y) * inv;
-            GZ[c][P + m] = (w * (z * GZ[q][P + m] + r1) - r2 * GZ[c][P + m] - T(2) * r0 * z) * inv;
-            R[c][P + m] = (w * z * r1 - r2 * r0) * inv;
-        }
-        if (n == 1) {
-            R[c][P] = z * R[q][P]; GX[c][P] = T(0); GY[c][P] = T(0); GZ[c][P] = R[q][P];
-            R[c][P + 1] = x * T(0.5); GX[c][P + 1] = T(0.5); GY[c][P + 1] = T(0); GZ[c][P + 1] = T(0);
-            R[c][P - 1] = -y * T(0.5); GX[c][P - 1] = T(0); GY[c][P - 1] = T(-0.5); GZ[c][P - 1] = T(0);
-        } else {
-            const int a = P + n - 1, b = P - (n - 1);
-            const T dp = R[q][a], dm = R[q][b];
-            const T dpx = GX[q][a], dpy = GY[q][a], dpz = GZ[q][a], dmx = GX[q][b], dmy = GY[q][b], dmz = GZ[q][b];
-            const T h = T(1) / T(2 * n);
-            R[c][a] = z * dp; GX[c][a] = z * dpx; GY[c][a] = z * dpy; GZ[c][a] = z * dpz + dp;
-            R[c][b] = z * dm; GX[c][b] = z * dmx; GY[c][b] = z * dmy; GZ[c][b] = z * dmz + dm;
-            R[c][P + n] = (x * dp + y * dm) * h;
-            GX[c][P + n] = (x * dpx + y * dmx + dp) * h;
-            GY[c][P + n] = (x * dpy + y * dmy + dm) * h;
-            GZ[c][P + n] = (x * dpz + y * dmz) * h;
-            R[c][P - n] = (x * dm - y * dp) * h;
-            GX[c][P - n] = (x * dmx - y * dpx + dm) * h;
-            GY[c][P - n] = (x * dmy - y * dpy - dp) * h;
-            GZ[c][P - n] = (x * dmz - y * dpz) * h;
-        }
-#pragma unroll
-        for (int m = -n; m <= n; ++m) emit(n, m, R[c][P + m], GX[c][P + m], GY[c][P + m], GZ[c][P + m]);
-    }
-}
-
 // ------------------------------------------------------------------------------------------------ P2M (a4), warp per leaf
 constexpr int WARPS_PER_BLOCK = 4;
 
@@ -204,6 +158,13 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
     }
 }
 
+__device__ inline void idx_to_nm(int idx, int& n, int& m) {
+    n = (int)sqrtf((float)idx);
+    while (n * n > idx) --n;
+    while ((n + 1) * (n + 1) <= idx) ++n;
+    m = idx - n * n - n;
+}
+
 // ------------------------------------------------------------------------------------------------ L2P (a8) + finalize (a10), warp per leaf
 template <typename T, int P>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
@@ -212,7 +173,16 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
                                                               const T* __restrict__ Lc, const typename V4<T>::type* __restrict__ near,
                                                               const int32_t* __restrict__ perm, T* __restrict__ pot, T* __restrict__ field) {
     constexpr int K = (P + 1) * (P + 1);
+    constexpr int KD = P > 0 ? P * P : 1;  // coefficients of degree <= P-1
+    // The field is evaluated from three DERIVED expansions instead of running the grad R^ recursions of App. A.3
+    // per particle.  In the paper's basis (R_n^m = R^_n^m - i R^_n^-m, R_n^-m = (-1)^m conj R_n^m) the
+    // recursions of A.3 integrate to the ladder identities
+    //     d/dz R_n^m = R_{n-1}^m,   (d/dx + i d/dy) R_n^m = -R_{n-1}^{m+1},   (d/dx - i d/dy) R_n^m = R_{n-1}^{m-1}
+    // (pinned against the finite differences of the oracle's A.3 in tests/test_oracle_basis.py), so that for weights w
+    //     d/dx sum w_n^m R^_n^m = sum X_{n-1}^k R^_{n-1}^k   etc. with the two- and three-term formulas below.  Per particle
+    // this leaves one R^ recursion and 4 FMAs per coefficient.
     __shared__ T sL[WARPS_PER_BLOCK][K];
+    __shared__ T sD[WARPS_PER_BLOCK][3][KD];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
     if (leaf >= n_leaves) return;
@@ -222,15 +192,44 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
     const T inva = T(1) / scale[g];
     for (int idx = lane; idx < K; idx += 32) sL[w][idx] = Lc[g * Kp + idx] * gnorm<T>(idx);
     __syncwarp();
+    {
+        const T* wl = sL[w];
+        auto Wc = [&](int n, int k) -> T { return (k >= 0 && k <= n) ? wl[n * n + n + k] : T(0); };  // cos-type weight (order k >= 0)
+        auto Ws = [&](int n, int k) -> T { return (k >= 1 && k <= n) ? wl[n * n + n - k] : T(0); };  // sin-type weight (order -k)
+        for (int idx = lane; idx < P * P; idx += 32) {
+            int n1, m1;
+            idx_to_nm(idx, n1, m1);
+            const int n = n1 + 1, k = m1 < 0 ? -m1 : m1;
+            T dx, dy, dz;
+            if (m1 >= 0) {  // coefficient of R^_{n-1}^{k}
+                dx = T(0.5) * Wc(n, k + 1) - (k >= 2 ? T(0.5) * Wc(n, k - 1) : (k == 1 ? Wc(n, 0) : T(0)));
+                dy = -T(0.5) * Ws(n, k + 1) - (k >= 2 ? T(0.5) * Ws(n, k - 1) : T(0));
+                dz = Wc(n, k);
+            } else {        // coefficient of R^_{n-1}^{-k}
+                dx = T(0.5) * Ws(n, k + 1) - (k >= 2 ? T(0.5) * Ws(n, k - 1) : T(0));
+                dy = T(0.5) * Wc(n, k + 1) + (k >= 2 ? T(0.5) * Wc(n, k - 1) : Wc(n, 0));
+                dz = Ws(n, k);
+            }
+            sD[w][0][idx] = dx;
+            sD[w][1][idx] = dy;
+            sD[w][2][idx] = dz;
+        }
+    }
+    __syncwarp();
     for (int base = 0; base < cnt; base += 32) {
         const int i = base + lane;
         if (i < cnt) {
             const typename V4<T>::type v = pq[st + i];
             const T x = (T)((double)v.x - cx) * inva, y = (T)((double)v.y - cy) * inva, z = (T)((double)v.z - cz) * inva;
             T phi = 0, gx = 0, gy = 0, gz = 0;
-            regular_grad_rec<P, T>(x, y, z, [&](int n, int m, T R, T GX, T GY, T GZ) {
-                const T l = sL[w][n * n + n + m];
-                phi += l * R; gx += l * GX; gy += l * GY; gz += l * GZ;
+            regular_rec<P, T>(x, y, z, [&](int n, int m, T R) {
+                const int idx = n * n + n + m;
+                phi += sL[w][idx] * R;
+                if (n < P) {
+                    gx += sD[w][0][idx] * R;
+                    gy += sD[w][1][idx] * R;
+                    gz += sD[w][2][idx] * R;
+                }
             });
             // finalize (a10): add the near field written by P2P; u = -(phi_far + phi_near)/4pi (eqs. (2), (9), (14)),
             // field = -grad u = (grad phi_far + grad phi_near)/4pi (reading S2); scatter back to input order
@@ -259,13 +258,6 @@ struct TabPtrs {
     const void* B;  // T-typed rotation blocks
     const double *H, *A;
 };
-
-__device__ inline void idx_to_nm(int idx, int& n, int& m) {
-    n = (int)sqrtf((float)idx);
-    while (n * n > idx) --n;
-    while ((n + 1) * (n + 1) <= idx) ++n;
-    m = idx - n * n - n;
-}
 
 template <typename T>
 __device__ inline void az_step(int K, const T* in, T* out, const T* c, const T* s, T sign, int lane) {

@@ -98,6 +98,34 @@ def test_regular_grad_finite_differences(r):
         assert np.max(np.abs(G[:, c] - fd)) < 2e-9 * max(1.0, np.linalg.norm(r)) ** p
 
 
+@pytest.mark.parametrize("r", PTS[:4])
+def test_regular_grad_ladder_identities(r):
+    """App. A.3 integrates to the ladder identities of the complex basis R_n^m = R^_n^m - i R^_n^-m,
+    R_n^-m = (-1)^m conj R_n^m:  d/dz R_n^m = R_{n-1}^m,  (d/dx + i d/dy) R_n^m = -R_{n-1}^{m+1},
+    (d/dx - i d/dy) R_n^m = R_{n-1}^{m-1}.  A second, independent pin of the oracle's grad R^ (a wrong sign or index in A.3
+    breaks one of the three), and the identity the CUDA L2P kernel uses instead of the A.3 recursions."""
+    p = 8
+    R, G = O.regular_basis(p, r), O.regular_grad(p, r)
+
+    def Rc(n, m):
+        if abs(m) > n:
+            return 0j
+        if m >= 0:
+            return R[O.idx(n, m)] - 1j * (R[O.idx(n, -m)] if m > 0 else 0.0)
+        return (-1) ** m * np.conj(Rc(n, -m))
+
+    def Gc(n, m, c):  # gradient component c of the complex R_n^m, m >= 0
+        return G[O.idx(n, m), c] - 1j * (G[O.idx(n, -m), c] if m > 0 else 0.0)
+
+    scale = max(1.0, np.linalg.norm(r)) ** p
+    for n in range(1, p + 1):
+        for m in range(0, n + 1):
+            gx, gy, gz = Gc(n, m, 0), Gc(n, m, 1), Gc(n, m, 2)
+            assert abs(gz - Rc(n - 1, m)) < 1e-12 * scale
+            assert abs((gx + 1j * gy) + Rc(n - 1, m + 1)) < 1e-12 * scale
+            assert abs((gx - 1j * gy) - Rc(n - 1, m - 1)) < 1e-12 * scale
+
+
 def test_regular_is_harmonic_and_homogeneous():
     r = np.array([0.3, 0.4, -0.2])
     p, h = 6, 1e-3
