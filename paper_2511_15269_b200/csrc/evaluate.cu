@@ -80,18 +80,21 @@ __device__ __forceinline__ void regular_rec(T x, T y, T z, F&& emit) {
 // ------------------------------------------------------------------------------------------------ P2M (a4), warp per leaf
 constexpr int WARPS_PER_BLOCK = 4;
 
-template <typename T, int P>
+// LPL = lanes per leaf: 32 (a warp per leaf) or 16 (two leaves per warp, for plans whose leaves hold <= 16 particles).
+template <typename T, int P, int LPL>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
                                                               const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
                                                               const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves, int Kp,
                                                               T* __restrict__ Mc) {
     constexpr int K = (P + 1) * (P + 1);
     constexpr int NJ = (K + 31) / 32;
-    const int lane = threadIdx.x & 31;
-    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (leaf >= n_leaves) return;
-    const int64_t g = leaf0 + leaf;
-    const int st = box_start[g], cnt = box_count[g];
+    constexpr int LPW = 32 / LPL;  // leaves per warp
+    const int lane = threadIdx.x & 31, hl = lane % LPL;
+    const int64_t leaf = ((int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5)) * LPW + lane / LPL;
+    const bool have = leaf < n_leaves;
+    if (LPL == 32 && !have) return;
+    const int64_t g = leaf0 + (have ? leaf : 0);
+    const int st = box_start[g], cnt = have ? box_count[g] : 0;
     const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
     const T inva = T(1) / scale[g];
     if constexpr (NJ * 32 * sizeof(T) / 4 <= 128) {
@@ -101,8 +104,9 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
         T w[KP];
 #pragma unroll
         for (int i = 0; i < KP; ++i) w[i] = T(0);
-        for (int base = 0; base < cnt; base += 32) {
-            const int i = base + lane;
+        const int cmax = LPL == 32 ? cnt : max(cnt, __shfl_xor_sync(0xffffffffu, cnt, 16));  // warp-uniform trip count
+        for (int base = 0; base < cmax; base += LPL) {
+            const int i = base + hl;
             T x = 0, y = 0, z = 0, q = 0;
             if (i < cnt) {
                 const typename V4<T>::type v = pq[st + i];
@@ -114,7 +118,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
             regular_rec<P, T>(x, y, z, [&](int n, int m, T val) { w[n * n + n + m] += q * val; });
         }
 #pragma unroll
-        for (int bit = 16, h = KP / 2; bit > 0; bit >>= 1, h >>= 1) {
+        for (int bit = LPL / 2, h = KP / 2; bit > 0; bit >>= 1, h >>= 1) {
             const bool up = (lane & bit) != 0;
 #pragma unroll
             for (int i = 0; i < h; ++i) {
@@ -123,12 +127,14 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_k(const typename V4<
                 w[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
             }
         }
+        constexpr int NF = KP / LPL;  // coefficients NF*hl .. NF*hl + NF-1 end up on lane hl of the leaf's lane group
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) {
-            const int idx = NJ * lane + j;
-            if (idx < K) Mc[g * Kp + idx] = w[j] * gnorm<T>(idx);
+        for (int j = 0; j < NF; ++j) {
+            const int idx = NF * hl + j;
+            if (have && idx < K) Mc[g * Kp + idx] = w[j] * gnorm<T>(idx);
         }
     } else {
+        static_assert(LPL == 32 || NJ * 32 * sizeof(T) / 4 <= 128, "two leaves per warp need the register reduce-scatter path");
         T acc[NJ];
 #pragma unroll
         for (int j = 0; j < NJ; ++j) acc[j] = T(0);
@@ -166,7 +172,7 @@ __device__ inline void idx_to_nm(int idx, int& n, int& m) {
 }
 
 // ------------------------------------------------------------------------------------------------ L2P (a8) + finalize (a10), warp per leaf
-template <typename T, int P>
+template <typename T, int P, int LPL>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ box_start,
                                                               const int32_t* __restrict__ box_count, const double* __restrict__ ctr,
                                                               const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves, int Kp,
@@ -181,22 +187,26 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
     // (pinned against the finite differences of the oracle's A.3 in tests/test_oracle_basis.py), so that for weights w
     //     d/dx sum w_n^m R^_n^m = sum X_{n-1}^k R^_{n-1}^k   etc. with the two- and three-term formulas below.  Per particle
     // this leaves one R^ recursion and 4 FMAs per coefficient.
-    __shared__ T sL[WARPS_PER_BLOCK][K];
-    __shared__ T sD[WARPS_PER_BLOCK][3][KD];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + w;
-    if (leaf >= n_leaves) return;
-    const int64_t g = leaf0 + leaf;
-    const int st = box_start[g], cnt = box_count[g];
+    constexpr int LPW = 32 / LPL;  // leaves per warp (LPL lanes per leaf, see p2m_k)
+    __shared__ T sLs[WARPS_PER_BLOCK * LPW][K];
+    __shared__ T sDs[WARPS_PER_BLOCK * LPW][3][KD];
+    const int lane = threadIdx.x & 31, hl = lane % LPL, w = (threadIdx.x >> 5) * LPW + lane / LPL;
+    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK * LPW + w;
+    const bool have = leaf < n_leaves;
+    if (LPL == 32 && !have) return;
+    const int64_t g = leaf0 + (have ? leaf : 0);
+    const int st = box_start[g], cnt = have ? box_count[g] : 0;
     const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
     const T inva = T(1) / scale[g];
-    for (int idx = lane; idx < K; idx += 32) sL[w][idx] = Lc[g * Kp + idx] * gnorm<T>(idx);
+    T(*sL)[K] = sLs;
+    T(*sD)[3][KD] = sDs;
+    for (int idx = hl; idx < K; idx += LPL) sL[w][idx] = Lc[g * Kp + idx] * gnorm<T>(idx);
     __syncwarp();
     {
         const T* wl = sL[w];
         auto Wc = [&](int n, int k) -> T { return (k >= 0 && k <= n) ? wl[n * n + n + k] : T(0); };  // cos-type weight (order k >= 0)
         auto Ws = [&](int n, int k) -> T { return (k >= 1 && k <= n) ? wl[n * n + n - k] : T(0); };  // sin-type weight (order -k)
-        for (int idx = lane; idx < P * P; idx += 32) {
+        for (int idx = hl; idx < P * P; idx += LPL) {
             int n1, m1;
             idx_to_nm(idx, n1, m1);
             const int n = n1 + 1, k = m1 < 0 ? -m1 : m1;
@@ -216,8 +226,8 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
         }
     }
     __syncwarp();
-    for (int base = 0; base < cnt; base += 32) {
-        const int i = base + lane;
+    for (int base = 0; base < cnt; base += LPL) {
+        const int i = base + hl;
         if (i < cnt) {
             const typename V4<T>::type v = pq[st + i];
             const T x = (T)((double)v.x - cx) * inva, y = (T)((double)v.y - cy) * inva, z = (T)((double)v.z - cz) * inva;
@@ -518,17 +528,27 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
     }
 }
 
-template <typename T, int P>
-void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
+template <typename T, int P, int LPL>
+void launch_p2m_l2p_t(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
     using T4 = typename V4<T>::type;
     const int64_t leaf0 = Pl.level_off[Pl.L];
-    const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK);
+    const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK * (32 / LPL));
     if (!l2p)
-        p2m_k<T, P><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p,
-                                                           leaf0, Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p);
+        p2m_k<T, P, LPL><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
+                                                                (const T*)Pl.box_scale.p, leaf0, Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p);
     else
-        l2p_k<T, P><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p,
-                                                           leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p, (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
+        l2p_k<T, P, LPL><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
+                                                                (const T*)Pl.box_scale.p, leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p,
+                                                                (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
+}
+
+template <typename T, int P>
+void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
+    // leaves of <= 16 particles (e.g. config 4: N_max = 64, s = 3): two leaves per warp.  fp32, p <= 8 only (compile time).
+    if constexpr (sizeof(T) == 4 && P <= 8) {
+        if (Pl.max_leaf <= 16) { launch_p2m_l2p_t<T, P, 16>(Pl, l2p, d_pot, d_field, st); return; }
+    }
+    launch_p2m_l2p_t<T, P, 32>(Pl, l2p, d_pot, d_field, st);
 }
 
 template <typename T>
