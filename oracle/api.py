@@ -40,13 +40,13 @@ def lib():
         L.orc_translate.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp]
         L.orc_tree_depth.argtypes = [C.c_int64, C.c_int, C.c_int]
         L.orc_tree_depth.restype = C.c_int
-        L.orc_plan_create.argtypes = [_dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double]
+        L.orc_plan_create.argtypes = [_dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int]
         L.orc_plan_create.restype = C.c_void_p
         L.orc_plan_destroy.argtypes = [C.c_void_p]
         L.orc_plan_info.argtypes = [C.c_void_p, C.POINTER(C.c_int)] + [_ip] * 5
         L.orc_plan_copy_tree.argtypes = [C.c_void_p, _ip, _ip, _ip, _dp, _dp, _dp, _dp]
         L.orc_plan_copy_lists.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip]
-        L.orc_lists_from_geometry.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, _ip, _ip]
+        L.orc_lists_from_geometry.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_int, _ip, _ip]
         L.orc_evaluate.argtypes = [C.c_void_p, _dp, _bp, _dp, _dp]
         L.orc_direct.argtypes = [_dp, _dp, C.c_int64, _ip, C.c_int64, _dp, _dp]
         L.orc_num_threads.restype = C.c_int
@@ -127,12 +127,13 @@ def num_threads():
 class Plan:
     """Oracle hierarchy + lists for fixed positions (reusable for new charges)."""
 
-    def __init__(self, pos, p, N_max, s, theta=0.77):
+    def __init__(self, pos, p, N_max, s, theta=0.77, cross_level=0):
         self.pos = np.ascontiguousarray(pos, dtype=np.float64)
         assert self.pos.ndim == 2 and self.pos.shape[1] == 3
         self.N = self.pos.shape[0]
         self.p, self.N_max, self.s, self.theta = int(p), int(N_max), int(s), float(theta)
-        self._h = lib().orc_plan_create(_d(self.pos), self.N, self.p, self.N_max, self.s, self.theta)
+        self.cross_level = int(cross_level)
+        self._h = lib().orc_plan_create(_d(self.pos), self.N, self.p, self.N_max, self.s, self.theta, self.cross_level)
         L = C.c_int()
         v = [C.c_int64() for _ in range(5)]
         lib().orc_plan_info(self._h, C.byref(L), *[C.byref(x) for x in v])
@@ -173,13 +174,13 @@ class Plan:
         return pot, fld
 
 
-def lists_from_geometry(s, L, ctr, rad, theta):
+def lists_from_geometry(s, L, ctr, rad, theta, cross_level=0):
     ctr = np.ascontiguousarray(ctr, dtype=np.float64)
     rad = np.ascontiguousarray(rad, dtype=np.float64)
     nb = rad.shape[0]
     nw = np.empty(nb, np.int64)
     ns = np.empty(1 << (s * L), np.int64)
-    lib().orc_lists_from_geometry(s, L, _d(ctr), _d(rad), float(theta), _i(nw), _i(ns))
+    lib().orc_lists_from_geometry(s, L, _d(ctr), _d(rad), float(theta), int(cross_level), _i(nw), _i(ns))
     return nw, ns
 
 

@@ -18,8 +18,9 @@
 // orthogonality; rotations vs recomputation from rotated points; M2M/L2L exactness;
 // M2L convergence; tree brute force + PAPER.md:50 counts; list partition identity and
 // the theta=0.7637 cube pin; whole FMM vs O(N^2) direct sum.
-// "parity unpinned": none of the functions below (cross-level lists, Table I are not
-// implemented here).
+// Cross-level (level-marching) lists: partition identity over all level pairs, symmetry of
+// the covered particle pairs, accuracy vs the O(N^2) sum and the count reduction against same-level lists.
+// "parity unpinned": the interaction counts of Table I -- the helix point set is not given.
 //
 // Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py)
 // Coefficient layout: K=(p+1)^2 doubles, index(n,m) = n*n + n + m, -n<=m<=n;
@@ -375,8 +376,16 @@ struct Lists {
     std::vector<int64_t> strong_off; std::vector<int64_t> strong_src;
 };
 
-// PAPER.md:72-74, rules L2-L5.
-void build_lists(const Tree& T, double theta, Lists& Ls) {
+// PAPER.md:72-74, rules L2-L5 (cross_level = 0), and the level-marching generalisation PAPER.md:82-89 (cross_level = 1,
+// reading S9 of DESIGN.md): candidate pairs (target box on level lt, source box on level ls) start at (root, root) with
+// lt = ls = 0; admissible candidates (eq. (4)) become weak pairs of their target; the others are refined and re-tested.
+//   cross_level = 0: both boxes are refined together, (lt, ls) = (0,0), (1,1), ..., (L,L).
+//   cross_level = 1: one side at a time.  "Increase the level with the larger average box radius; if equal, increase the
+//     source level; if there are no more source levels, increase the target level".  Sources and targets
+//     share one hierarchy here, whose mean box radius shrinks from level to level, so the rule yields the fixed sequence
+//     (0,0), (1,0), (1,1), (2,1), ..., (L,L-1), (L,L): refine the sources, then the targets, alternately.
+// Pairs still failing at (L,L) are the strong leaf pairs (L3).
+void build_lists(const Tree& T, double theta, Lists& Ls, int cross_level = 0) {
     const int s = T.s, L = T.L;
     const int64_t nch = (int64_t)1 << s;
     const int64_t nb = T.level_off[L + 1];
@@ -384,23 +393,29 @@ void build_lists(const Tree& T, double theta, Lists& Ls) {
     const int64_t n_leaves = (int64_t)1 << (s * L);
     std::vector<std::vector<int64_t>> strong_rows(n_leaves);
     std::vector<std::pair<int64_t, int64_t>> cand, fail;
-    cand.push_back({0, 0});  // (root, root), level-local indices
-    for (int l = 0; l <= L; ++l) {
+    cand.push_back({0, 0});  // (root, root), level-local indices (target, source)
+    int lt = 0, ls = 0;
+    for (;;) {
         fail.clear();
         for (auto& pr : cand) {
-            const int64_t ga = T.level_off[l] + pr.first, gb = T.level_off[l] + pr.second;
+            const int64_t ga = T.level_off[lt] + pr.first, gb = T.level_off[ls] + pr.second;
             if (admissible(T, ga, gb, theta)) weak_rows[ga].push_back(gb);
             else fail.push_back(pr);
         }
-        if (l == L) break;
+        if (lt == L && ls == L) break;
+        const bool refine_src = cross_level ? (ls == lt) : true;
+        const bool refine_tgt = cross_level ? (ls != lt) : true;
         cand.clear();
         for (auto& pr : fail)
-            for (int64_t i = 0; i < nch; ++i)
-                for (int64_t j = 0; j < nch; ++j) {
-                    const int64_t a = pr.first * nch + i, b = pr.second * nch + j;
-                    if (T.box_count[T.level_off[l + 1] + a] == 0 || T.box_count[T.level_off[l + 1] + b] == 0) continue;  // T5
+            for (int64_t i = 0; i < (refine_tgt ? nch : 1); ++i)
+                for (int64_t j = 0; j < (refine_src ? nch : 1); ++j) {
+                    const int64_t a = refine_tgt ? pr.first * nch + i : pr.first, b = refine_src ? pr.second * nch + j : pr.second;
+                    if (T.box_count[T.level_off[lt + (refine_tgt ? 1 : 0)] + a] == 0 || T.box_count[T.level_off[ls + (refine_src ? 1 : 0)] + b] == 0)
+                        continue;  // T5
                     cand.push_back({a, b});
                 }
+        if (refine_tgt) ++lt;
+        if (refine_src) ++ls;
     }
     for (auto& pr : fail) strong_rows[pr.first].push_back(pr.second);  // L3, includes (t,t)
     Ls.weak_off.assign(nb + 1, 0); Ls.weak_src.clear();
@@ -558,12 +573,12 @@ void orc_shift(int kind, int p, const double* in, double r, double* out) {
 void orc_translate(int kind, int p, const double* in, const double* b, double* out) { translate(kind, p, in, b, out); }
 int orc_tree_depth(int64_t N, int N_max, int s) { return tree_depth(N, N_max, s); }
 
-void* orc_plan_create(const double* pos, int64_t N, int p, int N_max, int s, double theta) {
+void* orc_plan_create(const double* pos, int64_t N, int p, int N_max, int s, double theta, int cross_level) {
     Plan* P = new Plan();
     P->p = p; P->theta = theta;
     P->pos.assign(pos, pos + 3 * N);
     build_tree(P->pos.data(), N, N_max, s, P->T);
-    build_lists(P->T, theta, P->Ls);
+    build_lists(P->T, theta, P->Ls, cross_level);
     return P;
 }
 void orc_plan_destroy(void* h) { delete (Plan*)h; }
@@ -597,7 +612,7 @@ void orc_plan_copy_lists(void* h, int64_t* weak_off, int64_t* weak_src, int64_t*
     if (strong_src) std::copy(Ls.strong_src.begin(), Ls.strong_src.end(), strong_src);
 }
 // lists from hand-made geometry (pin PAPER.md:80): boxes given by ctr/rad, tree shape (s, L) complete
-void orc_lists_from_geometry(int s, int L, const double* ctr, const double* rad, double theta,
+void orc_lists_from_geometry(int s, int L, const double* ctr, const double* rad, double theta, int cross_level,
                              int64_t* n_weak_per_box, int64_t* n_strong_per_leaf) {
     Tree T; T.s = s; T.L = L;
     T.level_off.assign(L + 2, 0);
@@ -605,7 +620,7 @@ void orc_lists_from_geometry(int s, int L, const double* ctr, const double* rad,
     const int64_t nb = T.level_off[L + 1];
     T.ctr.assign(ctr, ctr + 3 * nb); T.rad.assign(rad, rad + nb);
     T.box_count.assign(nb, 1); T.box_start.assign(nb, 0);
-    Lists Ls; build_lists(T, theta, Ls);
+    Lists Ls; build_lists(T, theta, Ls, cross_level);
     for (int64_t g = 0; g < nb; ++g) n_weak_per_box[g] = Ls.weak_off[g + 1] - Ls.weak_off[g];
     const int64_t nl = (int64_t)1 << (s * L);
     for (int64_t t = 0; t < nl; ++t) n_strong_per_leaf[t] = Ls.strong_off[t + 1] - Ls.strong_off[t];

@@ -64,6 +64,27 @@ def test_deep_trees_error_falls_with_p(N, N_max, s):
     assert prev < 1e-3
 
 
+@pytest.mark.parametrize("N,N_max,s", [(4096, 64, 3), (1024, 16, 1), (2048, 8, 3)])
+def test_cross_level_lists_error_falls_with_p(N, N_max, s):
+    """Level-marching lists against the O(N^2) definition: every weak pair obeys the same eq. (4), so the
+    error falls with p like the same-level lists' (eq. (5)) and stays within a small factor of it, with
+    fewer M2L pairs."""
+    pos, q = inputs.uniform_cube(N, 7)
+    ud, fd = O.direct(pos, q)
+    prev = None
+    for p in (2, 4, 6):
+        Pc = O.Plan(pos, p, N_max, s, 0.77, cross_level=1)
+        Ps = O.Plan(pos, p, N_max, s, 0.77)
+        assert Pc.n_weak < Ps.n_weak and Pc.n_strong <= Ps.n_strong
+        uc, fc = Pc.evaluate(q)
+        us, fs = Ps.evaluate(q)
+        ec, es = rel2(uc, ud), rel2(us, ud)
+        assert ec < 3.0 * es and rel2(fc, fd) < 3.0 * rel2(fs, fd)
+        assert prev is None or ec < 0.5 * prev
+        prev = ec
+    assert prev < 1e-3
+
+
 def test_p0_and_all_near_field_degenerate_cases():
     pos, q = inputs.uniform_cube(300, 2)
     ud, fd = O.direct(pos, q)

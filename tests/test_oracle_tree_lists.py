@@ -146,6 +146,59 @@ def test_lists_partition_identity(N, N_max, s, theta):
             assert hits == 1
 
 
+@pytest.mark.parametrize("N,N_max,s,theta", [(1500, 8, 2, 0.77), (800, 6, 1, 0.5), (2048, 16, 3, 0.7)])
+def test_cross_level_lists_partition_identity(N, N_max, s, theta):
+    """Level marching, PAPER.md:82-89 (one hierarchy for sources and targets => level pairs (0,0), (1,0), (1,1), (2,1), ...,
+    (L,L)): for every ordered leaf pair (t,s) exactly one of {strong; weak at exactly one step of the march} holds; a weak
+    pair satisfies eq. (4), its source sits on the target's level or one below, and the pair of every earlier step fails
+    eq. (4).  (Unlike the same-level lists neither list is symmetric: the steps (l+1, l) test (coarse target, fine source)
+    only, so leaf a may reach leaf b through an M2L of its parent while b sums a directly.)"""
+    pos, _ = inputs.uniform_cube(N, 9)
+    P = O.Plan(pos, 2, N_max, s, theta, cross_level=1)
+    Ps = O.Plan(pos, 2, N_max, s, theta)
+    t, ls, lss = P.tree(), P.lists(), Ps.lists()
+    L, nl = P.L, P.n_leaves
+    off = [sum(2 ** (s * k) for k in range(l)) for l in range(L + 2)]
+    level = lambda g: max(l for l in range(L + 1) if off[l] <= g)
+    anc = lambda leaf, l: off[l] + (leaf >> (s * (L - l)))
+    march = [(0, 0)]
+    while march[-1] != (L, L):
+        lt, lsrc = march[-1]
+        march.append((lt, lsrc + 1) if lsrc == lt else (lt + 1, lsrc))  # refine the sources first, then the targets
+    weak = set()
+    for g in range(P.n_boxes):
+        row = ls["weak_src"][ls["weak_off"][g]: ls["weak_off"][g + 1]]
+        assert np.all(np.diff(row) > 0)
+        for src in row:
+            assert level(int(src)) - level(g) in (0, 1) and _adm(t, g, int(src), theta)
+            weak.add((g, int(src)))
+    strong = set()
+    for tl in range(nl):
+        row = ls["strong_src"][ls["strong_off"][tl]: ls["strong_off"][tl + 1]]
+        assert np.all(np.diff(row) > 0)
+        strong.update((tl, int(src)) for src in row)
+    assert all((tl, tl) in strong for tl in range(nl))
+    # strong pairs fail every test of the march, in particular all same-level ones: subset of the same-level strong list
+    strong_same = set()
+    for tl in range(nl):
+        strong_same.update((tl, int(src)) for src in lss["strong_src"][lss["strong_off"][tl]: lss["strong_off"][tl + 1]])
+    assert strong <= strong_same
+    assert P.n_weak < Ps.n_weak  # the point of the scheme (PAPER.md:89, Table I)
+    rng = np.random.default_rng(0)
+    pairs = [(int(a), int(b)) for a, b in rng.integers(0, nl, (4000, 2))] + [(a, a) for a in range(0, nl, 7)]
+    for (a, b) in pairs:
+        hits = []
+        for k, (lt, lsrc) in enumerate(march):
+            if (anc(a, lt), anc(b, lsrc)) in weak:
+                hits.append(k)
+        if (a, b) in strong:
+            assert not hits
+            assert not any(_adm(t, anc(a, lt), anc(b, lsrc), theta) for (lt, lsrc) in march)
+        else:
+            assert len(hits) == 1
+            assert not any(_adm(t, anc(a, lt), anc(b, lsrc), theta) for (lt, lsrc) in march[:hits[0]])
+
+
 def test_lists_reproduce_nearest_neighbour_on_cubes(golden_dir):
     """theta = sqrt(3)/(4-sqrt(3)) ~ 0.7637 is the nearest-neighbour geometry of the uniform FMM; the
     default 0.77 reproduces it.  Hand-made geometry: 8x8x8 equal cubes (side a, radius sqrt(3)/2 a) in an octree
