@@ -41,7 +41,7 @@ typedef enum {
     FMM_ERR_INVALID_ARG = 1, /* NULL pointer, N<1, p<0 or p>FMM_P_MAX, N_max<1, s<1, theta not in (0,1), non-finite position */
     FMM_ERR_ALLOC = 2,       /* device or host allocation failed */
     FMM_ERR_CUDA = 3,        /* any other CUDA runtime error (message in fmm_last_error) */
-    FMM_ERR_UNSUPPORTED = 4  /* cross_level != 0, or a tree too deep for 31-bit box ids */
+    FMM_ERR_UNSUPPORTED = 4  /* a tree too deep for 31-bit box ids, lists beyond 2^31 pairs */
 } fmm_status;
 
 typedef enum { FMM_F32 = 0, FMM_F64 = 1 } fmm_dtype;
@@ -51,7 +51,10 @@ typedef enum { FMM_F32 = 0, FMM_F64 = 1 } fmm_dtype;
 /* Admissibility parameters of eq. (4):  R + theta*r < theta*d. */
 typedef struct {
     double theta;    /* 0 < theta < 1; the paper's default is 0.77 */
-    int cross_level; /* 0 = same-level lists.  1 (level marching) is reserved. */
+    int cross_level; /* 0 = same-level lists (the default).  1 = level-marching lists: weak
+                      * pairs may join a target box with a source box one level below it; the march over (target level,
+                      * source level) is (0,0), (1,0), (1,1), (2,1), ..., (L,L) (reading S9).  Fewer M2L pairs
+                      * at the same eq. (4). */
 } fmm_admissibility;
 
 /* Build hierarchy + lists for N charges (Listing 2; lists PAPER.md:72-74).

@@ -58,10 +58,12 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
         if (N_max < 1 || s < 1) { set_error("N_max and s must be >= 1"); return FMM_ERR_INVALID_ARG; }
         if (dtype != FMM_F32 && dtype != FMM_F64) { set_error("unknown dtype"); return FMM_ERR_INVALID_ARG; }
         double theta = 0.77;
+        int cross_level = 0;
         if (adm) {
             theta = adm->theta;
+            cross_level = adm->cross_level;
             if (!(theta > 0.0 && theta < 1.0)) { set_error("theta must be in (0,1)"); return FMM_ERR_INVALID_ARG; }
-            if (adm->cross_level != 0) { set_error("cross_level lists are not implemented"); return FMM_ERR_UNSUPPORTED; }
+            if (cross_level != 0 && cross_level != 1) { set_error("cross_level must be 0 or 1"); return FMM_ERR_INVALID_ARG; }
         }
         int ndev = 0;
         if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -73,7 +75,7 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
-            P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta;
+            P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta; P.cross_level = cross_level;
             P.K = (p + 1) * (p + 1);
             P.Kp = (P.K + 3) & ~3;
             int L = 0;  // smallest L with ceil(N / 2^(sL)) <= N_max

@@ -79,6 +79,7 @@ struct Plan {
     int p = 0, N_max = 0, s = 0, L = 0;
     fmm_dtype dtype = FMM_F32;
     double theta = 0.77;
+    int cross_level = 0;  // 1: level-marching lists
     int K = 0, Kp = 0;  // (p+1)^2 and the padded row stride of coefficient arrays
     int64_t n_boxes = 0, n_leaves = 0, n_weak = 0, n_strong = 0, n_p2p_pairs = 0;
     std::vector<int64_t> level_off;  // L+2

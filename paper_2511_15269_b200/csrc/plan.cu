@@ -460,6 +460,65 @@ __global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const i
     }
 }
 
+// ---- level-marching (cross-level) lists, reading S9: steps (lt, ls) = (0,0), (1,0), (1,1), (2,1), ..., (L,L).
+// Failing pairs (target box on level lt, source box on level ls; level-local indices) are refined on ONE side per step:
+// the sources when lt == ls, else the targets.  Invariant: for a fixed target the sources appear in ascending order, so a
+// stable sort by target at the end gives the canonical CSR form (L4) that is compared bit by bit with the oracle.
+struct MarchArgs {
+    const int32_t *ftgt, *fsrc;
+    int64_t nfail;
+    int s;
+    int refine_src;                 // 1: candidates (t, s * nch + c) ; 0: candidates (t * nch + c, s)
+    int64_t off_t, off_s;           // global id offsets of the candidates' levels
+    const int32_t* box_count;
+    const double *ctr, *rad;
+    double theta;
+};
+__device__ inline void march_decode(const MarchArgs& A, int64_t idx, int32_t& t, int32_t& sc) {
+    const int nch = 1 << A.s;
+    const int64_t e = idx >> A.s;
+    const int c = (int)(idx & (nch - 1));
+    t = A.refine_src ? A.ftgt[e] : A.ftgt[e] * nch + c;
+    sc = A.refine_src ? A.fsrc[e] * nch + c : A.fsrc[e];
+}
+__global__ void march_classify_k(MarchArgs A, uint8_t* codes) {
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (A.nfail << A.s)) return;
+    int32_t t, sc;
+    march_decode(A, idx, t, sc);
+    const int64_t gt = A.off_t + t, gs = A.off_s + sc;
+    uint8_t code = 0;
+    if (A.box_count[gt] > 0 && A.box_count[gs] > 0) code = admissible(A.ctr, A.rad, gt, gs, A.theta) ? 1 : 2;
+    codes[idx] = code;
+}
+__global__ void march_compact_k(MarchArgs A, const uint8_t* codes, const unsigned long long* S, int32_t* wtgt, int32_t* wsrc, int32_t* ftgt2,
+                                int32_t* fsrc2) {
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (A.nfail << A.s)) return;
+    int32_t t, sc;
+    march_decode(A, idx, t, sc);
+    const uint8_t c = codes[idx];
+    const unsigned long long sv = S[idx];
+    if (c == 1) {
+        const int64_t o = (int64_t)(sv & 0xffffffffull);
+        wtgt[o] = (int32_t)(A.off_t + t);
+        wsrc[o] = (int32_t)(A.off_s + sc);
+    } else if (c == 2) {
+        const int64_t o = (int64_t)(sv >> 32);
+        ftgt2[o] = t;
+        fsrc2[o] = sc;
+    }
+}
+__global__ void count_keys_k(const int32_t* keys, int64_t n, unsigned long long* cnt) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) atomicAdd(cnt + keys[i], 1ull);
+}
+struct CntLoad {
+    const unsigned long long* p;
+    int64_t n;
+    __device__ int64_t operator()(int64_t i) const { return i < n ? (int64_t)p[i] : 0; }
+};
+
 // ---- batched copy of the weak list for m2l_stream.cu: every target's sources in batches of 32, padded with -1
 struct BatLoad {
     const int64_t* woff;
@@ -507,12 +566,172 @@ void build_tree(Plan& P, const void* d_positions, cudaStream_t st) {
     else build_tree_t<double, uint64_t>(P, (const double*)d_positions, st);
 }
 
+// after the strong list exists: number of P2P particle pairs and the P2P work items
+static void finish_lists(Plan& P, cudaStream_t st) {
+    const int L = P.L;
+    DevBuf<unsigned long long> cnt;
+    cnt.alloc(2);
+    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 16, st));
+    count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], P.n_leaves, cnt.p);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    unsigned long long h[2] = {0, 0};
+    FMM_CUDA_CHECK(cudaMemcpyAsync(h, cnt.p, 16, cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    P.n_p2p_pairs = (int64_t)h[0];
+    {
+        // work items of the P2P kernel: budget = twice the mean number of source particles per target leaf (at least 1024)
+        const int32_t* lcnt = P.box_count.p + P.level_off[L];
+        const int64_t mean_src = (int64_t)(h[1] / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
+        const int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
+        DevBuf<int32_t> nseg, any_multi;
+        DevBuf<int64_t> seg_off, scratch;
+        nseg.alloc(P.n_leaves);
+        any_multi.alloc(1);
+        FMM_CUDA_CHECK(cudaMemsetAsync(any_multi.p, 0, sizeof(int32_t), st));
+        seg_off.alloc(P.n_leaves + 1);
+        scratch.alloc(scan_scratch_elems(P.n_leaves + 1));
+        p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, nullptr, nullptr,
+                                                                 any_multi.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        exclusive_scan<int64_t>(SegLoad{nseg.p, P.n_leaves}, seg_off.p, P.n_leaves + 1, scratch.p, st);
+        int64_t n_items = 0;
+        int32_t multi = 0;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&n_items, seg_off.p + P.n_leaves, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&multi, any_multi.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        P.n_p2p_items = n_items;
+        P.p2p_multi = multi != 0;
+        P.p2p_items.alloc((size_t)n_items * sizeof(P2PItem));
+        if (n_items > 0) {
+            p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, seg_off.p,
+                                                                     reinterpret_cast<P2PItem*>(P.p2p_items.p), nullptr);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+    }
+}
+
+static void build_lists_cross(Plan& P, cudaStream_t st) {
+    const int s = P.s, L = P.L;
+    const int nch = 1 << s;
+    P.weak_off.alloc(P.n_boxes + 1);
+    P.weak_level_off.assign(L + 2, 0);
+    DevBuf<int32_t> ftgt, fsrc;
+    ftgt.alloc(1); fsrc.alloc(1);
+    FMM_CUDA_CHECK(cudaMemsetAsync(ftgt.p, 0, 4, st));  // (root, root) fails eq. (4): d = 0
+    FMM_CUDA_CHECK(cudaMemsetAsync(fsrc.p, 0, 4, st));
+    int64_t nfail = 1;
+    std::vector<DevBuf<int32_t>> wt(2 * L + 1), ws(2 * L + 1);
+    std::vector<int64_t> wn(2 * L + 1, 0);
+    int lt = 0, ls = 0, step = 0;
+    int64_t n_weak = 0;
+    while (!(lt == L && ls == L)) {
+        const int refine_src = lt == ls;  // PAPER.md:85-87 for one hierarchy: sources first, then targets
+        if (refine_src) ++ls; else ++lt;
+        const int64_t total = nfail << s;
+        MarchArgs A{ftgt.p, fsrc.p, nfail, s, refine_src, P.level_off[lt], P.level_off[ls], P.box_count.p, P.box_ctr.p, P.box_rad.p, P.theta};
+        DevBuf<uint8_t> codes;
+        DevBuf<unsigned long long> S, scr;
+        codes.alloc(total + 1);
+        S.alloc(total + 1);
+        scr.alloc(scan_scratch_elems(total + 1));
+        if (total > 0) {
+            march_classify_k<<<nblocks(total, 256), 256, 0, st>>>(A, codes.p);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+        exclusive_scan<unsigned long long, CodeLoad>(CodeLoad{codes.p, total}, S.p, total + 1, scr.p, st);
+        unsigned long long tot = 0;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&tot, S.p + total, sizeof(tot), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        const int64_t nweak_l = (int64_t)(tot & 0xffffffffull), nfail2 = (int64_t)(tot >> 32);
+        if (nweak_l >= 0xffffffffll || nfail2 >= 0xffffffffll) {
+            set_error("interaction list of one step exceeds 2^32-1 pairs");
+            throw CudaFail{FMM_ERR_UNSUPPORTED};
+        }
+        wt[step].alloc(nweak_l); ws[step].alloc(nweak_l); wn[step] = nweak_l;
+        DevBuf<int32_t> ftgt2, fsrc2;
+        ftgt2.alloc(nfail2); fsrc2.alloc(nfail2);
+        if (total > 0) {
+            march_compact_k<<<nblocks(total, 256), 256, 0, st>>>(A, codes.p, S.p, wt[step].p, ws[step].p, ftgt2.p, fsrc2.p);
+            FMM_CUDA_CHECK(cudaGetLastError());
+        }
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        std::swap(ftgt.p, ftgt2.p); std::swap(ftgt.n, ftgt2.n);
+        std::swap(fsrc.p, fsrc2.p); std::swap(fsrc.n, fsrc2.n);
+        nfail = nfail2;
+        n_weak += nweak_l;
+        ++step;
+    }
+    (void)nch;
+    if (n_weak > 0x7fffff00ll || nfail > 0x7fffff00ll) { set_error("interaction lists exceed 2^31 pairs"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+
+    // canonical form: stable sort by target id (steps concatenated in chronological order), CSR offsets by counting
+    auto sort_by_key = [&](DevBuf<int32_t>& keys, DevBuf<int32_t>& vals, int64_t n, int64_t n_keys, int64_t* off_out /*n_keys + 1, device*/) {
+        DevBuf<unsigned long long> cnt;
+        DevBuf<int64_t> scr64;
+        cnt.alloc(n_keys + 1);
+        scr64.alloc(scan_scratch_elems(n_keys + 1));
+        FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, (n_keys + 1) * sizeof(unsigned long long), st));
+        if (n > 0) {
+            int bits = 8;
+            while (((int64_t)1 << bits) < n_keys) bits += 8;
+            DevBuf<int32_t> kb, vb, hist, scr;
+            kb.alloc(n); vb.alloc(n);
+            const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
+            hist.alloc((size_t)256 * nblk + 1);
+            scr.alloc(scan_scratch_elems((int64_t)256 * nblk));
+            const int where = radix_sort_pairs<uint32_t>(reinterpret_cast<uint32_t*>(keys.p), vals.p, reinterpret_cast<uint32_t*>(kb.p), vb.p, n, bits,
+                                                         hist.p, scr.p, st);
+            if (where == 1) {
+                FMM_CUDA_CHECK(cudaMemcpyAsync(keys.p, kb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+                FMM_CUDA_CHECK(cudaMemcpyAsync(vals.p, vb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+            }
+            count_keys_k<<<nblocks(n, 256), 256, 0, st>>>(keys.p, n, cnt.p);
+            FMM_CUDA_CHECK(cudaGetLastError());
+            FMM_CUDA_CHECK(cudaStreamSynchronize(st));  // temporaries are freed on scope exit
+        }
+        exclusive_scan<int64_t>(CntLoad{cnt.p, n_keys}, off_out, n_keys + 1, scr64.p, st);
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    };
+    P.n_weak = n_weak;
+    P.weak_tgt.alloc(n_weak); P.weak_src.alloc(n_weak);
+    {
+        int64_t o = 0;
+        for (int k = 0; k < step; ++k) {
+            if (!wn[k]) continue;
+            FMM_CUDA_CHECK(cudaMemcpyAsync(P.weak_tgt.p + o, wt[k].p, wn[k] * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+            FMM_CUDA_CHECK(cudaMemcpyAsync(P.weak_src.p + o, ws[k].p, wn[k] * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+            o += wn[k];
+        }
+    }
+    sort_by_key(P.weak_tgt, P.weak_src, n_weak, P.n_boxes, P.weak_off.p);
+    for (int l = 0; l <= L + 1; ++l)  // weak pairs are sorted by target id, hence by target level
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&P.weak_level_off[l], P.weak_off.p + P.level_off[l], sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    // strong list = pairs still failing at (L, L) (rule L3)
+    P.n_strong = nfail;
+    P.strong_off.alloc(P.n_leaves + 1);
+    P.strong_src.alloc(nfail);
+    sort_by_key(ftgt, fsrc, nfail, P.n_leaves, P.strong_off.p);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_src.p, fsrc.p, nfail * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+}
+
 void build_lists(Plan& P, cudaStream_t st) {
     cudaEvent_t e0, e1;
     FMM_CUDA_CHECK(cudaEventCreate(&e0));
     FMM_CUDA_CHECK(cudaEventCreate(&e1));
     FMM_CUDA_CHECK(cudaEventRecord(e0, st));
     const int s = P.s, L = P.L;
+    if (P.cross_level) {
+        build_lists_cross(P, st);
+        finish_lists(P, st);
+        FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        float msx = 0;
+        cudaEventElapsedTime(&msx, e0, e1);
+        P.plan_ms[2] = msx;
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+        return;
+    }
     P.weak_off.alloc(P.n_boxes + 1);
     FMM_CUDA_CHECK(cudaMemsetAsync(P.weak_off.p, 0, (P.n_boxes + 1) * sizeof(int64_t), st));
     P.weak_level_off.assign(L + 2, 0);
@@ -593,45 +812,7 @@ void build_lists(Plan& P, cudaStream_t st) {
     P.strong_src.alloc(nfail);
     FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_off.p, foff.p, (P.n_leaves + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
     FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_src.p, fsrc.p, nfail * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-    DevBuf<unsigned long long> cnt;
-    cnt.alloc(2);
-    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 16, st));
-    count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], P.n_leaves, cnt.p);
-    FMM_CUDA_CHECK(cudaGetLastError());
-    unsigned long long h[2] = {0, 0};
-    FMM_CUDA_CHECK(cudaMemcpyAsync(h, cnt.p, 16, cudaMemcpyDeviceToHost, st));
-    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-    P.n_p2p_pairs = (int64_t)h[0];
-    {
-        // work items of the P2P kernel: budget = twice the mean number of source particles per target leaf (at least 1024)
-        const int32_t* lcnt = P.box_count.p + P.level_off[L];
-        const int64_t mean_src = (int64_t)(h[1] / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
-        const int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
-        DevBuf<int32_t> nseg, any_multi;
-        DevBuf<int64_t> seg_off, scratch;
-        nseg.alloc(P.n_leaves);
-        any_multi.alloc(1);
-        FMM_CUDA_CHECK(cudaMemsetAsync(any_multi.p, 0, sizeof(int32_t), st));
-        seg_off.alloc(P.n_leaves + 1);
-        scratch.alloc(scan_scratch_elems(P.n_leaves + 1));
-        p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, nullptr, nullptr,
-                                                                 any_multi.p);
-        FMM_CUDA_CHECK(cudaGetLastError());
-        exclusive_scan<int64_t>(SegLoad{nseg.p, P.n_leaves}, seg_off.p, P.n_leaves + 1, scratch.p, st);
-        int64_t n_items = 0;
-        int32_t multi = 0;
-        FMM_CUDA_CHECK(cudaMemcpyAsync(&n_items, seg_off.p + P.n_leaves, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        FMM_CUDA_CHECK(cudaMemcpyAsync(&multi, any_multi.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-        P.n_p2p_items = n_items;
-        P.p2p_multi = multi != 0;
-        P.p2p_items.alloc((size_t)n_items * sizeof(P2PItem));
-        if (n_items > 0) {
-            p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, seg_off.p,
-                                                                     reinterpret_cast<P2PItem*>(P.p2p_items.p), nullptr);
-            FMM_CUDA_CHECK(cudaGetLastError());
-        }
-    }
+    finish_lists(P, st);
     FMM_CUDA_CHECK(cudaEventRecord(e1, st));
     FMM_CUDA_CHECK(cudaStreamSynchronize(st));
     float ms = 0;

@@ -187,13 +187,14 @@ def fmm_plan_copy_lists(plan):
 class Plan:
     """gen_hierarchy(...) / eval_potential(...) of Listing 1 as an object: build once, evaluate many."""
 
-    def __init__(self, positions, p, N_max, s, theta=0.77, stream=None):
+    def __init__(self, positions, p, N_max, s, theta=0.77, stream=None, cross_level=0):
         self.N = positions.shape[0]
         self.dtype = _dtype_code(positions)
         self.tdtype = positions.dtype
         self.device = positions.device
         self.p, self.N_max, self.s, self.theta = p, N_max, s, theta
-        self.handle = fmm_plan_create(positions, p, N_max, s, theta, 0, stream)
+        self.cross_level = int(cross_level)
+        self.handle = fmm_plan_create(positions, p, N_max, s, theta, self.cross_level, stream)
         self.info = fmm_plan_info(self.handle)
 
     def evaluate(self, charges, want_potential=True, want_field=True, stream=None):

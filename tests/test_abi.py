@@ -41,8 +41,8 @@ def test_argument_errors_are_status_codes(L):
         adm = fmm.fmm_admissibility(theta, 0)
         st = L.fmm_plan_create(dummy, N, p, nmax, s, C.byref(adm), fmm.FMM_F32, None, C.byref(h))
         assert st == fmm.FMM_ERR_INVALID_ARG and h.value is None
-    adm = fmm.fmm_admissibility(0.77, 1)
-    assert L.fmm_plan_create(dummy, 10, 4, 8, 2, C.byref(adm), fmm.FMM_F32, None, C.byref(h)) == fmm.FMM_ERR_UNSUPPORTED
+    adm = fmm.fmm_admissibility(0.77, 2)  # cross_level is 0 (same-level lists) or 1 (level marching)
+    assert L.fmm_plan_create(dummy, 10, 4, 8, 2, C.byref(adm), fmm.FMM_F32, None, C.byref(h)) == fmm.FMM_ERR_INVALID_ARG
     assert L.fmm_evaluate(None, None, None, None, None) == fmm.FMM_ERR_INVALID_ARG
     assert L.fmm_plan_destroy(None) == fmm.FMM_OK
     assert fmm.fmm_version().startswith("paper_2511_15269_b200")

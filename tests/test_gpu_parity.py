@@ -20,9 +20,9 @@ def rel2(a, b):
     return np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b)
 
 
-def gpu_plan(pos, p, N_max, s, theta=0.77):
+def gpu_plan(pos, p, N_max, s, theta=0.77, cross_level=0):
     tp = torch.from_numpy(np.ascontiguousarray(pos)).cuda()
-    return fmm.Plan(tp, p, N_max, s, theta)
+    return fmm.Plan(tp, p, N_max, s, theta, cross_level=cross_level)
 
 
 def gpu_eval(P, q):
@@ -194,6 +194,47 @@ def test_kernel_families_agree_with_the_oracle_fp32(N, N_max, s, p):
         u, f = gpu_eval(P, q)
         assert rel2(u, uo) <= 1e-5 and rel2(f, fo) <= 1e-5, (variant, rel2(u, uo), rel2(f, fo))
     P.close()
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("N,N_max,s,p,theta", [(4096, 64, 3, 6, 0.77), (1024, 16, 1, 6, 0.77), (4096, 8, 3, 4, 0.5), (3000, 20, 2, 8, 0.77),
+                                                (5, 8, 3, 4, 0.77), (129, 128, 3, 3, 0.77), (1000, 1, 1, 2, 0.77)])
+def test_cross_level_lists(dtype, N, N_max, s, p, theta):
+    """cross_level = 1 (level marching): hierarchy and both lists bit-exact against the oracle's, potential and
+    field within the north_star tolerance of the oracle evaluated on the same lists, and fewer weak pairs than same-level."""
+    pos, q = inputs.uniform_cube(N, 21, dtype)
+    P = gpu_plan(pos, p, N_max, s, theta, cross_level=1)
+    Po = O.Plan(pos, p, N_max, s, theta, cross_level=1)
+    assert_same_hierarchy(P, Po, dtype)
+    u, f = gpu_eval(P, q)
+    uo, fo = Po.evaluate(q)
+    assert rel2(u, uo) <= TOL[dtype] and rel2(f, fo) <= TOL[dtype]
+    if Po.L >= 2:
+        assert P.info["n_weak"] < O.Plan(pos, p, N_max, s, theta).n_weak
+    if dtype == np.float32:
+        for variant in (1, 2, 3):
+            fmm.fmm_plan_set_m2l_variant(P.handle, variant)
+            u, f = gpu_eval(P, q)
+            assert rel2(u, uo) <= TOL[dtype] and rel2(f, fo) <= TOL[dtype], variant
+    P.close()
+
+
+def test_cross_level_clusters_and_lattice_fp32():
+    """non-uniform and all-ties inputs through the marching builder (stable sort by target must keep sources ascending)"""
+    for name, n in (("clusters", 30000), ("film", 0)):
+        if name == "clusters":
+            pos, q = inputs.gaussian_clusters(n, 5, np.float32)
+            args = (8, 32, 3)
+        else:
+            pos, q = inputs.thin_film(32, 32, 4, 6, np.float32)
+            args = (6, 16, 3)
+        P = gpu_plan(pos, *args, cross_level=1)
+        Po = O.Plan(pos, *args, cross_level=1)
+        assert_same_hierarchy(P, Po, np.float32)
+        u, f = gpu_eval(P, q)
+        uo, fo = Po.evaluate(q)
+        assert rel2(u, uo) <= 1e-5 and rel2(f, fo) <= 1e-5
+        P.close()
 
 
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
