@@ -287,14 +287,14 @@ def test_non_finite_positions_are_rejected():
 
 
 # ------------------------------------------------------------------------------------------- full-size configs (sampled oracle)
-def sampled_case(name, n_sample_leaves=12, seed=0):
+def sampled_case(name, n_sample_leaves=12, seed=0, cross_level=0):
     """BASELINE full-size configs in the configuration bench.py times: hierarchy/lists bit-exact on everything;
     potential/field compared on the particles of a random sample of leaves (the oracle computes exactly those,
     with the same arithmetic as a full run) and against the O(N^2) definition on the same particles."""
     pos, q, c = inputs.make(name)
     dt = pos.dtype.type
-    P = gpu_plan(pos, c["p"], c["N_max"], c["s"], c["theta"])
-    Po = O.Plan(pos, c["p"], c["N_max"], c["s"], c["theta"])
+    P = gpu_plan(pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=cross_level)
+    Po = O.Plan(pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=cross_level)
     assert_same_hierarchy(P, Po, dt)
     u, f = gpu_eval(P, q)
     assert np.all(np.isfinite(u)) and np.all(np.isfinite(f))
@@ -310,10 +310,24 @@ def sampled_case(name, n_sample_leaves=12, seed=0):
     assert rel2(u[sel], ud) <= 1.5 * rel2(uo[sel], ud)
     assert rel2(f[sel], fd) <= 1.5 * rel2(fo[sel], fd)
     P.close()
+    return dict(n_weak=Po.n_weak, err_u=rel2(u[sel], ud), err_f=rel2(f[sel], fd), err_u_oracle=rel2(uo[sel], ud), err_f_oracle=rel2(fo[sel], fd))
 
 
 def test_config2_full_size_sampled():
     sampled_case("cfg2_cube1M_f32")
+
+
+@pytest.mark.parametrize("name,nl,slack", [("cfg2_cube1M_f32", 12, 3.0), ("cfg3_clusters1M_f32_s3", 8, 3.0), ("cfg4_film_f32", 24, 10.0)])
+def test_full_size_sampled_cross_level(name, nl, slack):
+    """level-marching lists at full size: same acceptance as the same-level lists (GPU == oracle on the same lists, error vs
+    the O(N^2) definition within 1.5x the oracle's).  Against the same-level lists at equal theta the scheme itself trades
+    accuracy for pairs: measured on B200, -42 % pairs / 1.6x the error (uniform cube), -51 % / 1.5x (clusters),
+    -62 % / 7x (lattice with tight boxes, p = 6); the bound here only guards the order of magnitude."""
+    rc = sampled_case(name, n_sample_leaves=nl, cross_level=1)
+    rs = sampled_case(name, n_sample_leaves=nl, cross_level=0)
+    print(name, "cross", rc, "same", rs)
+    assert rc["n_weak"] < 0.7 * rs["n_weak"]
+    assert rc["err_u"] < slack * rs["err_u"] and rc["err_f"] < slack * rs["err_f"]
 
 
 @pytest.mark.parametrize("name", ["cfg3_clusters1M_f32_s3", "cfg3_clusters1M_f32_s1"])
