@@ -216,7 +216,7 @@ def run_ours(args):
     esize = pos.dtype.itemsize
     d_pos = torch.from_numpy(pos).cuda()
     d_q = torch.from_numpy(q).cuda()
-    P = fmm.Plan(d_pos, c["p"], c["N_max"], c["s"], c["theta"])
+    P = fmm.Plan(d_pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=args.cross_level)
     plan_ms = P.timings()
     info = P.info
     d_u = torch.empty(N, dtype=tdt, device="cuda")
@@ -276,6 +276,27 @@ def run_ours(args):
     e2e_ms = e2e_s * 1e3 / n_e2e
     assert bool(torch.isfinite(h_u).all()) and bool(torch.isfinite(h_f).all())
 
+    # the same workload with the paper's level-marching lists (fmm_admissibility.cross_level = 1): fewer M2L
+    # pairs at the same theta, somewhat larger error.  Reported beside the headline, not instead of it.
+    alt = None
+    if rank == 0 and not args.no_alt_lists:
+        Pa = fmm.Plan(d_pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=1 - args.cross_level)
+        n_alt = min(args.steps, 50)
+        for _ in range(3):
+            flush.zero_()
+            fmm.fmm_evaluate(Pa.handle, d_q, d_u, d_f)
+        eva = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_alt)]
+        for a, b in eva:
+            flush.zero_()
+            a.record()
+            fmm.fmm_evaluate(Pa.handle, d_q, d_u, d_f)
+            b.record()
+        torch.cuda.synchronize()
+        ms_alt = float(np.mean([a.elapsed_time(b) for a, b in eva]))
+        alt = dict(cross_level=1 - args.cross_level, n_weak=Pa.info["n_weak"], n_strong=Pa.info["n_strong"], ms_per_step=ms_alt,
+                   value=N / ms_alt / 1e3, unit=UNIT, steps=n_alt, plan_ms=Pa.timings())
+        Pa.close()
+
     tmax = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -327,14 +348,15 @@ def run_ours(args):
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms_per_step,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if esize == 4 else "f64", data="synthetic",
-                config=dict(workload=args.workload, N=N, p=c["p"], s=c["s"], N_max=c["N_max"], theta=c["theta"], outputs="potential+field",
+                config=dict(workload=args.workload, N=N, p=c["p"], s=c["s"], N_max=c["N_max"], theta=c["theta"], cross_level=args.cross_level,
+                            outputs="potential+field",
                             L=info["L"], n_boxes=info["n_boxes"], n_weak=info["n_weak"], n_strong=info["n_strong"], n_p2p_pairs=info["n_p2p_pairs"],
                             l2="flushed between timed steps (512 MiB memset outside the event pairs)", parallelism="replicas x%d" % world,
                             schedule="concurrent: P2P, the tree passes (M2M, upper-level M2L, L2L) and the leaf-level M2L on three forked streams"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
                 gpu_launches=launches * args.steps, gpu_launches_per_step=launches, roofline=roofline, stages=stages, plan_ms=plan_ms,
-                min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
+                alt_lists=alt, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
     print(json.dumps(line), flush=True)
     P.close()
     if world > 1:
@@ -351,6 +373,9 @@ def main():
     ap.add_argument("--cpu-leaves", type=int, default=48, help="leaves in the cpu_baseline sample")
     ap.add_argument("--ref-leaves", type=int, default=16, help="leaves per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cross-level", type=int, default=0, choices=[0, 1],
+                    help="interaction lists of the timed plan: 0 = same-level (paper default, PAPER.md:72-74), 1 = level marching (PAPER.md:82-89)")
+    ap.add_argument("--no-alt-lists", action="store_true", help="skip the extra measurement with the other list kind")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
