@@ -56,7 +56,7 @@ constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two
 
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
 // the leaf population hold zeros (zero charge), so whole groups can be used without masks.
-template <int TPT>
+template <int TPT, int HS>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
                                                       const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
@@ -163,28 +163,46 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
         const ulonglong2* T2 = reinterpret_cast<const ulonglong2*>(&sm[warp][b][0]);
         for (int j = sl; j < ng; j += nsl) {
             const ulonglong2 xs = T2[4 * j], ys = T2[4 * j + 1], zs = T2[4 * j + 2], qs = T2[4 * j + 3];
+            // staged over the NC = HS * TPT independent chains (all distances, then all rsqrt, then the accumulation) so that
+            // the MUFU latency of one chain is covered by the arithmetic of the others inside one warp
+            constexpr int NC = HS * TPT;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const u64 sx = h ? xs.y : xs.x, sy = h ? ys.y : ys.x, sz = h ? zs.y : zs.x, sq = h ? qs.y : qs.x;
+            for (int h0 = 0; h0 < 2; h0 += HS) {
+                u64 dx[NC], dy[NC], dz[NC], r2[NC];
 #pragma unroll
-                for (int k = 0; k < TPT; ++k) {
-                    const u64 dx = add2(TX[k], sx), dy = add2(TY[k], sy), dz = add2(TZ[k], sz);
-                    u64 r2 = mul2(dx, dx);
-                    r2 = fma2(dy, dy, r2);
-                    r2 = fma2(dz, dz, r2);
+                for (int c = 0; c < NC; ++c) {
+                    const int h = h0 + c / TPT, k = c % TPT;
+                    const u64 sx = h ? xs.y : xs.x, sy = h ? ys.y : ys.x, sz = h ? zs.y : zs.x;
+                    dx[c] = add2(TX[k], sx); dy[c] = add2(TY[k], sy); dz[c] = add2(TZ[k], sz);
+                    r2[c] = mul2(dx[c], dx[c]);
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) r2[c] = fma2(dy[c], dy[c], r2[c]);
+#pragma unroll
+                for (int c = 0; c < NC; ++c) r2[c] = fma2(dz[c], dz[c], r2[c]);
+                float ia[NC], ib[NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
                     float a, b2;
-                    upk(r2, a, b2);
-                    float ia = rsq(a), ib = rsq(b2);
+                    upk(r2[c], a, b2);
+                    ia[c] = rsq(a); ib[c] = rsq(b2);
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const int h = h0 + c / TPT, k = c % TPT;
+                    const u64 sq = h ? qs.y : qs.x;
+                    float a, b2;
+                    upk(r2[c], a, b2);
                     // reading S3: coincident pairs contribute nothing (r^2 below FLT_MIN counts as coincident in fp32)
-                    ia = a >= 1.17549435e-38f ? ia : 0.f;
-                    ib = b2 >= 1.17549435e-38f ? ib : 0.f;
-                    const u64 inv = pk(ia, ib);
+                    const float ja = a >= 1.17549435e-38f ? ia[c] : 0.f;
+                    const float jb = b2 >= 1.17549435e-38f ? ib[c] : 0.f;
+                    const u64 inv = pk(ja, jb);
                     const u64 qi = mul2(sq, inv), inv2 = mul2(inv, inv);
                     const u64 q3 = mul2(qi, inv2);
                     PH[k] = add2(PH[k], qi);
-                    GX[k] = fma2(q3, dx, GX[k]);
-                    GY[k] = fma2(q3, dy, GY[k]);
-                    GZ[k] = fma2(q3, dz, GZ[k]);
+                    GX[k] = fma2(q3, dx[c], GX[k]);
+                    GY[k] = fma2(q3, dy[c], GY[k]);
+                    GZ[k] = fma2(q3, dz[c], GZ[k]);
                 }
             }
         }
@@ -226,7 +244,7 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
 
 }  // namespace
 
-template <int TPT>
+template <int TPT, int HS>
 static void p2p_launch_t(const Plan& P, cudaStream_t st) {
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
@@ -234,10 +252,39 @@ static void p2p_launch_t(const Plan& P, cudaStream_t st) {
     if (n_items == 0) return;
     if (P.p2p_multi) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
-    p2p_fast_k<TPT><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
+    p2p_fast_k<TPT, HS><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
                                               reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
 
-void p2p_fast_launch(const Plan& P, cudaStream_t st) { p2p_launch_t<4>(P, st); }  // measured on B200: TPT 2 / 4 / 8 -> 0.50 / 0.49 / 0.49 ms (config 2)
+// Targets per lane.  A median-split tree gives every leaf the same population (+-1), so max_leaf decides the lane layout for
+// the whole launch: the warp holds ntgp = 8, 16 or 32 target groups of TPT targets (x 4, 2 or 1 source slices); pick the
+// layout that wastes the fewest target slots, ties to the fewest groups (most register reuse of a staged source).
+// Measured on B200 (P2P stage, CUDA events): config 2 (leaves of 30-31): <TPT, HS> = <4,1> 0.488, <4,2> 0.482, <2,2> 0.525,
+// <1,2> 0.494, <8,1> 0.489 ms; config 4 (leaves of 16): <4,*> 0.562, <2,2> 0.433 ms.
+static int choose_tpt(int max_leaf) {
+    int best = 4;
+    double best_eff = -1.0;
+    const int m = max_leaf < 1 ? 1 : (max_leaf > 256 ? 256 : max_leaf);  // larger leaves are cut into chunks of 32 * TPT targets
+    for (int ntgp = 8; ntgp <= 32; ntgp *= 2) {
+        const int tpt = (m + ntgp - 1) / ntgp;
+        if (tpt > 8) continue;
+        const double eff = (double)m / (tpt * ntgp);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = tpt; }
+    }
+    return best;
+}
+
+void p2p_fast_launch(const Plan& P, cudaStream_t st) {
+    switch (choose_tpt(P.max_leaf)) {
+        case 1: p2p_launch_t<1, 2>(P, st); break;
+        case 2: p2p_launch_t<2, 2>(P, st); break;
+        case 3: p2p_launch_t<3, 2>(P, st); break;
+        case 4: p2p_launch_t<4, 2>(P, st); break;
+        case 5: p2p_launch_t<5, 1>(P, st); break;
+        case 6: p2p_launch_t<6, 1>(P, st); break;
+        case 7: p2p_launch_t<7, 1>(P, st); break;
+        default: p2p_launch_t<8, 1>(P, st); break;
+    }
+}
 
 }  // namespace fmm

@@ -53,7 +53,7 @@ struct XArgs {
 
 // XW warps per CTA; SYNC = lockstep barriers (all warps then run the operator, also on padding lanes)
 template <typename T, int P, int KIND, int XW, bool SYNC>
-__global__ void __launch_bounds__(XW * 32, XW == 8 ? 2 : (XW == 4 ? 4 : 1)) xlate_fast_k(XArgs a) {
+__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (XW == 4 ? 4 : 1))) xlate_fast_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -182,7 +182,7 @@ bool dispatch(int p, const XArgs& a, cudaStream_t st) {
 
 }  // namespace
 
-bool xlate_fast_available(int p, fmm_dtype dt) { return dt == FMM_F32 && p >= 1 && p <= 8; }
+bool xlate_fast_available(int p, fmm_dtype dt) { return p >= 1 && p <= 8 && (dt == FMM_F32 || dt == FMM_F64); }
 
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     XArgs a{};
@@ -206,7 +206,11 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
     }
     if (a.n <= 0) return;
     bool ok = false;
-    if (kind == 0) ok = dispatch<float, 0>(P.p, a, st);
+    if (P.dtype == FMM_F64) {
+        if (kind == 0) ok = dispatch<double, 0>(P.p, a, st);
+        else if (kind == 1) ok = dispatch<double, 1>(P.p, a, st);
+        else ok = dispatch<double, 2>(P.p, a, st);
+    } else if (kind == 0) ok = dispatch<float, 0>(P.p, a, st);
     else if (kind == 1) ok = dispatch<float, 1>(P.p, a, st);
     else ok = dispatch<float, 2>(P.p, a, st);
     if (!ok) { set_error("no register translation kernel for this order"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }

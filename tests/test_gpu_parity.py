@@ -177,7 +177,8 @@ def test_plan_reuse_and_linearity():
     u3, f3 = gpu_eval(P, 2.0 * q1 - 3.0 * q2)
     assert rel2(u3, 2.0 * u1 - 3.0 * u2) < 1e-12 and rel2(f3, 2.0 * f1 - 3.0 * f2) < 1e-12
     u1b, f1b = gpu_eval(P, q1)
-    assert np.array_equal(u1, u1b) and np.array_equal(f1, f1b)  # deterministic
+    # repeatable to rounding: the register translation kernels accumulate M2L/L2L results with atomics, whose order varies
+    assert rel2(u1b, u1) < 1e-13 and rel2(f1b, f1) < 1e-13
     P.close()
 
 
