@@ -138,6 +138,9 @@ int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evalua
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
 bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0 = 0, int64_t e1 = -1);  // kind 1: weak pairs [e0, e1)
+// xlate_smem.cu: the same three operators for 9 <= p <= 12, one thread per translation with the state vector in shared memory
+bool xlate_smem_available(int p, fmm_dtype dt);
+void xlate_smem_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1);
 // m2l_packed.cu: fp32 M2L with two weak pairs per thread in packed f32x2 arithmetic (p <= 8); results are ADDED to Lc
 bool m2l_packed_available(int p, fmm_dtype dt);
 void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1);  // weak pairs [e0, e1)

@@ -182,9 +182,11 @@ bool dispatch(int p, const XArgs& a, cudaStream_t st) {
 
 }  // namespace
 
-bool xlate_fast_available(int p, fmm_dtype dt) { return p >= 1 && p <= 8 && (dt == FMM_F32 || dt == FMM_F64); }
+// p <= 8: state vector in registers (this file); 9 <= p <= 12: state vector in shared memory (xlate_smem.cu)
+bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && ((p >= 1 && p <= 8) || xlate_smem_available(p, dt)); }
 
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
+    if (P.p > 8) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }
     XArgs a{};
     a.box_count = P.box_count.p;
     a.ctr = P.box_ctr.p;
