@@ -63,7 +63,7 @@ P2P_FLOP_PER_PAIR = 20.0  # 3 sub, mul+2 FMA, rsqrt, 3 mul, 1+3 FMA, mask (SURVE
 
 # dram__bytes_read.sum + dram__bytes_write.sum per evaluate of the named kernel, from the committed `ncu --set full` capture
 # profiles/r01_ncu_full_evaluate.md (M2L = leaf-level launch 71.27 MB + upper-levels launch 8.66 MB)
-NCU_DRAM_BYTES = {"cfg2_cube1M_f32": {"m2l": 79.93e6, "p2p": 36.84e6}}
+NCU_DRAM_BYTES = {"cfg2_cube1M_f32": {"m2l": 79.58e6, "p2p": 37.13e6}}
 
 
 class ClockSampler:

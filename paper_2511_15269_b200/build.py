@@ -56,5 +56,15 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_ubench():
+    """Stand-alone FP32-pipe micro-benchmark (csrc/ubench_fp32_pipe.cu); not part of the library."""
+    exe = os.path.join(HERE, "ubench_fp32_pipe")
+    subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, os.path.join(CSRC, "ubench_fp32_pipe.cu")])
+    return exe
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--ubench" in sys.argv:
+        print(build_ubench())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
