@@ -50,6 +50,15 @@ def lib():
         L.orc_evaluate.argtypes = [C.c_void_p, _dp, _bp, _dp, _dp]
         L.orc_direct.argtypes = [_dp, _dp, C.c_int64, _ip, C.c_int64, _dp, _dp]
         L.orc_num_threads.restype = C.c_int
+        _i32p = C.POINTER(C.c_int)
+        L.orc_plan_st_create.argtypes = [_dp, C.c_int64, _dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double]
+        L.orc_plan_st_create.restype = C.c_void_p
+        L.orc_plan_st_destroy.argtypes = [C.c_void_p]
+        L.orc_plan_st_info.argtypes = [C.c_void_p, C.c_int, _i32p] + [_ip] * 5 + [_i32p]
+        L.orc_plan_st_copy_tree.argtypes = [C.c_void_p, C.c_int, _ip, _ip, _ip, _dp, _dp, _dp, _dp]
+        L.orc_plan_st_copy_lists.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, _i32p]
+        L.orc_evaluate_st.argtypes = [C.c_void_p, _dp, _dp, _dp]
+        L.orc_direct_st.argtypes = [_dp, _dp, C.c_int64, _dp, C.c_int64, _dp, _dp]
         _lib = L
     return _lib
 
@@ -193,4 +202,71 @@ def direct(pos, q, targets=None):
     pot = np.empty(tg.shape[0])
     fld = np.empty((tg.shape[0], 3))
     lib().orc_direct(_d(pos), _d(q), N, _i(tg), tg.shape[0], _d(pot), _d(fld))
+    return pot, fld
+
+
+class PlanST:
+    """Oracle plan for separate sources and targets: two hierarchies, level-marching lists."""
+
+    def __init__(self, src_pos, tgt_pos, p, N_max, s, theta=0.77):
+        self.spos = np.ascontiguousarray(src_pos, dtype=np.float64)
+        self.tpos = np.ascontiguousarray(tgt_pos, dtype=np.float64)
+        assert self.spos.ndim == 2 and self.spos.shape[1] == 3 and self.tpos.ndim == 2 and self.tpos.shape[1] == 3
+        self.Ns, self.Nt = self.spos.shape[0], self.tpos.shape[0]
+        self.p, self.N_max, self.s, self.theta = int(p), int(N_max), int(s), float(theta)
+        self._h = lib().orc_plan_st_create(_d(self.spos), self.Ns, _d(self.tpos), self.Nt, self.p, self.N_max, self.s, self.theta)
+        self.info = {}
+        for which, name in ((0, "src"), (1, "tgt")):
+            L = C.c_int()
+            ns = C.c_int()
+            v = [C.c_int64() for _ in range(5)]
+            lib().orc_plan_st_info(self._h, which, C.byref(L), *[C.byref(x) for x in v], C.byref(ns))
+            self.info[name] = dict(L=L.value, n_boxes=v[0].value, n_leaves=v[1].value)
+            self.n_weak, self.n_strong, self.n_p2p_pairs, self.n_steps = v[2].value, v[3].value, v[4].value, ns.value
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().orc_plan_st_destroy(self._h)
+            self._h = None
+
+    def tree(self, which):
+        """which: 'src' or 'tgt'"""
+        w = 0 if which == "src" else 1
+        nb = self.info[which]["n_boxes"]
+        N = self.Ns if w == 0 else self.Nt
+        t = dict(perm=np.empty(N, np.int64), box_start=np.empty(nb, np.int64), box_count=np.empty(nb, np.int64),
+                 lo=np.empty((nb, 3)), hi=np.empty((nb, 3)), ctr=np.empty((nb, 3)), rad=np.empty(nb))
+        lib().orc_plan_st_copy_tree(self._h, w, _i(t["perm"]), _i(t["box_start"]), _i(t["box_count"]), _d(t["lo"]), _d(t["hi"]),
+                                    _d(t["ctr"]), _d(t["rad"]))
+        return t
+
+    def lists(self):
+        """weak: CSR by target box (global id in the target hierarchy), sources = global ids in the source hierarchy;
+        strong: CSR by target leaf, sources = source leaf indices; steps: the (l_trg, l_src) pairs visited."""
+        ls = dict(weak_off=np.empty(self.info["tgt"]["n_boxes"] + 1, np.int64), weak_src=np.empty(self.n_weak, np.int64),
+                  strong_off=np.empty(self.info["tgt"]["n_leaves"] + 1, np.int64), strong_src=np.empty(self.n_strong, np.int64))
+        steps = np.empty(2 * self.n_steps, np.int32)
+        lib().orc_plan_st_copy_lists(self._h, _i(ls["weak_off"]), _i(ls["weak_src"]), _i(ls["strong_off"]), _i(ls["strong_src"]),
+                                     steps.ctypes.data_as(C.POINTER(C.c_int)))
+        ls["steps"] = steps.reshape(-1, 2)
+        return ls
+
+    def evaluate(self, q):
+        """potential (Nt,), field (Nt,3) at the targets, in target input order."""
+        q = np.ascontiguousarray(q, dtype=np.float64)
+        assert q.shape == (self.Ns,)
+        pot = np.empty(self.Nt)
+        fld = np.empty((self.Nt, 3))
+        lib().orc_evaluate_st(self._h, _d(q), _d(pot), _d(fld))
+        return pot, fld
+
+
+def direct_st(src_pos, q, tgt_pos):
+    """Plain definition at separate targets: u(t_i) = -(1/4pi) sum_j q_j/|t_i - s_j|, field = -grad u."""
+    sp = np.ascontiguousarray(src_pos, dtype=np.float64)
+    tp = np.ascontiguousarray(tgt_pos, dtype=np.float64)
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    pot = np.empty(tp.shape[0])
+    fld = np.empty((tp.shape[0], 3))
+    lib().orc_direct_st(_d(sp), _d(q), sp.shape[0], _d(tp), tp.shape[0], _d(pot), _d(fld))
     return pot, fld

@@ -550,6 +550,186 @@ void evaluate(const Plan& P, const double* q, const uint8_t* leaf_mask, double* 
     }
 }
 
+// -------------------------------------------------------------------------------------
+// Separate sources and targets: one hierarchy over the source points, one over the target points
+// (same rules T1-T7, same N_max and s), interaction lists by level marching over the two hierarchies, evaluate =
+// P2M/M2M on the source hierarchy, M2L across, L2L/L2P on the target hierarchy, P2P between target and source leaves.
+// -------------------------------------------------------------------------------------
+// eq. (4) between a target box and a source box; the same expression and evaluation order as admissible()
+bool admissible_st(const Tree& Tt, int64_t gt, const Tree& Ts, int64_t gs, double theta) {
+    const double ra = Tt.rad[gt], rb = Ts.rad[gs];
+    const double R = std::max(ra, rb), r = std::min(ra, rb);
+    const double dx = Tt.ctr[3 * gt] - Ts.ctr[3 * gs], dy = Tt.ctr[3 * gt + 1] - Ts.ctr[3 * gs + 1], dz = Tt.ctr[3 * gt + 2] - Ts.ctr[3 * gs + 2];
+    const double d = std::sqrt((dx * dx + dy * dy) + dz * dz);
+    return R + theta * r < theta * d;
+}
+// "average box radius" of a level: mean of the radii of its non-empty boxes, summed in box order
+double mean_radius(const Tree& T, int l) {
+    double sum = 0.0; int64_t cnt = 0;
+    for (int64_t b = 0; b < ((int64_t)1 << (T.s * l)); ++b) {
+        const int64_t g = T.level_off[l] + b;
+        if (T.box_count[g] > 0) { sum += T.rad[g]; ++cnt; }
+    }
+    return cnt ? sum / (double)cnt : 0.0;
+}
+// Level marching, started at (l_trg, l_src) = (0, 0): 1. increase the level with the larger average box
+// radius; 2. if equal, the source level; 3. if one hierarchy has no more levels, the other; 4. stop when no pair is left
+// or both are at their leaf level.  Weak rows: per target box (global id in Tt) the source boxes (global ids in Ts),
+// ascending; strong rows: per target leaf the source leaves still failing at (L_trg, L_src).  steps: the (l_trg, l_src) visited.
+void build_lists_st(const Tree& Tt, const Tree& Ts, double theta, Lists& Ls, std::vector<int>& steps) {
+    const int s = Tt.s, Lt = Tt.L, Lsrc = Ts.L;
+    const int64_t nch = (int64_t)1 << s;
+    const int64_t nbt = Tt.level_off[Lt + 1];
+    const int64_t n_tleaves = (int64_t)1 << (s * Lt);
+    std::vector<std::vector<int64_t>> weak_rows(nbt), strong_rows(n_tleaves);
+    std::vector<std::pair<int64_t, int64_t>> cand, fail;
+    cand.push_back({0, 0});
+    int lt = 0, ls = 0;
+    steps.clear();
+    for (;;) {
+        steps.push_back(lt); steps.push_back(ls);
+        fail.clear();
+        for (auto& pr : cand) {
+            const int64_t gt = Tt.level_off[lt] + pr.first, gs = Ts.level_off[ls] + pr.second;
+            if (admissible_st(Tt, gt, Ts, gs, theta)) weak_rows[gt].push_back(gs);
+            else fail.push_back(pr);
+        }
+        if (lt == Lt && ls == Lsrc) break;
+        bool refine_src;
+        if (ls == Lsrc) refine_src = false;            // rule 3
+        else if (lt == Lt) refine_src = true;          // rule 3
+        else refine_src = !(mean_radius(Tt, lt) > mean_radius(Ts, ls));  // rules 1, 2
+        cand.clear();
+        for (auto& pr : fail)
+            for (int64_t c = 0; c < nch; ++c) {
+                const int64_t a = refine_src ? pr.first : pr.first * nch + c, b = refine_src ? pr.second * nch + c : pr.second;
+                if (Tt.box_count[Tt.level_off[lt + (refine_src ? 0 : 1)] + a] == 0 || Ts.box_count[Ts.level_off[ls + (refine_src ? 1 : 0)] + b] == 0)
+                    continue;  // T5
+                cand.push_back({a, b});
+            }
+        if (refine_src) ++ls; else ++lt;
+    }
+    for (auto& pr : fail) strong_rows[pr.first].push_back(pr.second);
+    Ls.weak_off.assign(nbt + 1, 0); Ls.weak_src.clear();
+    for (int64_t g = 0; g < nbt; ++g) {
+        std::sort(weak_rows[g].begin(), weak_rows[g].end());
+        for (int64_t v : weak_rows[g]) Ls.weak_src.push_back(v);
+        Ls.weak_off[g + 1] = (int64_t)Ls.weak_src.size();
+    }
+    Ls.strong_off.assign(n_tleaves + 1, 0); Ls.strong_src.clear();
+    for (int64_t t = 0; t < n_tleaves; ++t) {
+        std::sort(strong_rows[t].begin(), strong_rows[t].end());
+        for (int64_t v : strong_rows[t]) Ls.strong_src.push_back(v);
+        Ls.strong_off[t + 1] = (int64_t)Ls.strong_src.size();
+    }
+}
+
+struct PlanST {
+    int p = 0; double theta = 0.77;
+    std::vector<double> spos, tpos;
+    Tree Ts, Tt; Lists Ls;
+    std::vector<int> steps;
+};
+
+// potential and field at the targets from charges q at the sources; steps E1-E7 with the two hierarchies
+void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
+    const Tree& Ts = P.Ts; const Tree& Tt = P.Tt; const Lists& Ls = P.Ls;
+    const int p = P.p, K = (p + 1) * (p + 1), s = Ts.s;
+    const int64_t nch = (int64_t)1 << s;
+    const int64_t nbs = Ts.level_off[Ts.L + 1], nbt = Tt.level_off[Tt.L + 1];
+    const int64_t n_sleaves = (int64_t)1 << (s * Ts.L), n_tleaves = (int64_t)1 << (s * Tt.L);
+    const int64_t sleaf0 = Ts.level_off[Ts.L], tleaf0 = Tt.level_off[Tt.L];
+    const double* spos = P.spos.data(); const double* tpos = P.tpos.data();
+    std::vector<double> C((size_t)nbs * K, 0.0), D((size_t)nbt * K, 0.0);
+    // E1: P2M at the source leaves, eq. (13)
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < n_sleaves; ++t) {
+        const int64_t g = sleaf0 + t;
+        std::vector<double> R(K);
+        for (int64_t k = Ts.box_start[g]; k < Ts.box_start[g] + Ts.box_count[g]; ++k) {
+            const int64_t i = Ts.perm[k];
+            regular_basis(p, spos[3 * i] - Ts.ctr[3 * g], spos[3 * i + 1] - Ts.ctr[3 * g + 1], spos[3 * i + 2] - Ts.ctr[3 * g + 2], R.data());
+            for (int c = 0; c < K; ++c) C[(size_t)g * K + c] += q[i] * R[c];
+        }
+    }
+    // E2: M2M in the source hierarchy; b = child centre - parent centre
+    for (int l = Ts.L; l >= 1; --l) {
+        const int64_t nbp = (int64_t)1 << (s * (l - 1));
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t bp = 0; bp < nbp; ++bp) {
+            const int64_t gp = Ts.level_off[l - 1] + bp;
+            std::vector<double> tmp(K);
+            for (int64_t j = 0; j < nch; ++j) {
+                const int64_t gc = Ts.level_off[l] + bp * nch + j;
+                if (Ts.box_count[gc] == 0) continue;
+                const double b[3] = {Ts.ctr[3 * gc] - Ts.ctr[3 * gp], Ts.ctr[3 * gc + 1] - Ts.ctr[3 * gp + 1], Ts.ctr[3 * gc + 2] - Ts.ctr[3 * gp + 2]};
+                translate(0, p, &C[(size_t)gc * K], b, tmp.data());
+                for (int c = 0; c < K; ++c) C[(size_t)gp * K + c] += tmp[c];
+            }
+        }
+    }
+    // E3: M2L over the weak list; b = source centre - target centre
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t gt = 0; gt < nbt; ++gt) {
+        std::vector<double> tmp(K);
+        for (int64_t e = Ls.weak_off[gt]; e < Ls.weak_off[gt + 1]; ++e) {
+            const int64_t gs = Ls.weak_src[e];
+            const double b[3] = {Ts.ctr[3 * gs] - Tt.ctr[3 * gt], Ts.ctr[3 * gs + 1] - Tt.ctr[3 * gt + 1], Ts.ctr[3 * gs + 2] - Tt.ctr[3 * gt + 2]};
+            translate(1, p, &C[(size_t)gs * K], b, tmp.data());
+            for (int c = 0; c < K; ++c) D[(size_t)gt * K + c] += tmp[c];
+        }
+    }
+    // E4: L2L in the target hierarchy; b = parent centre - child centre
+    for (int l = 1; l <= Tt.L; ++l) {
+        const int64_t nbl = (int64_t)1 << (s * l);
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t bc = 0; bc < nbl; ++bc) {
+            const int64_t gc = Tt.level_off[l] + bc, gp = Tt.level_off[l - 1] + bc / nch;
+            if (Tt.box_count[gc] == 0) continue;
+            std::vector<double> tmp(K);
+            const double b[3] = {Tt.ctr[3 * gp] - Tt.ctr[3 * gc], Tt.ctr[3 * gp + 1] - Tt.ctr[3 * gc + 1], Tt.ctr[3 * gp + 2] - Tt.ctr[3 * gc + 2]};
+            translate(2, p, &D[(size_t)gp * K], b, tmp.data());
+            for (int c = 0; c < K; ++c) D[(size_t)gc * K + c] += tmp[c];
+        }
+    }
+    // E5 L2P, E6 P2P (every source of the strong-listed source leaves; zero-distance pairs contribute nothing, S3), E7
+    const double inv4pi = 1.0 / (4.0 * M_PI);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t t = 0; t < n_tleaves; ++t) {
+        const int64_t g = tleaf0 + t;
+        std::vector<double> R(K), G(3 * K);
+        for (int64_t k = Tt.box_start[g]; k < Tt.box_start[g] + Tt.box_count[g]; ++k) {
+            const int64_t i = Tt.perm[k];
+            const double x = tpos[3 * i] - Tt.ctr[3 * g], y = tpos[3 * i + 1] - Tt.ctr[3 * g + 1], z = tpos[3 * i + 2] - Tt.ctr[3 * g + 2];
+            regular_basis(p, x, y, z, R.data());
+            regular_grad(p, x, y, z, R.data(), G.data());
+            double phi_far = 0.0, gfar[3] = {0, 0, 0};
+            for (int n = 0; n <= p; ++n)
+                for (int m = -n; m <= n; ++m) {
+                    const double w = ((m == 0) ? 1.0 : 2.0) * sgn(m) * D[(size_t)g * K + IDX(n, m)];
+                    phi_far += w * R[IDX(n, m)];
+                    for (int c = 0; c < 3; ++c) gfar[c] += w * G[3 * IDX(n, m) + c];
+                }
+            double phi_near = 0.0, gnear[3] = {0, 0, 0};
+            for (int64_t e = Ls.strong_off[t]; e < Ls.strong_off[t + 1]; ++e) {
+                const int64_t gs = sleaf0 + Ls.strong_src[e];
+                for (int64_t kk = Ts.box_start[gs]; kk < Ts.box_start[gs] + Ts.box_count[gs]; ++kk) {
+                    const int64_t j = Ts.perm[kk];
+                    const double dx = tpos[3 * i] - spos[3 * j], dy = tpos[3 * i + 1] - spos[3 * j + 1], dz = tpos[3 * i + 2] - spos[3 * j + 2];
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 == 0.0) continue;  // S3
+                    const double r = std::sqrt(r2);
+                    phi_near += q[j] / r;
+                    const double f = q[j] / (r2 * r);
+                    gnear[0] -= f * dx; gnear[1] -= f * dy; gnear[2] -= f * dz;
+                }
+            }
+            if (pot) pot[i] = -(phi_far + phi_near) * inv4pi;
+            if (field) for (int c = 0; c < 3; ++c) field[3 * i + c] = (gfar[c] + gnear[c]) * inv4pi;
+        }
+    }
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -648,6 +828,69 @@ void orc_direct(const double* pos, const double* q, int64_t N, const int64_t* tg
         }
         if (pot) pot[a] = -ph * inv4pi;
         if (field) for (int c = 0; c < 3; ++c) field[3 * a + c] = g[c] * inv4pi;
+    }
+}
+// ---- separate sources and targets
+void* orc_plan_st_create(const double* spos, int64_t Ns, const double* tpos, int64_t Nt, int p, int N_max, int s, double theta) {
+    PlanST* P = new PlanST();
+    P->p = p; P->theta = theta;
+    P->spos.assign(spos, spos + 3 * Ns); P->tpos.assign(tpos, tpos + 3 * Nt);
+    build_tree(P->spos.data(), Ns, N_max, s, P->Ts);
+    build_tree(P->tpos.data(), Nt, N_max, s, P->Tt);
+    build_lists_st(P->Tt, P->Ts, theta, P->Ls, P->steps);
+    return P;
+}
+void orc_plan_st_destroy(void* h) { delete (PlanST*)h; }
+// which: 0 = source hierarchy, 1 = target hierarchy
+void orc_plan_st_info(void* h, int which, int* L, int64_t* n_boxes, int64_t* n_leaves, int64_t* n_weak, int64_t* n_strong, int64_t* n_p2p_pairs, int* n_steps) {
+    PlanST* P = (PlanST*)h; const Tree& T = which ? P->Tt : P->Ts;
+    *L = T.L; *n_boxes = T.level_off[T.L + 1]; *n_leaves = (int64_t)1 << (T.s * T.L);
+    *n_weak = (int64_t)P->Ls.weak_src.size(); *n_strong = (int64_t)P->Ls.strong_src.size();
+    int64_t pairs = 0;
+    const int64_t tleaf0 = P->Tt.level_off[P->Tt.L], sleaf0 = P->Ts.level_off[P->Ts.L];
+    for (int64_t t = 0; t < ((int64_t)1 << (P->Tt.s * P->Tt.L)); ++t)
+        for (int64_t e = P->Ls.strong_off[t]; e < P->Ls.strong_off[t + 1]; ++e)
+            pairs += P->Tt.box_count[tleaf0 + t] * P->Ts.box_count[sleaf0 + P->Ls.strong_src[e]];
+    *n_p2p_pairs = pairs;
+    *n_steps = (int)(P->steps.size() / 2);
+}
+void orc_plan_st_copy_tree(void* h, int which, int64_t* perm, int64_t* box_start, int64_t* box_count, double* lo, double* hi, double* ctr, double* rad) {
+    PlanST* P = (PlanST*)h; const Tree& T = which ? P->Tt : P->Ts;
+    const int64_t nb = T.level_off[T.L + 1];
+    if (perm) std::copy(T.perm.begin(), T.perm.end(), perm);
+    if (box_start) std::copy(T.box_start.begin(), T.box_start.end(), box_start);
+    if (box_count) std::copy(T.box_count.begin(), T.box_count.end(), box_count);
+    if (lo) std::copy(T.lo.begin(), T.lo.begin() + 3 * nb, lo);
+    if (hi) std::copy(T.hi.begin(), T.hi.begin() + 3 * nb, hi);
+    if (ctr) std::copy(T.ctr.begin(), T.ctr.begin() + 3 * nb, ctr);
+    if (rad) std::copy(T.rad.begin(), T.rad.begin() + nb, rad);
+}
+void orc_plan_st_copy_lists(void* h, int64_t* weak_off, int64_t* weak_src, int64_t* strong_off, int64_t* strong_src, int* steps) {
+    PlanST* P = (PlanST*)h; const Lists& Ls = P->Ls;
+    if (weak_off) std::copy(Ls.weak_off.begin(), Ls.weak_off.end(), weak_off);
+    if (weak_src) std::copy(Ls.weak_src.begin(), Ls.weak_src.end(), weak_src);
+    if (strong_off) std::copy(Ls.strong_off.begin(), Ls.strong_off.end(), strong_off);
+    if (strong_src) std::copy(Ls.strong_src.begin(), Ls.strong_src.end(), strong_src);
+    if (steps) std::copy(P->steps.begin(), P->steps.end(), steps);
+}
+void orc_evaluate_st(void* h, const double* q, double* pot, double* field) { evaluate_st(*(PlanST*)h, q, pot, field); }
+// plain definition at separate targets: u(t_i) = -(1/4pi) sum_j q_j/|t_i - s_j|, field = -grad u; zero-distance pairs skipped (S3)
+void orc_direct_st(const double* spos, const double* q, int64_t Ns, const double* tpos, int64_t Nt, double* pot, double* field) {
+    const double inv4pi = 1.0 / (4.0 * M_PI);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < Nt; ++i) {
+        double ph = 0.0, g[3] = {0, 0, 0};
+        for (int64_t j = 0; j < Ns; ++j) {
+            const double dx = tpos[3 * i] - spos[3 * j], dy = tpos[3 * i + 1] - spos[3 * j + 1], dz = tpos[3 * i + 2] - spos[3 * j + 2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 == 0.0) continue;
+            const double r = std::sqrt(r2);
+            ph += q[j] / r;
+            const double f = q[j] / (r2 * r);
+            g[0] -= f * dx; g[1] -= f * dy; g[2] -= f * dz;
+        }
+        if (pot) pot[i] = -ph * inv4pi;
+        if (field) for (int c = 0; c < 3; ++c) field[3 * i + c] = g[c] * inv4pi;
     }
 }
 int orc_num_threads() {
