@@ -77,6 +77,31 @@ fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_pot
  * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);
 
+/* Separate sources and targets: potential and field AT the Nt targets caused by charges AT the Ns sources.
+ * Two hierarchies are built with the same rules (N_max, s): one over the sources, one over the targets; source boxes are
+ * compared with target boxes by eq. (4) while marching through the levels from (l_trg, l_src) = (0, 0): 1. increase the
+ * level with the larger average box radius (mean radius of the non-empty boxes of the level); 2. if equal, the source
+ * level; 3. if one hierarchy has no more levels, the other; 4. stop when no pair is left or both are at their leaf
+ * level.  Pairs still failing there are summed directly (P2P between a target leaf and a source leaf).
+ *   d_sources : DEVICE, Ns x 3, dtype;  d_targets : DEVICE, Nt x 3, dtype.  Read only during this call.
+ *   adm       : HOST pointer or NULL (theta = 0.77); cross_level is ignored (two hierarchies are always marched).
+ * On such a plan fmm_evaluate / fmm_evaluate_host / fmm_evaluate_profiled take Ns charges (source input order) and
+ * write Nt potentials / Nt x 3 field vectors (target input order); a target that coincides with a source gets no
+ * contribution from it (reading S3).  fmm_plan_info / fmm_plan_copy_tree describe the TARGET hierarchy,
+ * fmm_plan_source_info / fmm_plan_copy_source_tree the SOURCE hierarchy; in fmm_plan_copy_lists rows are target boxes /
+ * target leaves and entries are source boxes (global ids of the source hierarchy) / source leaves. */
+fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void* d_targets, int64_t Nt, int p, int N_max, int s,
+                                   const fmm_admissibility* adm, fmm_dtype dtype, void* cuda_stream, fmm_plan** out_plan);
+
+/* Source hierarchy of a plan (HOST outputs, any may be NULL); for a plan made by fmm_plan_create it is the one hierarchy. */
+fmm_status fmm_plan_source_info(const fmm_plan* plan, int64_t* Ns, int* L, int64_t* n_boxes, int64_t* n_leaves);
+/* As fmm_plan_copy_tree, for the source hierarchy (sizes from fmm_plan_source_info). */
+fmm_status fmm_plan_copy_source_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_box_start, int32_t* h_box_count,
+                                     void* h_box_lo, void* h_box_hi, double* h_box_ctr, double* h_box_rad);
+/* The (l_trg, l_src) level pairs the level march visited, in order (plans with cross_level = 1 or separate targets;
+ * n_steps = 0 otherwise).  h_steps: 2 * n_steps int32, may be NULL to query n_steps (at most L_trg + L_src + 1). */
+fmm_status fmm_plan_copy_march(const fmm_plan* plan, int32_t* h_steps, int32_t* n_steps);
+
 /* Frees all device memory of the plan.  NULL is allowed. */
 fmm_status fmm_plan_destroy(fmm_plan* plan);
 

@@ -40,6 +40,41 @@ fmm_status guarded(F&& f) {
 
 size_t esize(fmm_dtype d) { return d == FMM_F32 ? 4 : 8; }
 
+// N, p, N_max, s, dtype -> depth and box numbering of one hierarchy (rule T1 / T2); false if the tree is too large
+bool init_shape(Plan& P, int64_t N, int p, int N_max, int s, fmm_dtype dtype, double theta) {
+    P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta;
+    P.K = (p + 1) * (p + 1);
+    P.Kp = (P.K + 3) & ~3;
+    int L = 0;  // smallest L with ceil(N / 2^(sL)) <= N_max
+    for (;; ++L) {
+        int64_t q = N;
+        for (int i = 0; i < s * L; ++i) q = (q + 1) / 2;
+        if (q <= N_max) break;
+    }
+    if ((int64_t)s * L > 30) { set_error("tree too deep: s*L > 30"); return false; }
+    P.L = L;
+    P.level_off.assign(L + 2, 0);
+    for (int l = 0; l <= L; ++l) P.level_off[l + 1] = P.level_off[l] + ((int64_t)1 << (s * l));
+    P.n_boxes = P.level_off[L + 1];
+    P.n_leaves = (int64_t)1 << (s * L);
+    if (P.n_boxes > 0x7fffff00ll) { set_error("too many boxes"); return false; }
+    return true;
+}
+
+fmm_status copy_tree_impl(const Plan& P, int32_t* h_perm, int32_t* h_box_start, int32_t* h_box_count, void* h_box_lo, void* h_box_hi,
+                          double* h_box_ctr, double* h_box_rad) {
+    const size_t es = esize(P.dtype);
+    FMM_CUDA_CHECK(cudaDeviceSynchronize());
+    if (h_perm) FMM_CUDA_CHECK(cudaMemcpy(h_perm, P.perm.p, P.N * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (h_box_start) FMM_CUDA_CHECK(cudaMemcpy(h_box_start, P.box_start.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (h_box_count) FMM_CUDA_CHECK(cudaMemcpy(h_box_count, P.box_count.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (h_box_lo) FMM_CUDA_CHECK(cudaMemcpy(h_box_lo, P.box_lo.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
+    if (h_box_hi) FMM_CUDA_CHECK(cudaMemcpy(h_box_hi, P.box_hi.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
+    if (h_box_ctr) FMM_CUDA_CHECK(cudaMemcpy(h_box_ctr, P.box_ctr.p, P.n_boxes * 3 * sizeof(double), cudaMemcpyDeviceToHost));
+    if (h_box_rad) FMM_CUDA_CHECK(cudaMemcpy(h_box_rad, P.box_rad.p, P.n_boxes * sizeof(double), cudaMemcpyDeviceToHost));
+    return FMM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -75,22 +110,8 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
-            P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta; P.cross_level = cross_level;
-            P.K = (p + 1) * (p + 1);
-            P.Kp = (P.K + 3) & ~3;
-            int L = 0;  // smallest L with ceil(N / 2^(sL)) <= N_max
-            for (;; ++L) {
-                int64_t q = N;
-                for (int i = 0; i < s * L; ++i) q = (q + 1) / 2;
-                if (q <= N_max) break;
-            }
-            if ((int64_t)s * L > 30) { set_error("tree too deep: s*L > 30"); delete h; return FMM_ERR_UNSUPPORTED; }
-            P.L = L;
-            P.level_off.assign(L + 2, 0);
-            for (int l = 0; l <= L; ++l) P.level_off[l + 1] = P.level_off[l] + ((int64_t)1 << (s * l));
-            P.n_boxes = P.level_off[L + 1];
-            P.n_leaves = (int64_t)1 << (s * L);
-            if (P.n_boxes > 0x7fffff00ll) { set_error("too many boxes"); delete h; return FMM_ERR_UNSUPPORTED; }
+            P.cross_level = cross_level;
+            if (!init_shape(P, N, p, N_max, s, dtype, theta)) { delete h; return FMM_ERR_UNSUPPORTED; }
             tables();
             cudaEvent_t e0, e1;
             FMM_CUDA_CHECK(cudaEventCreate(&e0));
@@ -118,6 +139,95 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
         *out_plan = h;
         return FMM_OK;
     });
+}
+
+fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void* d_targets, int64_t Nt, int p, int N_max, int s,
+                                   const fmm_admissibility* adm, fmm_dtype dtype, void* cuda_stream, fmm_plan** out_plan) {
+    if (out_plan) *out_plan = nullptr;
+    return guarded([&]() -> fmm_status {
+        g_err.clear();
+        if (!out_plan || !d_sources || !d_targets) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (Ns < 1 || Ns > 0x7fffff00ll || Nt < 1 || Nt > 0x7fffff00ll) { set_error("Ns and Nt must be in [1, 2^31)"); return FMM_ERR_INVALID_ARG; }
+        if (p < 0 || p > PMAX) { set_error("p must be in [0, FMM_P_MAX]"); return FMM_ERR_INVALID_ARG; }
+        if (N_max < 1 || s < 1) { set_error("N_max and s must be >= 1"); return FMM_ERR_INVALID_ARG; }
+        if (dtype != FMM_F32 && dtype != FMM_F64) { set_error("unknown dtype"); return FMM_ERR_INVALID_ARG; }
+        double theta = 0.77;
+        if (adm) {
+            theta = adm->theta;  // cross_level is ignored: two hierarchies are always marched level by level
+            if (!(theta > 0.0 && theta < 1.0)) { set_error("theta must be in (0,1)"); return FMM_ERR_INVALID_ARG; }
+        }
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+            cudaGetLastError();
+            set_error("no CUDA device: this library has no CPU fallback");
+            return FMM_ERR_CUDA;
+        }
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        fmm_plan* h = new fmm_plan();
+        Plan& P = h->P;
+        try {
+            P.cross_level = 1;
+            P.S.reset(new Plan());
+            Plan& S = *P.S;
+            S.cross_level = 1;
+            if (!init_shape(P, Nt, p, N_max, s, dtype, theta) || !init_shape(S, Ns, p, N_max, s, dtype, theta)) { delete h; return FMM_ERR_UNSUPPORTED; }
+            tables();
+            cudaEvent_t e0, e1;
+            FMM_CUDA_CHECK(cudaEventCreate(&e0));
+            FMM_CUDA_CHECK(cudaEventCreate(&e1));
+            FMM_CUDA_CHECK(cudaEventRecord(e0, st));
+            build_tree(S, d_sources, st);
+            const double sort_s = S.plan_ms[0], tree_s = S.plan_ms[1];
+            build_tree(P, d_targets, st);
+            P.plan_ms[0] += sort_s; P.plan_ms[1] += tree_s;
+            build_lists(P, st);
+            const size_t es = esize(dtype);
+            S.pq.alloc((size_t)Ns * 4 * es);
+            S.Mc.alloc((size_t)S.n_boxes * S.Kp * es);
+            FMM_CUDA_CHECK(cudaMemsetAsync(S.Mc.p, 0, S.Mc.n, st));
+            P.pq.alloc((size_t)Nt * 4 * es);
+            P.near.alloc((size_t)Nt * 4 * es);
+            P.Lc.alloc((size_t)P.n_boxes * P.Kp * es);
+            FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+            FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+            float ms = 0;
+            cudaEventElapsedTime(&ms, e0, e1);
+            P.plan_ms[3] = ms;
+            cudaEventDestroy(e0);
+            cudaEventDestroy(e1);
+        } catch (...) {
+            delete h;
+            throw;
+        }
+        *out_plan = h;
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_source_info(const fmm_plan* plan, int64_t* Ns, int* L, int64_t* n_boxes, int64_t* n_leaves) {
+    if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+    const Plan& S = plan->P.S ? *plan->P.S : plan->P;
+    if (Ns) *Ns = S.N;
+    if (L) *L = S.L;
+    if (n_boxes) *n_boxes = S.n_boxes;
+    if (n_leaves) *n_leaves = S.n_leaves;
+    return FMM_OK;
+}
+
+fmm_status fmm_plan_copy_source_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_box_start, int32_t* h_box_count, void* h_box_lo,
+                                     void* h_box_hi, double* h_box_ctr, double* h_box_rad) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        return copy_tree_impl(plan->P.S ? *plan->P.S : plan->P, h_perm, h_box_start, h_box_count, h_box_lo, h_box_hi, h_box_ctr, h_box_rad);
+    });
+}
+
+fmm_status fmm_plan_copy_march(const fmm_plan* plan, int32_t* h_steps, int32_t* n_steps) {
+    if (!plan || !n_steps) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+    const std::vector<int>& m = plan->P.march_steps;
+    *n_steps = (int32_t)(m.size() / 2);
+    if (h_steps) for (size_t i = 0; i < m.size(); ++i) h_steps[i] = m[i];
+    return FMM_OK;
 }
 
 fmm_status fmm_plan_destroy(fmm_plan* plan) {
@@ -162,9 +272,10 @@ fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* 
         Plan& P = const_cast<Plan&>(plan->P);
         const size_t es = esize(P.dtype);
         cudaStream_t st = (cudaStream_t)cuda_stream;
-        if (!P.h2d_q.p) P.h2d_q.alloc((size_t)P.N * es);
+        const int64_t Nq = P.S ? P.S->N : P.N;  // charges live on the sources
+        if (!P.h2d_q.p) P.h2d_q.alloc((size_t)Nq * es);
         if (!P.d2h_out.p) P.d2h_out.alloc((size_t)P.N * 4 * es);
-        FMM_CUDA_CHECK(cudaMemcpyAsync(P.h2d_q.p, h_charges, (size_t)P.N * es, cudaMemcpyHostToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.h2d_q.p, h_charges, (size_t)Nq * es, cudaMemcpyHostToDevice, st));
         char* dpot = h_potential ? P.d2h_out.p : nullptr;
         char* dfld = h_field ? P.d2h_out.p + (size_t)P.N * es : nullptr;
         run_evaluate(P, P.h2d_q.p, dpot, dfld, st, nullptr);
@@ -192,17 +303,7 @@ fmm_status fmm_plan_copy_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_
                               void* h_box_hi, double* h_box_ctr, double* h_box_rad) {
     return guarded([&]() -> fmm_status {
         if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
-        const Plan& P = plan->P;
-        const size_t es = esize(P.dtype);
-        FMM_CUDA_CHECK(cudaDeviceSynchronize());
-        if (h_perm) FMM_CUDA_CHECK(cudaMemcpy(h_perm, P.perm.p, P.N * sizeof(int32_t), cudaMemcpyDeviceToHost));
-        if (h_box_start) FMM_CUDA_CHECK(cudaMemcpy(h_box_start, P.box_start.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
-        if (h_box_count) FMM_CUDA_CHECK(cudaMemcpy(h_box_count, P.box_count.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost));
-        if (h_box_lo) FMM_CUDA_CHECK(cudaMemcpy(h_box_lo, P.box_lo.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
-        if (h_box_hi) FMM_CUDA_CHECK(cudaMemcpy(h_box_hi, P.box_hi.p, P.n_boxes * 3 * es, cudaMemcpyDeviceToHost));
-        if (h_box_ctr) FMM_CUDA_CHECK(cudaMemcpy(h_box_ctr, P.box_ctr.p, P.n_boxes * 3 * sizeof(double), cudaMemcpyDeviceToHost));
-        if (h_box_rad) FMM_CUDA_CHECK(cudaMemcpy(h_box_rad, P.box_rad.p, P.n_boxes * sizeof(double), cudaMemcpyDeviceToHost));
-        return FMM_OK;
+        return copy_tree_impl(plan->P, h_perm, h_box_start, h_box_count, h_box_lo, h_box_hi, h_box_ctr, h_box_rad);
     });
 }
 

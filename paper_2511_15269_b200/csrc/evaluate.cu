@@ -34,7 +34,7 @@ __global__ void permute_k(const T* __restrict__ pos_tree, const T* __restrict__ 
                           typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ src_slot, float* __restrict__ srcg, int64_t N) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    const T x = pos_tree[3 * k], y = pos_tree[3 * k + 1], z = pos_tree[3 * k + 2], qq = q[perm[k]];
+    const T x = pos_tree[3 * k], y = pos_tree[3 * k + 1], z = pos_tree[3 * k + 2], qq = q ? q[perm[k]] : T(0);  // q == nullptr: pure targets
     pq[k] = make4<T>(x, y, z, qq);
     if (srcg) {  // fp32 only: P2P source groups (-x[4], -y[4], -z[4], q[4]), see p2p_fast.cu
         const int32_t sl = src_slot[k];
@@ -390,7 +390,8 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) m2m_k(int p, int s, int6
 template <typename T>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) m2l_generic_k(int p, int64_t n_boxes, const int64_t* __restrict__ weak_off,
                                                                       const int32_t* __restrict__ weak_src, const double* __restrict__ ctr,
-                                                                      const T* __restrict__ scale, int Kp, const T* __restrict__ Mc,
+                                                                      const T* __restrict__ scale, const double* __restrict__ ctr_s,
+                                                                      const T* __restrict__ scale_s, int Kp, const T* __restrict__ Mc,
                                                                       T* __restrict__ Lc, TabPtrs tp) {
     __shared__ WarpScratch<T> wsm[WARPS_PER_BLOCK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -406,7 +407,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) m2l_generic_k(int p, int
     const T at = scale[gt];
     for (int64_t e = e0; e < e1; ++e) {
         const int64_t gs = weak_src[e];
-        translate_warp<T>(1, p, Mc + gs * Kp, ctr[3 * gs] - tx, ctr[3 * gs + 1] - ty, ctr[3 * gs + 2] - tz, scale[gs], at, wsm[w], tp, lane);
+        translate_warp<T>(1, p, Mc + gs * Kp, ctr_s[3 * gs] - tx, ctr_s[3 * gs + 1] - ty, ctr_s[3 * gs + 2] - tz, scale_s[gs], at, wsm[w], tp, lane);
 #pragma unroll
         for (int jj = 0; jj < NJMAX; ++jj) {
             const int idx = lane + 32 * jj;
@@ -447,8 +448,10 @@ constexpr int P2P_TILE = 512;
 
 template <typename T>
 __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ leaf_start,
-                                                     const int32_t* __restrict__ leaf_cnt, const int64_t* __restrict__ strong_off,
-                                                     const int32_t* __restrict__ strong_src, typename V4<T>::type* __restrict__ near) {
+                                                     const int32_t* __restrict__ leaf_cnt, const typename V4<T>::type* __restrict__ pq_s,
+                                                     const int32_t* __restrict__ sleaf_start, const int32_t* __restrict__ sleaf_cnt,
+                                                     const int64_t* __restrict__ strong_off, const int32_t* __restrict__ strong_src,
+                                                     typename V4<T>::type* __restrict__ near) {  // *_s: the sources' hierarchy (== the targets' unless PAPER.md:82)
     using T4 = typename V4<T>::type;
     __shared__ T4 sh[P2P_TILE];
     __shared__ T red[P2P_THREADS * P2P_TPT * 4];
@@ -483,9 +486,9 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
             __syncthreads();
             while (e < e1 && tile_n < P2P_TILE) {
                 const int sleaf = strong_src[e];
-                const int sst = leaf_start[sleaf], sc = leaf_cnt[sleaf];
+                const int sst = sleaf_start[sleaf], sc = sleaf_cnt[sleaf];
                 const int take = min(sc - sub, P2P_TILE - tile_n);
-                for (int i = tid; i < take; i += P2P_THREADS) sh[tile_n + i] = pq[sst + sub + i];
+                for (int i = tid; i < take; i += P2P_THREADS) sh[tile_n + i] = pq_s[sst + sub + i];
                 tile_n += take;
                 sub += take;
                 if (sub >= sc) { ++e; sub = 0; }
@@ -576,6 +579,88 @@ void ensure_streams(const Plan& Pl) {
         FMM_CUDA_CHECK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
 }
 
+// Separate sources and targets (fmm_plan_create_targets): Pl holds the targets' hierarchy, Pl.S the sources'.
+// permute + P2M + M2M run on the source hierarchy, the M2L joins the two, L2L + L2P run on the target hierarchy and the P2P sums
+// source leaves into target leaves.  Weak pairs may join any two levels, so the whole upward pass precedes the M2L; the P2P
+// still runs beside the far-field chain on its own stream.  ev != nullptr: serial, one event per stage (same order as run_t).
+template <typename T>
+void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+    using T4 = typename V4<T>::type;
+    const Plan& S = *Pl.S;
+    const Tables& tb = tables();
+    TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
+    const int p = Pl.p, s = Pl.s;
+    const bool serial = ev != nullptr || Pl.serial;
+    cudaStream_t sF = st, sN = st;
+    if (!serial) {
+        ensure_streams(Pl);
+        sF = Pl.s_far; sN = Pl.s_near;
+        FMM_CUDA_CHECK(cudaEventRecord(Pl.e_fork, st));
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(sF, Pl.e_fork, 0));
+    }
+    auto mark = [&](int i) { if (ev) FMM_CUDA_CHECK(cudaEventRecord(ev[i], st)); };
+    auto after = [&](cudaStream_t waiter, cudaStream_t producer, cudaEvent_t e) {
+        if (serial) return;
+        FMM_CUDA_CHECK(cudaEventRecord(e, producer));
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(waiter, e, 0));
+    };
+    const bool fast = Pl.m2l_variant != 1 && xlate_fast_available(p, Pl.dtype);
+    const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
+    const int64_t leaf0 = Pl.level_off[Pl.L], sleaf0 = S.level_off[S.L];
+    auto launch_p2p = [&](cudaStream_t q) {
+        if (fast_p2p) p2p_fast_launch(Pl, q);
+        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
+                                                                  S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    };
+    mark(0);
+    permute_k<T><<<nblocks(S.N, 256), 256, 0, sF>>>((const T*)S.pos_tree.p, (const T*)d_q, S.perm.p, (T4*)S.pq.p, S.src_slot.p,
+                                                    sizeof(T) == 4 ? S.srcg.p : nullptr, S.N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    permute_k<T><<<nblocks(Pl.N, 256), 256, 0, sF>>>((const T*)Pl.pos_tree.p, nullptr, Pl.perm.p, (T4*)Pl.pq.p, nullptr, nullptr, Pl.N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    after(sN, sF, Pl.e_perm);
+    if (!serial) launch_p2p(sN);
+    FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, sF));
+    mark(1);
+    dispatch_p2m_l2p<T>(S, false, nullptr, nullptr, sF);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(2);
+    if (fast && S.L > 0) FMM_CUDA_CHECK(cudaMemsetAsync(S.Mc.p, 0, (size_t)S.level_off[S.L] * S.Kp * sizeof(T), sF));
+    for (int l = S.L; l >= 1; --l) {
+        if (fast) { xlate_fast_launch(S, 0, l, sF); continue; }
+        const int64_t nbp = (int64_t)1 << (s * (l - 1));
+        m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(p, s, S.level_off[l - 1], S.level_off[l], nbp, S.box_count.p, S.box_ctr.p,
+                                                                                (const T*)S.box_scale.p, S.Kp, (T*)S.Mc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(3);
+    if (Pl.n_weak > 0) {
+        if (fast) xlate_fast_launch(Pl, 1, 0, sF, 0, Pl.n_weak);
+        else
+            m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(
+                p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, S.box_ctr.p, (const T*)S.box_scale.p, Pl.Kp,
+                (const T*)S.Mc.p, (T*)Pl.Lc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(4);
+    for (int l = 1; l <= Pl.L; ++l) {
+        if (fast) { xlate_fast_launch(Pl, 2, l, sF); continue; }
+        const int64_t nbc = (int64_t)1 << (s * l);
+        l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p, Pl.box_ctr.p,
+                                                                                (const T*)Pl.box_scale.p, Pl.Kp, (T*)Pl.Lc.p, tp);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    mark(5);
+    if (serial) launch_p2p(st);
+    else after(sF, sN, Pl.e_near);
+    mark(6);
+    dispatch_p2m_l2p<T>(Pl, true, d_pot, d_field, sF);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    mark(7);
+    after(st, sF, Pl.e_done);
+}
+
 // One evaluate.  ev == nullptr: the production schedule -- three internal streams forked from / joined to the caller's
 // stream: far chain (permute, P2M, leaf-level M2L, L2P + finalize), tree chain (M2M levels, the M2L of the upper levels, then
 // the L2L levels, all concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and L2P).
@@ -610,8 +695,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
         if (fast_p2p) p2p_fast_launch(Pl, q);
-        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p,
-                                                                  Pl.strong_src.p, (T4*)Pl.near.p);
+        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
+                                                                  Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
         FMM_CUDA_CHECK(cudaGetLastError());
     };
 
@@ -660,7 +745,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
             m2l_range(0, Pl.n_weak, sF);
         } else {
             m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(
-                p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp, (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
+                p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.Kp,
+                (const T*)Pl.Mc.p, (T*)Pl.Lc.p, tp);
         }
         FMM_CUDA_CHECK(cudaGetLastError());
     }
@@ -689,6 +775,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
 }  // namespace
 
 int64_t evaluate_launches(const Plan& P) {
+    if (P.S) return 5 + (int64_t)P.S->L + (int64_t)P.L + (P.n_weak > 0 ? 1 : 0);  // 2 permutes, P2M, P2P, L2P + M2M/L2L levels + M2L
     const bool fast = P.m2l_variant != 1 && xlate_fast_available(P.p, P.dtype);
     const int64_t w_leaf = (int64_t)P.weak_level_off.size() > P.L ? P.weak_level_off[P.L] : 0;
     int64_t m2l = P.n_weak > 0 ? 1 : 0;
@@ -707,7 +794,10 @@ void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cu
         FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
         g_const_uploaded = true;
     }
-    if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev);
+    if (P.S) {
+        if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev);
+        else run_st<double>(P, d_q, d_pot, d_field, st, ev);
+    } else if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev);
     else run_t<double>(P, d_q, d_pot, d_field, st, ev);
 }
 

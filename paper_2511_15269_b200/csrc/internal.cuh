@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <memory>
 #include <string>
 #include <vector>
 
@@ -86,6 +87,11 @@ struct Plan {
     std::vector<int64_t> weak_level_off;  // L+2: offsets of each level's pairs in the weak list
     int m2l_variant = 0;
     int max_leaf = 0;  // largest leaf population
+    // Separate sources and targets (fmm_plan_create_targets): THIS plan holds the hierarchy of the targets,
+    // the local coefficients Lc, `near` and both lists (weak: target box id here -> source box id in S; strong: target leaf ->
+    // source leaf of S); S holds the hierarchy of the sources, their permuted particles (pq, srcg) and the multipoles Mc.
+    std::unique_ptr<Plan> S;
+    std::vector<int> march_steps;  // (l_trg, l_src) pairs visited by the level march (cross_level = 1 or separate targets)
 
     DevBuf<int32_t> perm;                 // N: tree order -> input index
     DevBuf<char> pos_tree;                // N x 3 dtype, tree order

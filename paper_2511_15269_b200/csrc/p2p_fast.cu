@@ -249,10 +249,12 @@ static void p2p_launch_t(const Plan& P, cudaStream_t st) {
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
     const int64_t n_items = P.n_p2p_items * nchunk;
+    // separate targets: a target leaf may have an empty strong list and then no work item; its near field must read zero
+    if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
-    if (P.p2p_multi) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
-    p2p_fast_k<TPT, HS><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)P.srcg.p, P.src_G, P.box_start.p + leaf0, P.box_count.p + leaf0,
+    const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources (separate targets)
+    p2p_fast_k<TPT, HS><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
                                               reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
 

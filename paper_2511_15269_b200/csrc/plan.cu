@@ -312,6 +312,16 @@ void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
 
 // ---------------------------------------------------------------------------------------------- lists
 // eq. (4) PAPER.md:68-70 (rule L1): R + theta*r < theta*d, strict, IEEE fp64 without contraction.
+// (ctr_a, rad_a) / (ctr_b, rad_b): geometry arrays of the hierarchy box a / box b belongs to (the same arrays for one hierarchy)
+__device__ inline bool admissible2(const double* ctr, const double* rad, int64_t ga, const double* ctr_b, const double* rad_b, int64_t gb, double theta) {
+    const double ra = rad[ga], rb = rad_b[gb];
+    const double R = fmax(ra, rb), r = fmin(ra, rb);
+    const double dx = __dsub_rn(ctr[3 * ga], ctr_b[3 * gb]);
+    const double dy = __dsub_rn(ctr[3 * ga + 1], ctr_b[3 * gb + 1]);
+    const double dz = __dsub_rn(ctr[3 * ga + 2], ctr_b[3 * gb + 2]);
+    const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+    return __dadd_rn(R, __dmul_rn(theta, r)) < __dmul_rn(theta, d);
+}
 __device__ inline bool admissible(const double* ctr, const double* rad, int64_t ga, int64_t gb, double theta) {
     const double ra = rad[ga], rb = rad[gb];
     const double R = fmax(ra, rb), r = fmin(ra, rb);
@@ -408,11 +418,11 @@ __global__ void expand_offsets_k(ExpandArgs A, const unsigned long long* S, int6
 }
 
 // out[0] = number of particle pairs of the P2P stage, out[1] = sum over non-empty target leaves of their source particles
-__global__ void count_p2p_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_cnt, int64_t n_leaves, unsigned long long* out) {
+__global__ void count_p2p_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_cnt, const int32_t* src_cnt, int64_t n_leaves, unsigned long long* out) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long acc = 0, ssum = 0;
     if (t < n_leaves && leaf_cnt[t] > 0) {
-        for (int64_t e = soff[t]; e < soff[t + 1]; ++e) ssum += (unsigned long long)leaf_cnt[ssrc[e]];
+        for (int64_t e = soff[t]; e < soff[t + 1]; ++e) ssum += (unsigned long long)src_cnt[ssrc[e]];
         acc = ssum * (unsigned long long)leaf_cnt[t];
     }
 #pragma unroll
@@ -435,7 +445,7 @@ struct SegLoad {
     int64_t n;
     __device__ int64_t operator()(int64_t i) const { return i < n ? (int64_t)p[i] : 0; }
 };
-__global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_start, const int32_t* leaf_cnt, int64_t n_leaves, int64_t budget,
+__global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const int32_t* leaf_start, const int32_t* leaf_cnt, const int32_t* src_cnt, int64_t n_leaves, int64_t budget,
                                int32_t* nseg, const int64_t* seg_off, P2PItem* items, int* any_multi) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_leaves) return;
@@ -445,7 +455,7 @@ __global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const i
         int64_t acc = 0, e0 = soff[t];
         const int64_t eend = soff[t + 1];
         for (int64_t e = e0; e < eend; ++e) {
-            acc += leaf_cnt[ssrc[e]];
+            acc += src_cnt[ssrc[e]];
             if (acc >= budget || e + 1 == eend) {
                 if (items) items[seg_off[t] + n] = P2PItem{leaf_start[t], leaf_cnt[t], e0, total > 1 ? ~(e + 1) : e + 1};
                 ++n;
@@ -470,8 +480,10 @@ struct MarchArgs {
     int s;
     int refine_src;                 // 1: candidates (t, s * nch + c) ; 0: candidates (t * nch + c, s)
     int64_t off_t, off_s;           // global id offsets of the candidates' levels
-    const int32_t* box_count;
+    const int32_t* box_count;       // target hierarchy
     const double *ctr, *rad;
+    const int32_t* count_s;         // source hierarchy (the same arrays when sources and targets share one hierarchy)
+    const double *ctr_s, *rad_s;
     double theta;
 };
 __device__ inline void march_decode(const MarchArgs& A, int64_t idx, int32_t& t, int32_t& sc) {
@@ -488,7 +500,7 @@ __global__ void march_classify_k(MarchArgs A, uint8_t* codes) {
     march_decode(A, idx, t, sc);
     const int64_t gt = A.off_t + t, gs = A.off_s + sc;
     uint8_t code = 0;
-    if (A.box_count[gt] > 0 && A.box_count[gs] > 0) code = admissible(A.ctr, A.rad, gt, gs, A.theta) ? 1 : 2;
+    if (A.box_count[gt] > 0 && A.count_s[gs] > 0) code = admissible2(A.ctr, A.rad, gt, A.ctr_s, A.rad_s, gs, A.theta) ? 1 : 2;
     codes[idx] = code;
 }
 __global__ void march_compact_k(MarchArgs A, const uint8_t* codes, const unsigned long long* S, int32_t* wtgt, int32_t* wsrc, int32_t* ftgt2,
@@ -572,7 +584,9 @@ static void finish_lists(Plan& P, cudaStream_t st) {
     DevBuf<unsigned long long> cnt;
     cnt.alloc(2);
     FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 16, st));
-    count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], P.n_leaves, cnt.p);
+    const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources
+    const int32_t* scnt = PS.box_count.p + PS.level_off[PS.L];
+    count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], scnt, P.n_leaves, cnt.p);
     FMM_CUDA_CHECK(cudaGetLastError());
     unsigned long long h[2] = {0, 0};
     FMM_CUDA_CHECK(cudaMemcpyAsync(h, cnt.p, 16, cudaMemcpyDeviceToHost, st));
@@ -590,7 +604,7 @@ static void finish_lists(Plan& P, cudaStream_t st) {
         FMM_CUDA_CHECK(cudaMemsetAsync(any_multi.p, 0, sizeof(int32_t), st));
         seg_off.alloc(P.n_leaves + 1);
         scratch.alloc(scan_scratch_elems(P.n_leaves + 1));
-        p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, nullptr, nullptr,
+        p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, scnt, P.n_leaves, budget, nseg.p, nullptr, nullptr,
                                                                  any_multi.p);
         FMM_CUDA_CHECK(cudaGetLastError());
         exclusive_scan<int64_t>(SegLoad{nseg.p, P.n_leaves}, seg_off.p, P.n_leaves + 1, scratch.p, st);
@@ -603,32 +617,84 @@ static void finish_lists(Plan& P, cudaStream_t st) {
         P.p2p_multi = multi != 0;
         P.p2p_items.alloc((size_t)n_items * sizeof(P2PItem));
         if (n_items > 0) {
-            p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, P.n_leaves, budget, nseg.p, seg_off.p,
+            p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, scnt, P.n_leaves, budget, nseg.p, seg_off.p,
                                                                      reinterpret_cast<P2PItem*>(P.p2p_items.p), nullptr);
             FMM_CUDA_CHECK(cudaGetLastError());
         }
     }
 }
 
+// mean radius of the non-empty boxes of every level, summed in box order on the host ("average box radius";
+// the oracle sums in the same order, so the comparison of two levels takes the same decision on both sides)
+static std::vector<double> mean_radii(const Plan& P, cudaStream_t st) {
+    std::vector<double> rad(P.n_boxes);
+    std::vector<int32_t> cnt(P.n_boxes);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(rad.data(), P.box_rad.p, P.n_boxes * sizeof(double), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaMemcpyAsync(cnt.data(), P.box_count.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    std::vector<double> m(P.L + 1, 0.0);
+    for (int l = 0; l <= P.L; ++l) {
+        double sum = 0.0;
+        int64_t n = 0;
+        for (int64_t g = P.level_off[l]; g < P.level_off[l + 1]; ++g)
+            if (cnt[g] > 0) { sum += rad[g]; ++n; }
+        m[l] = n ? sum / (double)n : 0.0;
+    }
+    return m;
+}
+
+// Level marching over the target hierarchy (P) and the source hierarchy (P.S, or P itself when sources and targets share one
+// hierarchy).  One hierarchy: the fixed sequence of reading S9.  Two hierarchies: PAPER.md:85-88 -- refine the side with the
+// larger mean box radius, ties -> sources, an exhausted side -> the other.
 static void build_lists_cross(Plan& P, cudaStream_t st) {
-    const int s = P.s, L = P.L;
+    const Plan& PS = P.S ? *P.S : P;
+    const int s = P.s, L = P.L, Lsrc = PS.L;
     const int nch = 1 << s;
+    std::vector<double> mr_t, mr_s;
+    if (P.S) { mr_t = mean_radii(P, st); mr_s = mean_radii(PS, st); }
     P.weak_off.alloc(P.n_boxes + 1);
     P.weak_level_off.assign(L + 2, 0);
     DevBuf<int32_t> ftgt, fsrc;
     ftgt.alloc(1); fsrc.alloc(1);
-    FMM_CUDA_CHECK(cudaMemsetAsync(ftgt.p, 0, 4, st));  // (root, root) fails eq. (4): d = 0
+    FMM_CUDA_CHECK(cudaMemsetAsync(ftgt.p, 0, 4, st));  // (root, root) is the first candidate pair
     FMM_CUDA_CHECK(cudaMemsetAsync(fsrc.p, 0, 4, st));
     int64_t nfail = 1;
-    std::vector<DevBuf<int32_t>> wt(2 * L + 1), ws(2 * L + 1);
-    std::vector<int64_t> wn(2 * L + 1, 0);
+    std::vector<DevBuf<int32_t>> wt(L + Lsrc + 2), ws(L + Lsrc + 2);
+    std::vector<int64_t> wn(L + Lsrc + 2, 0);
     int lt = 0, ls = 0, step = 0;
     int64_t n_weak = 0;
-    while (!(lt == L && ls == L)) {
-        const int refine_src = lt == ls;  // PAPER.md:85-87 for one hierarchy: sources first, then targets
+    P.march_steps.assign({0, 0});
+    if (P.S) {
+        // the root pair itself may already be admissible when the two point sets are far apart: classify it like any other
+        // candidate by starting the march one step "before" the roots: a single candidate (0, 0) at (lt, ls) = (0, 0)
+        MarchArgs A{ftgt.p, fsrc.p, 1, 0, 1, 0, 0, P.box_count.p, P.box_ctr.p, P.box_rad.p, PS.box_count.p, PS.box_ctr.p, PS.box_rad.p, P.theta};
+        DevBuf<uint8_t> code0;
+        code0.alloc(1);
+        march_classify_k<<<1, 32, 0, st>>>(A, code0.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        uint8_t h = 0;
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&h, code0.p, 1, cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        if (h == 1) {  // one weak pair (root, root); nothing fails
+            wt[step].alloc(1); ws[step].alloc(1); wn[step] = 1;
+            FMM_CUDA_CHECK(cudaMemsetAsync(wt[step].p, 0, 4, st));
+            FMM_CUDA_CHECK(cudaMemsetAsync(ws[step].p, 0, 4, st));
+            n_weak = 1;
+            nfail = 0;
+        }
+        ++step;
+    }
+    while (!(lt == L && ls == Lsrc)) {
+        int refine_src;
+        if (!P.S) refine_src = lt == ls;  // PAPER.md:85-87 for one hierarchy: sources first, then targets
+        else if (ls == Lsrc) refine_src = 0;
+        else if (lt == L) refine_src = 1;
+        else refine_src = !(mr_t[lt] > mr_s[ls]);
         if (refine_src) ++ls; else ++lt;
+        P.march_steps.push_back(lt); P.march_steps.push_back(ls);
         const int64_t total = nfail << s;
-        MarchArgs A{ftgt.p, fsrc.p, nfail, s, refine_src, P.level_off[lt], P.level_off[ls], P.box_count.p, P.box_ctr.p, P.box_rad.p, P.theta};
+        MarchArgs A{ftgt.p, fsrc.p, nfail, s, refine_src, P.level_off[lt], PS.level_off[ls], P.box_count.p, P.box_ctr.p, P.box_rad.p,
+                    PS.box_count.p, PS.box_ctr.p, PS.box_rad.p, P.theta};
         DevBuf<uint8_t> codes;
         DevBuf<unsigned long long> S, scr;
         codes.alloc(total + 1);

@@ -45,8 +45,10 @@ struct XArgs {
     int64_t off_parent, off_child;
     int s;
     const int32_t* box_count;
-    const double* ctr;
+    const double* ctr;            // box centres / scales of the hierarchy the OUTPUT boxes belong to
     const void* scale;
+    const double* ctr_s;          // ... and of the hierarchy the INPUT boxes belong to (the same arrays unless the M2L joins
+    const void* scale_s;          //     a source hierarchy to a separate target hierarchy)
     const void* in;
     void* out;
 };
@@ -101,10 +103,11 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
     T bx = T(0), by = T(0), bz = T(1), a_old = T(1), a_new = T(1);
     if (gs >= 0) {
         const T* sc = reinterpret_cast<const T*>(a.scale);
-        bx = (T)(a.ctr[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
-        by = (T)(a.ctr[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
-        bz = (T)(a.ctr[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
-        a_old = sc[gs];
+        const T* scs = reinterpret_cast<const T*>(a.scale_s);
+        bx = (T)(a.ctr_s[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
+        by = (T)(a.ctr_s[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
+        bz = (T)(a.ctr_s[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
+        a_old = scs[gs];
         a_new = sc[gt];
     }
     mbar_wait(bar, 0);
@@ -189,8 +192,8 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
     if (P.p > 8) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }
     XArgs a{};
     a.box_count = P.box_count.p;
-    a.ctr = P.box_ctr.p;
-    a.scale = P.box_scale.p;
+    a.ctr = a.ctr_s = P.box_ctr.p;
+    a.scale = a.scale_s = P.box_scale.p;
     a.s = P.s;
     if (kind == 1) {
         if (e1 < 0) e1 = P.n_weak;
@@ -199,6 +202,7 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
         a.src = P.weak_src.p + e0;
         a.in = P.Mc.p;
         a.out = P.Lc.p;
+        if (P.S) { a.ctr_s = P.S->box_ctr.p; a.scale_s = P.S->box_scale.p; a.in = P.S->Mc.p; }  // sources in their own hierarchy
     } else {
         a.n = (int64_t)1 << (P.s * level);  // children on `level`
         a.off_parent = P.level_off[level - 1];

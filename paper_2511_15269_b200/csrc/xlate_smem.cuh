@@ -23,8 +23,10 @@ struct SArgs {
     int64_t off_parent, off_child;
     int s;
     const int32_t* box_count;
-    const double* ctr;
+    const double* ctr;            // output side (see XArgs in xlate_fast.cu)
     const void* scale;
+    const double* ctr_s;          // input side
+    const void* scale_s;
     const void* in;
     void* out;
 };
@@ -180,10 +182,11 @@ __global__ void __launch_bounds__(NT) xlate_smem_k(SArgs a) {
     __syncwarp();
     if (gs >= 0) {
         const T* sc = reinterpret_cast<const T*>(a.scale);
-        const T bx = (T)(a.ctr[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
-        const T by = (T)(a.ctr[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
-        const T bz = (T)(a.ctr[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
-        translate_blocked<T, P, KIND, LD>(wcol + lane, bx, by, bz, sc[gs], sc[gt]);
+        const T* scs = reinterpret_cast<const T*>(a.scale_s);
+        const T bx = (T)(a.ctr_s[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
+        const T by = (T)(a.ctr_s[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
+        const T bz = (T)(a.ctr_s[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
+        translate_blocked<T, P, KIND, LD>(wcol + lane, bx, by, bz, scs[gs], sc[gt]);
     }
     __syncwarp();
 
@@ -240,8 +243,8 @@ template <typename T>
 bool smem_launch_t(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     SArgs a{};
     a.box_count = P.box_count.p;
-    a.ctr = P.box_ctr.p;
-    a.scale = P.box_scale.p;
+    a.ctr = a.ctr_s = P.box_ctr.p;
+    a.scale = a.scale_s = P.box_scale.p;
     a.s = P.s;
     if (kind == 1) {
         if (e1 < 0) e1 = P.n_weak;
@@ -250,6 +253,7 @@ bool smem_launch_t(const Plan& P, int kind, int level, cudaStream_t st, int64_t 
         a.src = P.weak_src.p + e0;
         a.in = P.Mc.p;
         a.out = P.Lc.p;
+        if (P.S) { a.ctr_s = P.S->box_ctr.p; a.scale_s = P.S->box_scale.p; a.in = P.S->Mc.p; }
     } else {
         a.n = (int64_t)1 << (P.s * level);  // children on `level`
         a.off_parent = P.level_off[level - 1];

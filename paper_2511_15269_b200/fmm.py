@@ -18,7 +18,7 @@ FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
-           "fmm_version"]
+           "fmm_version", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
 
 class fmm_admissibility(C.Structure):
@@ -50,6 +50,10 @@ def lib():
         L.fmm_plan_info.argtypes = [vp, C.POINTER(C.c_int), i64p, i64p, i64p, i64p, i64p]
         L.fmm_plan_copy_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
         L.fmm_plan_copy_lists.argtypes = [vp, i64p, i32p, i64p, i32p]
+        L.fmm_plan_create_targets.argtypes = [vp, C.c_int64, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
+        L.fmm_plan_source_info.argtypes = [vp, i64p, C.POINTER(C.c_int), i64p, i64p]
+        L.fmm_plan_copy_source_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
+        L.fmm_plan_copy_march.argtypes = [vp, i32p, i32p]
         L.fmm_plan_timings.argtypes = [vp, dp]
         L.fmm_plan_set_m2l_variant.argtypes = [vp, C.c_int]
         L.fmm_plan_set_schedule.argtypes = [vp, C.c_int]
@@ -100,6 +104,48 @@ def fmm_plan_create(positions, p, N_max, s, theta=0.77, cross_level=0, stream=No
     _check(lib().fmm_plan_create(C.c_void_p(positions.data_ptr()), positions.shape[0], int(p), int(N_max), int(s), C.byref(adm),
                                  _dtype_code(positions), _stream_ptr(stream), C.byref(h)))
     return h
+
+
+def fmm_plan_create_targets(sources, targets, p, N_max, s, theta=0.77, stream=None):
+    """sources (Ns,3), targets (Nt,3): contiguous CUDA tensors of one dtype.  Returns a plan handle."""
+    for a in (sources, targets):
+        if not a.is_cuda or not a.is_contiguous() or a.dim() != 2 or a.shape[1] != 3:
+            raise ValueError("sources and targets must be contiguous CUDA tensors of shape (N,3)")
+    if sources.dtype != targets.dtype:
+        raise ValueError("sources and targets must have the same dtype")
+    adm = fmm_admissibility(float(theta), 1)
+    h = C.c_void_p()
+    _check(lib().fmm_plan_create_targets(C.c_void_p(sources.data_ptr()), sources.shape[0], C.c_void_p(targets.data_ptr()), targets.shape[0], int(p),
+                                         int(N_max), int(s), C.byref(adm), _dtype_code(sources), _stream_ptr(stream), C.byref(h)))
+    return h
+
+
+def fmm_plan_source_info(plan):
+    Ns, L, nb, nl = C.c_int64(), C.c_int(), C.c_int64(), C.c_int64()
+    _check(lib().fmm_plan_source_info(plan, C.byref(Ns), C.byref(L), C.byref(nb), C.byref(nl)))
+    return dict(N=Ns.value, L=L.value, n_boxes=nb.value, n_leaves=nl.value)
+
+
+def fmm_plan_copy_source_tree(plan, dtype):
+    info = fmm_plan_source_info(plan)
+    nb, N = info["n_boxes"], info["N"]
+    fl = np.float32 if dtype == FMM_F32 else np.float64
+    t = dict(perm=np.empty(N, np.int32), box_start=np.empty(nb, np.int32), box_count=np.empty(nb, np.int32), lo=np.empty((nb, 3), fl),
+             hi=np.empty((nb, 3), fl), ctr=np.empty((nb, 3), np.float64), rad=np.empty(nb, np.float64))
+    i32p, dp = C.POINTER(C.c_int32), C.POINTER(C.c_double)
+    _check(lib().fmm_plan_copy_source_tree(plan, t["perm"].ctypes.data_as(i32p), t["box_start"].ctypes.data_as(i32p), t["box_count"].ctypes.data_as(i32p),
+                                           C.c_void_p(t["lo"].ctypes.data), C.c_void_p(t["hi"].ctypes.data), t["ctr"].ctypes.data_as(dp),
+                                           t["rad"].ctypes.data_as(dp)))
+    return t
+
+
+def fmm_plan_copy_march(plan):
+    n = C.c_int32()
+    _check(lib().fmm_plan_copy_march(plan, None, C.byref(n)))
+    steps = np.empty(2 * n.value, np.int32)
+    if n.value:
+        _check(lib().fmm_plan_copy_march(plan, steps.ctypes.data_as(C.POINTER(C.c_int32)), C.byref(n)))
+    return steps.reshape(-1, 2)
 
 
 def fmm_plan_destroy(plan):
@@ -209,6 +255,50 @@ class Plan:
 
     def lists(self):
         return fmm_plan_copy_lists(self.handle)
+
+    def timings(self):
+        return fmm_plan_timings(self.handle)
+
+    def close(self):
+        if self.handle is not None:
+            fmm_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class PlanTargets:
+    """Separate sources and targets: potential / field at `targets` from charges at `sources`."""
+
+    def __init__(self, sources, targets, p, N_max, s, theta=0.77, stream=None):
+        self.Ns, self.Nt = sources.shape[0], targets.shape[0]
+        self.dtype = _dtype_code(sources)
+        self.tdtype = sources.dtype
+        self.device = sources.device
+        self.p, self.N_max, self.s, self.theta = p, N_max, s, theta
+        self.handle = fmm_plan_create_targets(sources, targets, p, N_max, s, theta, stream)
+        self.info = fmm_plan_info(self.handle)
+        self.source_info = fmm_plan_source_info(self.handle)
+
+    def evaluate(self, charges, want_potential=True, want_field=True, stream=None):
+        import torch
+        pot = torch.empty(self.Nt, dtype=self.tdtype, device=self.device) if want_potential else None
+        fld = torch.empty((self.Nt, 3), dtype=self.tdtype, device=self.device) if want_field else None
+        fmm_evaluate(self.handle, charges, pot, fld, stream)
+        return pot, fld
+
+    def tree(self, which):
+        """which: 'tgt' or 'src'"""
+        return fmm_plan_copy_tree(self.handle, self.Nt, self.dtype) if which == "tgt" else fmm_plan_copy_source_tree(self.handle, self.dtype)
+
+    def lists(self):
+        ls = fmm_plan_copy_lists(self.handle)
+        ls["steps"] = fmm_plan_copy_march(self.handle)
+        return ls
 
     def timings(self):
         return fmm_plan_timings(self.handle)
