@@ -297,6 +297,31 @@ def run_ours(args):
                    value=N / ms_alt / 1e3, unit=UNIT, steps=n_alt, plan_ms=Pa.timings())
         Pa.close()
 
+    # the paper's second workload: the same sources evaluated at N separate targets (uniform in the unit cube, seed 102)
+    st_line = None
+    if rank == 0 and not args.no_alt_lists:
+        tgt = np.ascontiguousarray(np.random.default_rng(102).random((N, 3)).astype(pos.dtype))
+        d_tgt = torch.from_numpy(tgt).cuda()
+        Pt = fmm.PlanTargets(d_pos, d_tgt, c["p"], c["N_max"], c["s"], c["theta"])
+        d_ut = torch.empty(N, dtype=tdt, device="cuda")
+        d_ft = torch.empty((N, 3), dtype=tdt, device="cuda")
+        n_st = min(args.steps, 50)
+        for _ in range(3):
+            flush.zero_()
+            fmm.fmm_evaluate(Pt.handle, d_q, d_ut, d_ft)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_st)]
+        for a, b in evs:
+            flush.zero_()
+            a.record()
+            fmm.fmm_evaluate(Pt.handle, d_q, d_ut, d_ft)
+            b.record()
+        torch.cuda.synchronize()
+        ms_st = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        st_line = dict(n_sources=N, n_targets=N, n_weak=Pt.info["n_weak"], n_strong=Pt.info["n_strong"], n_p2p_pairs=Pt.info["n_p2p_pairs"],
+                       ms_per_step=ms_st, value=N / ms_st / 1e3, unit="M targets/s", steps=n_st, plan_ms=Pt.timings())
+        Pt.close()
+        del d_tgt, d_ut, d_ft
+
     tmax = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -356,7 +381,7 @@ def run_ours(args):
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
                 gpu_launches=launches * args.steps, gpu_launches_per_step=launches, roofline=roofline, stages=stages, plan_ms=plan_ms,
-                alt_lists=alt, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
+                alt_lists=alt, separate_targets=st_line, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
     print(json.dumps(line), flush=True)
     P.close()
     if world > 1:
@@ -375,7 +400,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cross-level", type=int, default=0, choices=[0, 1],
                     help="interaction lists of the timed plan: 0 = same-level (paper default, PAPER.md:72-74), 1 = level marching (PAPER.md:82-89)")
-    ap.add_argument("--no-alt-lists", action="store_true", help="skip the extra measurement with the other list kind")
+    ap.add_argument("--no-alt-lists", action="store_true", help="skip the extra measurements (the other list kind; separate targets)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
