@@ -194,6 +194,20 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def aggregate_over_ranks(total_ms, e2e_ms, N, steps, world, device):
+    """Replicas: every rank evaluates its own problem of N particles; the job's time is the MAX over ranks
+    of the device time of `steps` steps (and of one end-to-end step), the job's value the particles of ALL ranks over that time.
+    Returns (ms_per_step, Mparticles/s, e2e ms per step, e2e Mparticles/s).  Needs an initialised process group if world > 1."""
+    import torch
+    import torch.distributed as dist
+    tmax = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms_max, e2e_ms_max = float(tmax[0]), float(tmax[1])
+    ms_per_step = total_ms_max / steps
+    return ms_per_step, world * N / ms_per_step / 1e3, e2e_ms_max, world * N / e2e_ms_max / 1e3
+
+
 # ---------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
@@ -322,18 +336,11 @@ def run_ours(args):
         Pt.close()
         del d_tgt, d_ut, d_ft
 
-    tmax = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max, e2e_ms_max = float(tmax[0]), float(tmax[1])
+    ms_per_step, value, e2e_ms_max, e2e_value = aggregate_over_ranks(total_ms, e2e_ms, N, args.steps, world, "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-
-    ms_per_step = total_ms_max / args.steps
-    value = world * N / ms_per_step / 1e3
-    e2e_value = world * N / e2e_ms_max / 1e3
 
     # roofline of the dominant kernel (both far-field and near-field leaders are reported under "stages")
     sm_hz = peaks["sm_max_mhz"] * 1e6
