@@ -609,6 +609,7 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     const int64_t leaf0 = Pl.level_off[Pl.L], sleaf0 = S.level_off[S.L];
     auto launch_p2p = [&](cudaStream_t q) {
         if (fast_p2p) p2p_fast_launch(Pl, q);
+        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q);
         else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
                                                                   S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
         FMM_CUDA_CHECK(cudaGetLastError());
@@ -695,6 +696,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
         if (fast_p2p) p2p_fast_launch(Pl, q);
+        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q);
         else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
                                                                   Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
         FMM_CUDA_CHECK(cudaGetLastError());

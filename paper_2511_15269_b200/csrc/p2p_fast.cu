@@ -242,6 +242,83 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
     }
 }
 
+// ---- fp64 near field: the same mapping (one target leaf, or one segment of its strong list, per warp; lanes = target groups x
+// source slices; TPT targets per lane in registers), plain scalar DFMA arithmetic.  The FP64 pipe runs at half the FP32 rate and
+// one (target, source) pair costs ~13 DFMA-class instructions plus a double-precision rsqrt (MUFU.RSQ64H + Newton steps), so a
+// source (one 32-byte (x, y, z, q) record) is simply read from `pq` through L1 -- eight lanes of a slice read the same address --
+// and no shared-memory staging is needed: 2 loads against ~90 FP64 instructions per source and lane.
+template <int TPT>
+__global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restrict__ pq, const double4* __restrict__ pq_s,
+                                                        const int32_t* __restrict__ sleaf_start, const int32_t* __restrict__ sleaf_cnt,
+                                                        const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
+                                                        double4* __restrict__ near, int64_t n_items, int nchunk) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t item = (int64_t)blockIdx.x * PW + warp;
+    if (item >= n_items) return;
+    const int64_t iw = item / nchunk;
+    const int chunk = (int)(item - iw * nchunk);
+    const P2PItem wi = items[iw];
+    const bool multi = wi.e1 < 0;
+    const int tst = wi.start, tcnt = wi.cnt;
+    const int t0 = chunk * 32 * TPT;
+    if (t0 >= tcnt) return;
+    const int tn = min(tcnt - t0, 32 * TPT);
+    const int ntg = (tn + TPT - 1) / TPT;
+    int lg = 0;
+    while ((1 << lg) < ntg) ++lg;
+    const int ntgp = 1 << lg, nsl = 32 >> lg;
+    const int tg = lane & (ntgp - 1), sl = lane >> lg;
+    double tx[TPT], ty[TPT], tz[TPT], ph[TPT], gx[TPT], gy[TPT], gz[TPT];
+#pragma unroll
+    for (int k = 0; k < TPT; ++k) {
+        const int ti = tg * TPT + k;
+        double4 v = make_double4(1e150, 1e150, 1e150, 0.0);  // unused slots are parked far away; their sums are discarded
+        if (ti < tn) v = pq[tst + t0 + ti];
+        tx[k] = v.x; ty[k] = v.y; tz[k] = v.z;
+        ph[k] = gx[k] = gy[k] = gz[k] = 0.0;
+    }
+    const int64_t e1 = multi ? ~wi.e1 : wi.e1;
+    for (int64_t e = wi.e0; e < e1; ++e) {
+        const int sleaf = strong_src[e];
+        const int sst = sleaf_start[sleaf], sc = sleaf_cnt[sleaf];
+#pragma unroll 2
+        for (int j = sl; j < sc; j += nsl) {
+            const double4 sv = pq_s[sst + j];
+#pragma unroll
+            for (int k = 0; k < TPT; ++k) {
+                const double dx = tx[k] - sv.x, dy = ty[k] - sv.y, dz = tz[k] - sv.z;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                double inv = rsqrt(r2);
+                inv = (r2 > 0.0) ? inv : 0.0;  // reading S3: self / coincident pairs contribute nothing
+                const double qi = sv.w * inv, inv2 = inv * inv;
+                const double q3 = qi * inv2;
+                ph[k] += qi;
+                gx[k] -= q3 * dx; gy[k] -= q3 * dy; gz[k] -= q3 * dz;
+            }
+        }
+    }
+    for (int d = ntgp; d < 32; d <<= 1) {
+#pragma unroll
+        for (int k = 0; k < TPT; ++k) {
+            ph[k] += __shfl_xor_sync(0xffffffffu, ph[k], d);
+            gx[k] += __shfl_xor_sync(0xffffffffu, gx[k], d);
+            gy[k] += __shfl_xor_sync(0xffffffffu, gy[k], d);
+            gz[k] += __shfl_xor_sync(0xffffffffu, gz[k], d);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < TPT; ++k) {
+        const int ti = tg * TPT + k;
+        if ((k & (nsl - 1)) == sl && ti < tn) {  // (phi_near, grad phi_near) in tree order for the L2P finalize
+            if (!multi) near[tst + t0 + ti] = make_double4(ph[k], gx[k], gy[k], gz[k]);
+            else {
+                double* o = reinterpret_cast<double*>(near + tst + t0 + ti);
+                atomicAdd(o, ph[k]); atomicAdd(o + 1, gx[k]); atomicAdd(o + 2, gy[k]); atomicAdd(o + 3, gz[k]);
+            }
+        }
+    }
+}
+
 }  // namespace
 
 template <int TPT, int HS>
@@ -286,6 +363,32 @@ void p2p_fast_launch(const Plan& P, cudaStream_t st) {
         case 6: p2p_launch_t<6, 1>(P, st); break;
         case 7: p2p_launch_t<7, 1>(P, st); break;
         default: p2p_launch_t<8, 1>(P, st); break;
+    }
+}
+
+template <int TPT>
+static void p2p_launch64_t(const Plan& P, cudaStream_t st) {
+    const Plan& PS = P.S ? *P.S : P;
+    const int64_t sleaf0 = PS.level_off[PS.L];
+    const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
+    const int64_t n_items = P.n_p2p_items * nchunk;
+    if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
+    if (n_items == 0) return;
+    const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
+    p2p_warp64_k<TPT><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
+                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+}
+
+void p2p_fast64_launch(const Plan& P, cudaStream_t st) {
+    switch (choose_tpt(P.max_leaf)) {
+        case 1: p2p_launch64_t<1>(P, st); break;
+        case 2: p2p_launch64_t<2>(P, st); break;
+        case 3: p2p_launch64_t<3>(P, st); break;
+        case 4: p2p_launch64_t<4>(P, st); break;
+        case 5: p2p_launch64_t<5>(P, st); break;
+        case 6: p2p_launch64_t<6>(P, st); break;
+        case 7: p2p_launch64_t<7>(P, st); break;
+        default: p2p_launch64_t<8>(P, st); break;
     }
 }
 
