@@ -56,15 +56,26 @@ def main():
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--quick", action="store_true", help="N <= 1e6, N_max = 128 only")
     ap.add_argument("--theta", type=float, default=0.77)
+    ap.add_argument("--sets", default="cube,sphere", help="comma list out of cube, sphere")
+    ap.add_argument("--N", default=None, help="comma list of particle counts (default 1e4..1e7)")
+    ap.add_argument("--p", default="4,8,12", help="comma list of orders")
+    ap.add_argument("--dtype", default="float32,float64", help="comma list out of float32, float64")
+    ap.add_argument("--nmax", default=None, help="comma list of N_max (default 32,128,512)")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         sys.exit("sweep needs a GPU")
     Ns = [10**4, 10**5, 10**6] + ([] if args.quick else [10**7])
     N_maxs = [128] if args.quick else [32, 128, 512]
+    if args.N:
+        Ns = [int(float(x)) for x in args.N.split(",")]
+    if args.nmax:
+        N_maxs = [int(x) for x in args.nmax.split(",")]
+    ps = [int(x) for x in args.p.split(",")]
+    dtypes = [dict(float32=np.float32, float64=np.float64)[x] for x in args.dtype.split(",")]
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
     lines = ["| set | N | dtype | p | N_max | L | weak pairs | P2P pairs | plan ms | evaluate min ms | mean ms | Mparticles/s (min) | M2L ms | P2P ms | other ms |",
              "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
-    for kind, N, dtype, p, N_max in itertools.product(["cube", "sphere"], Ns, [np.float32, np.float64], [4, 8, 12], N_maxs):
+    for kind, N, dtype, p, N_max in itertools.product(args.sets.split(","), Ns, dtypes, ps, N_maxs):
         try:
             r = run_case(kind, N, dtype, p, N_max, 3, args.theta, args.reps, flush)
         except Exception as e:  # report and go on: one failing case must not hide the others
