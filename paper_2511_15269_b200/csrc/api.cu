@@ -40,6 +40,20 @@ fmm_status guarded(F&& f) {
 
 size_t esize(fmm_dtype d) { return d == FMM_F32 ? 4 : 8; }
 
+// keep up to 8 GiB of freed blocks mapped in the device's default memory pool (see DevBuf)
+void init_pool() {
+    static bool done = false;
+    if (done) return;
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long thr = 8ull << 30;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    cudaGetLastError();
+    done = true;
+}
+
 // N, p, N_max, s, dtype -> depth and box numbering of one hierarchy (rule T1 / T2); false if the tree is too large
 bool init_shape(Plan& P, int64_t N, int p, int N_max, int s, fmm_dtype dtype, double theta) {
     P.N = N; P.p = p; P.N_max = N_max; P.s = s; P.dtype = dtype; P.theta = theta;
@@ -107,6 +121,8 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
             return FMM_ERR_CUDA;
         }
         cudaStream_t st = (cudaStream_t)cuda_stream;
+        init_pool();
+        AllocScope scope(st);
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
@@ -163,6 +179,8 @@ fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void
             return FMM_ERR_CUDA;
         }
         cudaStream_t st = (cudaStream_t)cuda_stream;
+        init_pool();
+        AllocScope scope(st);
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
@@ -231,6 +249,7 @@ fmm_status fmm_plan_copy_march(const fmm_plan* plan, int32_t* h_steps, int32_t* 
 }
 
 fmm_status fmm_plan_destroy(fmm_plan* plan) {
+    if (plan) cudaDeviceSynchronize();  // nothing of the plan may still be in flight on any stream when its memory returns to the pool
     delete plan;
     return FMM_OK;
 }
@@ -238,6 +257,7 @@ fmm_status fmm_plan_destroy(fmm_plan* plan) {
 fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream) {
     return guarded([&]() -> fmm_status {
         if (!plan || !d_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        AllocScope scope((cudaStream_t)cuda_stream);
         run_evaluate(plan->P, d_charges, d_potential, d_field, (cudaStream_t)cuda_stream, nullptr);
         return FMM_OK;
     });
@@ -250,6 +270,7 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
         cudaEvent_t ev[8];
         for (auto& e : ev) FMM_CUDA_CHECK(cudaEventCreate(&e));
         cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
         run_evaluate(plan->P, d_charges, d_potential, d_field, st, ev);
         FMM_CUDA_CHECK(cudaStreamSynchronize(st));
         for (int i = 0; i < 7; ++i) {
@@ -272,6 +293,7 @@ fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* 
         Plan& P = const_cast<Plan&>(plan->P);
         const size_t es = esize(P.dtype);
         cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
         const int64_t Nq = P.S ? P.S->N : P.N;  // charges live on the sources
         if (!P.h2d_q.p) P.h2d_q.alloc((size_t)Nq * es);
         if (!P.d2h_out.p) P.d2h_out.alloc((size_t)P.N * 4 * es);

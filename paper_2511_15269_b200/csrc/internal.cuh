@@ -30,6 +30,21 @@ struct CudaFail {
         }                                                                                                  \
     } while (0)
 
+// Device memory comes from the device's stream-ordered pool (cudaMallocAsync / cudaFreeAsync on the stream of the API call
+// that is running, see AllocScope): the many short-lived scratch buffers of a plan build are recycled inside the pool
+// instead of going through cudaMalloc / cudaFree (each of which synchronises the device), and a later plan of similar
+// size finds its memory already mapped.  Every API call that allocates ends with a stream synchronisation, so plan
+// buffers are safe to use from any stream afterwards.
+inline cudaStream_t& alloc_stream() {
+    static thread_local cudaStream_t s = nullptr;
+    return s;
+}
+struct AllocScope {
+    cudaStream_t prev;
+    explicit AllocScope(cudaStream_t st) : prev(alloc_stream()) { alloc_stream() = st; }
+    ~AllocScope() { alloc_stream() = prev; }
+};
+
 // device buffer owned by the plan
 template <typename T>
 struct DevBuf {
@@ -38,10 +53,10 @@ struct DevBuf {
     void alloc(size_t count) {
         release();
         n = count;
-        if (count) FMM_CUDA_CHECK(cudaMalloc((void**)&p, count * sizeof(T)));
+        if (count) FMM_CUDA_CHECK(cudaMallocAsync((void**)&p, count * sizeof(T), alloc_stream()));
     }
     void release() {
-        if (p) cudaFree(p);
+        if (p) cudaFreeAsync(p, alloc_stream());
         p = nullptr;
         n = 0;
     }
