@@ -311,6 +311,21 @@ def run_ours(args):
                    value=N / ms_alt / 1e3, unit=UNIT, steps=n_alt, plan_ms=Pa.timings())
         Pa.close()
 
+    # re-planning cost for changed positions (the paper pays minutes of JIT whenever positions change): wall time of
+    # plan create + destroy on the same positions with a warm memory pool, synchronised on both sides
+    replan = None
+    if rank == 0 and not args.no_alt_lists:
+        ts = []
+        for _ in range(6):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            Pr = fmm.Plan(d_pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=args.cross_level)
+            torch.cuda.synchronize()
+            ts.append((time.perf_counter() - t0) * 1e3)
+            last = Pr.timings()
+            Pr.close()
+        replan = dict(wall_ms_mean=float(np.mean(ts[1:])), wall_ms_min=float(np.min(ts[1:])), device_ms=last, n=5)
+
     # the paper's second workload: the same sources evaluated at N separate targets (uniform in the unit cube, seed 102)
     st_line = None
     if rank == 0 and not args.no_alt_lists:
@@ -388,7 +403,7 @@ def run_ours(args):
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
                 gpu_launches=launches * args.steps, gpu_launches_per_step=launches, roofline=roofline, stages=stages, plan_ms=plan_ms,
-                alt_lists=alt, separate_targets=st_line, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
+                alt_lists=alt, separate_targets=st_line, replan=replan, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
     print(json.dumps(line), flush=True)
     P.close()
     if world > 1:
