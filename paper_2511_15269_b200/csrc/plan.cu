@@ -596,7 +596,14 @@ static void finish_lists(Plan& P, cudaStream_t st) {
         // work items of the P2P kernel: budget = twice the mean number of source particles per target leaf (at least 1024)
         const int32_t* lcnt = P.box_count.p + P.level_off[L];
         const int64_t mean_src = (int64_t)(h[1] / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
-        const int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
+        int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
+        // small problems: fewer target leaves than the chip has warp slots -- cut the lists finer (down to 128 source particles
+        // per item) so that about 8 warps per SM find work; the partial sums of a leaf are then combined with atomics
+        const int64_t want_items = 148 * 8;
+        if (P.n_leaves < want_items) {
+            const int64_t fine = (int64_t)(h[1] / (unsigned long long)want_items);
+            budget = std::min(budget, std::max<int64_t>(128, fine));
+        }
         DevBuf<int32_t> nseg, any_multi;
         DevBuf<int64_t> seg_off, scratch;
         nseg.alloc(P.n_leaves);
