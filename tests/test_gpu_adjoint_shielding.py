@@ -4,7 +4,9 @@ The potential at targets t_i from charges at sources s_j is linear in q, phi = A
 vector-Jacobian product the paper obtains by JAX autodiff is q_bar = A^T phi_bar: the SAME kernel with the roles of sources and
 targets exchanged.  On the device that is one more plan, fmm_plan_create_targets(sources = t, targets = s), evaluated on phi_bar.
 It is the exact adjoint of the definition and agrees with the transpose of the forward FMM operator to truncation error (checked
-below by the dot-product identity); the adjoint of the field output (dipole sources) is not built.
+below by the dot-product identity).  The cotangent of the FIELD output needs no new kernel either: field = -grad_t u, so
+q_bar_j = sum_i f_bar_i . d field_i / d q_j = - sum_c [field component c, at s_j, of charges f_bar_c placed at the targets]: three
+more evaluates of the role-swapped plan, one per component (test_field_adjoint_dot_product_identity).
 The demo itself: 128 shield charges on a sphere of radius 2 are optimised by gradient descent so that the potential of
 256 random external charges (radius 5) has minimal variance on 1024 points at radius 1.5, while the shield's own potential at
 1024 points at radius 2.5 stays small (eqs. (16)-(19), w_in = 1, w_out = 0.2, w_reg = 0.1)."""
@@ -44,6 +46,19 @@ class Op:
         u, _ = self.adj.evaluate(torch.from_numpy(np.ascontiguousarray(g)).cuda(), want_field=False)
         return u.cpu().numpy()
 
+    def F(self, q):
+        """field at tgt, (Nt, 3)"""
+        _, f = self.fwd.evaluate(torch.from_numpy(np.ascontiguousarray(q)).cuda(), want_potential=False)
+        return f.cpu().numpy()
+
+    def FT(self, fbar):
+        """adjoint of F: q_bar = -sum_c field_c of the charges fbar[:, c] at the targets, evaluated at the sources"""
+        out = np.zeros(self.adj.Nt)
+        for c in range(3):
+            _, f = self.adj.evaluate(torch.from_numpy(np.ascontiguousarray(fbar[:, c])).cuda(), want_potential=False)
+            out -= f.cpu().numpy()[:, c]
+        return out
+
 
 def test_adjoint_dot_product_identity():
     rng = np.random.default_rng(80)
@@ -61,6 +76,25 @@ def test_adjoint_dot_product_identity():
     want, _ = O.direct_st(tgt, g, src)
     got = op.AT(g)
     assert np.linalg.norm(got - want) / np.linalg.norm(want) < 1e-4
+
+
+def test_field_adjoint_dot_product_identity():
+    rng = np.random.default_rng(82)
+    src = rng.random((2500, 3))
+    tgt = rng.random((1800, 3)) * 1.6 - 0.3
+    q, fbar = rng.uniform(-1, 1, 2500), rng.uniform(-1, 1, (1800, 3))
+    op = Op(src, tgt, p=10)
+    _, fd = O.direct_st(src, q, tgt)
+    exact = float(np.sum(fbar * fd))
+    scale = np.linalg.norm(fbar) * np.linalg.norm(fd)
+    lhs, rhs = float(np.sum(fbar * op.F(q))), float(op.FT(fbar) @ q)
+    assert abs(lhs - exact) < 5e-4 * scale and abs(rhs - exact) < 5e-4 * scale and abs(lhs - rhs) < 5e-4 * scale
+    # against the plain definition of the transposed field operator: q_bar_j = -(1/4pi) sum_i fbar_i . (t_i - s_j) / |t_i - s_j|^3
+    d = tgt[:, None, :] - src[None, :, :]
+    r3 = np.linalg.norm(d, axis=2) ** 3
+    want = -(np.einsum("ic,ijc->ij", fbar, d) / r3).sum(axis=0) / (4 * np.pi)
+    got = op.FT(fbar)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < 1e-3
 
 
 def test_active_shielding_demo():
