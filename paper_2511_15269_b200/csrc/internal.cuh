@@ -169,7 +169,7 @@ void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1); 
 bool m2l_stream_available(int p, fmm_dtype dt);
 void m2l_stream_launch(const Plan& P, cudaStream_t st, int64_t b0, int64_t b1);
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
-void p2p_fast_launch(const Plan& P, cudaStream_t st);
-void p2p_fast64_launch(const Plan& P, cudaStream_t st);  // fp64: same mapping, scalar DFMA arithmetic, sources read through L1
+void p2p_fast_launch(const Plan& P, cudaStream_t st, bool want_field);  // want_field = false: potential only (cheaper inner loop)
+void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field);  // fp64: same mapping, scalar DFMA arithmetic, sources read through L1
 
 }  // namespace fmm

@@ -56,7 +56,8 @@ constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two
 
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
 // the leaf population hold zeros (zero charge), so whole groups can be used without masks.
-template <int TPT, int HS>
+// WF = false: potential only (fmm_evaluate with d_field == NULL): 7 instead of 13 packed instructions per two pairs
+template <int TPT, int HS, bool WF>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
                                                       const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
@@ -197,12 +198,16 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                     const float ja = a >= 1.17549435e-38f ? ia[c] : 0.f;
                     const float jb = b2 >= 1.17549435e-38f ? ib[c] : 0.f;
                     const u64 inv = pk(ja, jb);
-                    const u64 qi = mul2(sq, inv), inv2 = mul2(inv, inv);
-                    const u64 q3 = mul2(qi, inv2);
-                    PH[k] = add2(PH[k], qi);
-                    GX[k] = fma2(q3, dx[c], GX[k]);
-                    GY[k] = fma2(q3, dy[c], GY[k]);
-                    GZ[k] = fma2(q3, dz[c], GZ[k]);
+                    if constexpr (WF) {
+                        const u64 qi = mul2(sq, inv), inv2 = mul2(inv, inv);
+                        const u64 q3 = mul2(qi, inv2);
+                        PH[k] = add2(PH[k], qi);
+                        GX[k] = fma2(q3, dx[c], GX[k]);
+                        GY[k] = fma2(q3, dy[c], GY[k]);
+                        GZ[k] = fma2(q3, dz[c], GZ[k]);
+                    } else {
+                        PH[k] = fma2(sq, inv, PH[k]);
+                    }
                 }
             }
         }
@@ -222,9 +227,11 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
 #pragma unroll
         for (int k = 0; k < TPT; ++k) {
             ph[k] += __shfl_xor_sync(0xffffffffu, ph[k], d);
-            gx[k] += __shfl_xor_sync(0xffffffffu, gx[k], d);
-            gy[k] += __shfl_xor_sync(0xffffffffu, gy[k], d);
-            gz[k] += __shfl_xor_sync(0xffffffffu, gz[k], d);
+            if constexpr (WF) {
+                gx[k] += __shfl_xor_sync(0xffffffffu, gx[k], d);
+                gy[k] += __shfl_xor_sync(0xffffffffu, gy[k], d);
+                gz[k] += __shfl_xor_sync(0xffffffffu, gz[k], d);
+            }
         }
     }
     // every lane now holds the full sums of its group; slice sl writes the targets k with k mod nsl == sl
@@ -236,7 +243,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
             if (!multi) near[tst + t0 + ti] = make_float4(ph[k], -gx[k], -gy[k], -gz[k]);
             else {  // several segments per leaf: `near` was zeroed by run_evaluate
                 float* o = reinterpret_cast<float*>(near + tst + t0 + ti);
-                atomicAdd(o, ph[k]); atomicAdd(o + 1, -gx[k]); atomicAdd(o + 2, -gy[k]); atomicAdd(o + 3, -gz[k]);
+                atomicAdd(o, ph[k]);
+                if constexpr (WF) { atomicAdd(o + 1, -gx[k]); atomicAdd(o + 2, -gy[k]); atomicAdd(o + 3, -gz[k]); }
             }
         }
     }
@@ -247,7 +255,7 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
 // one (target, source) pair costs ~13 DFMA-class instructions plus a double-precision rsqrt (MUFU.RSQ64H + Newton steps), so a
 // source (one 32-byte (x, y, z, q) record) is simply read from `pq` through L1 -- eight lanes of a slice read the same address --
 // and no shared-memory staging is needed: 2 loads against ~90 FP64 instructions per source and lane.
-template <int TPT>
+template <int TPT, bool WF>
 __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restrict__ pq, const double4* __restrict__ pq_s,
                                                         const int32_t* __restrict__ sleaf_start, const int32_t* __restrict__ sleaf_cnt,
                                                         const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
@@ -290,10 +298,12 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
                 const double r2 = dx * dx + dy * dy + dz * dz;
                 double inv = rsqrt(r2);
                 inv = (r2 > 0.0) ? inv : 0.0;  // reading S3: self / coincident pairs contribute nothing
-                const double qi = sv.w * inv, inv2 = inv * inv;
-                const double q3 = qi * inv2;
+                const double qi = sv.w * inv;
                 ph[k] += qi;
-                gx[k] -= q3 * dx; gy[k] -= q3 * dy; gz[k] -= q3 * dz;
+                if constexpr (WF) {
+                    const double q3 = qi * (inv * inv);
+                    gx[k] -= q3 * dx; gy[k] -= q3 * dy; gz[k] -= q3 * dz;
+                }
             }
         }
     }
@@ -301,9 +311,11 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
 #pragma unroll
         for (int k = 0; k < TPT; ++k) {
             ph[k] += __shfl_xor_sync(0xffffffffu, ph[k], d);
-            gx[k] += __shfl_xor_sync(0xffffffffu, gx[k], d);
-            gy[k] += __shfl_xor_sync(0xffffffffu, gy[k], d);
-            gz[k] += __shfl_xor_sync(0xffffffffu, gz[k], d);
+            if constexpr (WF) {
+                gx[k] += __shfl_xor_sync(0xffffffffu, gx[k], d);
+                gy[k] += __shfl_xor_sync(0xffffffffu, gy[k], d);
+                gz[k] += __shfl_xor_sync(0xffffffffu, gz[k], d);
+            }
         }
     }
 #pragma unroll
@@ -313,7 +325,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
             if (!multi) near[tst + t0 + ti] = make_double4(ph[k], gx[k], gy[k], gz[k]);
             else {
                 double* o = reinterpret_cast<double*>(near + tst + t0 + ti);
-                atomicAdd(o, ph[k]); atomicAdd(o + 1, gx[k]); atomicAdd(o + 2, gy[k]); atomicAdd(o + 3, gz[k]);
+                atomicAdd(o, ph[k]);
+                if constexpr (WF) { atomicAdd(o + 1, gx[k]); atomicAdd(o + 2, gy[k]); atomicAdd(o + 3, gz[k]); }
             }
         }
     }
@@ -322,7 +335,7 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
 }  // namespace
 
 template <int TPT, int HS>
-static void p2p_launch_t(const Plan& P, cudaStream_t st) {
+static void p2p_launch_t(const Plan& P, cudaStream_t st, bool wf) {
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
     const int64_t n_items = P.n_p2p_items * nchunk;
@@ -331,7 +344,9 @@ static void p2p_launch_t(const Plan& P, cudaStream_t st) {
     if (n_items == 0) return;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources (separate targets)
-    p2p_fast_k<TPT, HS><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+    if (wf) p2p_fast_k<TPT, HS, true><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
+    else p2p_fast_k<TPT, HS, false><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
                                               reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
 }
 
@@ -353,21 +368,21 @@ static int choose_tpt(int max_leaf) {
     return best;
 }
 
-void p2p_fast_launch(const Plan& P, cudaStream_t st) {
+void p2p_fast_launch(const Plan& P, cudaStream_t st, bool wf) {
     switch (choose_tpt(P.max_leaf)) {
-        case 1: p2p_launch_t<1, 2>(P, st); break;
-        case 2: p2p_launch_t<2, 2>(P, st); break;
-        case 3: p2p_launch_t<3, 2>(P, st); break;
-        case 4: p2p_launch_t<4, 2>(P, st); break;
-        case 5: p2p_launch_t<5, 1>(P, st); break;
-        case 6: p2p_launch_t<6, 1>(P, st); break;
-        case 7: p2p_launch_t<7, 1>(P, st); break;
-        default: p2p_launch_t<8, 1>(P, st); break;
+        case 1: p2p_launch_t<1, 2>(P, st, wf); break;
+        case 2: p2p_launch_t<2, 2>(P, st, wf); break;
+        case 3: p2p_launch_t<3, 2>(P, st, wf); break;
+        case 4: p2p_launch_t<4, 2>(P, st, wf); break;
+        case 5: p2p_launch_t<5, 1>(P, st, wf); break;
+        case 6: p2p_launch_t<6, 1>(P, st, wf); break;
+        case 7: p2p_launch_t<7, 1>(P, st, wf); break;
+        default: p2p_launch_t<8, 1>(P, st, wf); break;
     }
 }
 
 template <int TPT>
-static void p2p_launch64_t(const Plan& P, cudaStream_t st) {
+static void p2p_launch64_t(const Plan& P, cudaStream_t st, bool wf) {
     const Plan& PS = P.S ? *P.S : P;
     const int64_t sleaf0 = PS.level_off[PS.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
@@ -375,20 +390,22 @@ static void p2p_launch64_t(const Plan& P, cudaStream_t st) {
     if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
-    p2p_warp64_k<TPT><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
+    if (wf) p2p_warp64_k<TPT, true><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
+                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+    else p2p_warp64_k<TPT, false><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
                                                 reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
 }
 
-void p2p_fast64_launch(const Plan& P, cudaStream_t st) {
+void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool wf) {
     switch (choose_tpt(P.max_leaf)) {
-        case 1: p2p_launch64_t<1>(P, st); break;
-        case 2: p2p_launch64_t<2>(P, st); break;
-        case 3: p2p_launch64_t<3>(P, st); break;
-        case 4: p2p_launch64_t<4>(P, st); break;
-        case 5: p2p_launch64_t<5>(P, st); break;
-        case 6: p2p_launch64_t<6>(P, st); break;
-        case 7: p2p_launch64_t<7>(P, st); break;
-        default: p2p_launch64_t<8>(P, st); break;
+        case 1: p2p_launch64_t<1>(P, st, wf); break;
+        case 2: p2p_launch64_t<2>(P, st, wf); break;
+        case 3: p2p_launch64_t<3>(P, st, wf); break;
+        case 4: p2p_launch64_t<4>(P, st, wf); break;
+        case 5: p2p_launch64_t<5>(P, st, wf); break;
+        case 6: p2p_launch64_t<6>(P, st, wf); break;
+        case 7: p2p_launch64_t<7>(P, st, wf); break;
+        default: p2p_launch64_t<8>(P, st, wf); break;
     }
 }
 
