@@ -118,6 +118,8 @@ struct Plan {
     DevBuf<int32_t> weak_src, weak_tgt;   // n_weak (global ids)
     DevBuf<int64_t> strong_off;           // n_leaves+1
     DevBuf<int32_t> strong_src;           // n_strong (leaf indices)
+    DevBuf<uint8_t> strong_touch;         // n_strong: 1 if the tight boxes of target and source leaf touch or overlap, i.e. a zero
+                                          // distance is possible (the leaf itself; leaves sharing duplicated points): only those need the S3 mask
     // evaluate scratch
     DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)

@@ -16,6 +16,8 @@
 //     sm_100): 13 packed instructions + 2 MUFU.RSQ + 2 (FSETP+FSEL) per two particle pairs.  The FMA pipe issues a packed
 //     instruction every other cycle, which leaves the issue slots in between for MUFU, the mask, LDS and the loop;
 //   * slices are combined with warp shuffles (no block-level synchronisation anywhere in the kernel).
+#include <type_traits>
+
 #include "internal.cuh"
 #include "tma.cuh"
 
@@ -57,11 +59,13 @@ constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
 // the leaf population hold zeros (zero charge), so whole groups can be used without masks.
 // WF = false: potential only (fmm_evaluate with d_field == NULL): 7 instead of 13 packed instructions per two pairs
-template <int TPT, int HS, bool WF>
+// ZT = true: tiles without a touching leaf pair skip the zero-distance mask (pays for leaves of >~ 32 particles; with small
+// leaves every tile holds the target leaf itself)
+template <int TPT, int HS, bool WF, bool ZT>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
                                                       const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
-                                                      float4* __restrict__ near, int64_t n_items, int nchunk) {
+                                                      const uint8_t* __restrict__ strong_touch, float4* __restrict__ near, int64_t n_items, int nchunk) {
     __shared__ __align__(128) float sm[PW][2][TG * 16];
     __shared__ __align__(8) unsigned long long bars[PW][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -107,9 +111,12 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
     int sub = 0;  // groups of entry e already consumed
 
     // producer: fill tile `b` with up to TG groups starting at the cursor (e, sub); every lane issues the bulk copy of "its" entry
-    auto produce = [&](int b) -> int {
+    // zf: set if an entry copied into the tile may hold a source at zero distance from a target (strong_touch): only such
+    // tiles run the masked loop (reading S3); pad slots are parked far away by the plan and never coincide with anything
+    auto produce = [&](int b, bool& zf) -> int {
         int fill = 0;
         uint32_t bytes = 0;
+        zf = false;
         const uint32_t bar = bar0 + 8 * b, buf = buf0 + (uint32_t)b * (TG * 64);
         while (e < e1 && fill < TG) {
             const int nb = (int)min((int64_t)32, e1 - e);
@@ -134,6 +141,7 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                 bulk_g2s(buf + (uint32_t)(fill + excl) * 64u, srcg + g0 * 16, (uint32_t)ni * 64u, bar);
                 bytes += (uint32_t)ni * 64u;
             }
+            if constexpr (ZT) zf |= __any_sync(0xffffffffu, ni > 0 && strong_touch[e + lane] != 0);
             const int total = __shfl_sync(0xffffffffu, incl, 31);
             if (total <= room) {
                 fill += total;
@@ -154,14 +162,18 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
         return fill;
     };
 
-    int ng_next = (e < e1) ? produce(0) : 0;
+    bool zf_next = false;
+    int ng_next = (e < e1) ? produce(0, zf_next) : 0;
     for (int t = 0; ng_next > 0; ++t) {
         const int b = t & 1;
         const int ng = ng_next;
+        const bool zf = zf_next;
         __syncwarp();  // every lane has finished reading the other buffer (tile t-1)
-        ng_next = (e < e1) ? produce(b ^ 1) : 0;
+        ng_next = (e < e1) ? produce(b ^ 1, zf_next) : 0;
         mbar_wait(bar0 + 8 * b, (t >> 1) & 1);
         const ulonglong2* T2 = reinterpret_cast<const ulonglong2*>(&sm[warp][b][0]);
+        auto run_tile = [&](auto mkc) {
+        constexpr bool MK = decltype(mkc)::value;
         for (int j = sl; j < ng; j += nsl) {
             const ulonglong2 xs = T2[4 * j], ys = T2[4 * j + 1], zs = T2[4 * j + 2], qs = T2[4 * j + 3];
             // staged over the NC = HS * TPT independent chains (all distances, then all rsqrt, then the accumulation) so that
@@ -195,8 +207,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                     float a, b2;
                     upk(r2[c], a, b2);
                     // reading S3: coincident pairs contribute nothing (r^2 below FLT_MIN counts as coincident in fp32)
-                    const float ja = a >= 1.17549435e-38f ? ia[c] : 0.f;
-                    const float jb = b2 >= 1.17549435e-38f ? ib[c] : 0.f;
+                    const float ja = (!MK || a >= 1.17549435e-38f) ? ia[c] : 0.f;
+                    const float jb = (!MK || b2 >= 1.17549435e-38f) ? ib[c] : 0.f;
                     const u64 inv = pk(ja, jb);
                     if constexpr (WF) {
                         const u64 qi = mul2(sq, inv), inv2 = mul2(inv, inv);
@@ -211,6 +223,9 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
                 }
             }
         }
+        };
+        if (!ZT || zf) run_tile(std::true_type{});
+        else run_tile(std::false_type{});
     }
 
     // combine the two packed halves, then the source slices (lanes that differ in the bits above lg)
@@ -344,10 +359,10 @@ static void p2p_launch_t(const Plan& P, cudaStream_t st, bool wf) {
     if (n_items == 0) return;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources (separate targets)
-    if (wf) p2p_fast_k<TPT, HS, true><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
-    else p2p_fast_k<TPT, HS, false><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (float4*)P.near.p, n_items, nchunk);
+    if (wf) p2p_fast_k<TPT, HS, true, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+    else p2p_fast_k<TPT, HS, false, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
 }
 
 // Targets per lane.  A median-split tree gives every leaf the same population (+-1), so max_leaf decides the lane layout for

@@ -177,6 +177,10 @@ __global__ void gather_pos_k(const T* pos, const int32_t* perm, T* pos_tree, int
 }
 
 // P2P source-group slots (fp32): particle i of leaf l -> 4 * (l * G + i / 4) + (i & 3); one warp per leaf
+__global__ void srcg_init_k(float* srcg, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) srcg[i] = (i & 15) < 12 ? 1e18f : 0.f;  // group = (-x[4], -y[4], -z[4], q[4])
+}
 __global__ void src_slot_k(const int32_t* leaf_start, const int32_t* leaf_cnt, int64_t n_leaves, int G, int32_t* slot) {
     const int64_t leaf = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     if (leaf >= n_leaves) return;
@@ -292,7 +296,10 @@ void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
         }
         P.src_slot.alloc(N);
         P.srcg.alloc((size_t)n_leaves * P.src_G * 16);
-        FMM_CUDA_CHECK(cudaMemsetAsync(P.srcg.p, 0, P.srcg.n * sizeof(float), st));  // pad slots: zero charge, finite position
+        // pad slots: zero charge, parked at x = y = z = -1e18 (stored negated), far from every real particle and from the parked
+        // target slots at +1e18, so that their distance is never zero and no mask is needed for them
+        srcg_init_k<<<nblocks((int64_t)P.srcg.n, 256), 256, 0, st>>>(P.srcg.p, (int64_t)P.srcg.n);
+        FMM_CUDA_CHECK(cudaGetLastError());
         src_slot_k<<<nblocks(n_leaves * 32, 128), 128, 0, st>>>(P.box_start.p + P.level_off[P.L], P.box_count.p + P.level_off[P.L], n_leaves,
                                                                P.src_G, P.src_slot.p);
         FMM_CUDA_CHECK(cudaGetLastError());
@@ -415,6 +422,20 @@ __global__ void expand_offsets_k(ExpandArgs A, const unsigned long long* S, int6
     const unsigned long long sv = S[base];
     weak_off_global[A.off_child + t] = weak_base + (int64_t)(sv & 0xffffffffull);
     foff2[t] = (int64_t)(sv >> 32);
+}
+
+// strong_touch[e] = 1 iff the tight bounding boxes of the target leaf and the source leaf of entry e touch or overlap (exact
+// comparisons in the plan's dtype): only then can a target coincide with a source (reading S3)
+template <typename T>
+__global__ void strong_touch_k(const int64_t* soff, const int32_t* ssrc, const T* tlo, const T* thi, const T* slo, const T* shi, int64_t n_leaves, uint8_t* touch) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_leaves) return;
+    const T a0 = tlo[3 * t], a1 = tlo[3 * t + 1], a2 = tlo[3 * t + 2], b0 = thi[3 * t], b1 = thi[3 * t + 1], b2 = thi[3 * t + 2];
+    for (int64_t e = soff[t]; e < soff[t + 1]; ++e) {
+        const int64_t s = ssrc[e];
+        const bool hit = a0 <= shi[3 * s] && slo[3 * s] <= b0 && a1 <= shi[3 * s + 1] && slo[3 * s + 1] <= b1 && a2 <= shi[3 * s + 2] && slo[3 * s + 2] <= b2;
+        touch[e] = hit ? 1 : 0;
+    }
 }
 
 // out[0] = number of particle pairs of the P2P stage, out[1] = sum over non-empty target leaves of their source particles
@@ -586,6 +607,17 @@ static void finish_lists(Plan& P, cudaStream_t st) {
     FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, 16, st));
     const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources
     const int32_t* scnt = PS.box_count.p + PS.level_off[PS.L];
+    P.strong_touch.alloc(P.n_strong);
+    if (P.n_strong > 0) {
+        const size_t to = (size_t)P.level_off[L] * 3, so = (size_t)PS.level_off[PS.L] * 3;
+        if (P.dtype == FMM_F32)
+            strong_touch_k<float><<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, (const float*)P.box_lo.p + to, (const float*)P.box_hi.p + to,
+                                                                            (const float*)PS.box_lo.p + so, (const float*)PS.box_hi.p + so, P.n_leaves, P.strong_touch.p);
+        else
+            strong_touch_k<double><<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, (const double*)P.box_lo.p + to, (const double*)P.box_hi.p + to,
+                                                                             (const double*)PS.box_lo.p + so, (const double*)PS.box_hi.p + so, P.n_leaves, P.strong_touch.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
     count_p2p_k<<<nblocks(P.n_leaves, 256), 256, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_count.p + P.level_off[L], scnt, P.n_leaves, cnt.p);
     FMM_CUDA_CHECK(cudaGetLastError());
     unsigned long long h[2] = {0, 0};
