@@ -142,7 +142,9 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
  * for (p, dtype), else the generic kernels), 1 = force the generic kernels (any p <= FMM_P_MAX, both dtypes; used by the
  * tests to cross-check), 2 = as 0 but M2L by the two-pairs-per-thread packed-f32x2 kernel (m2l_packed.cu), 3 = as 0 but M2L by
  * the software-pipelined kernel over target-aligned batches (m2l_stream.cu; the batch copy of the weak list is built on the
- * first evaluate).  0 is the fastest measured on B200; 2 and 3 are kept as measured alternatives. */
+ * first evaluate).  0 is the fastest measured on B200; 2 and 3 are kept as measured alternatives.
+ * "Register translation kernels" covers p <= 8 (state in registers) and 9 <= p <= 12 (state in shared memory), fp32 and fp64;
+ * 2 and 3 exist for fp32, p <= 8, single-hierarchy plans only and fall back to 0 elsewhere (separate-targets plans included). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
 /* Schedule of subsequent fmm_evaluate / fmm_evaluate_host calls on this plan.  0 (default) = concurrent: the call forks
