@@ -265,6 +265,18 @@ __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__
     }
 }
 
+// 1/sqrt(x) for normal, finite x > 0 (squared distances): the hardware seed (MUFU.RSQ64H, relative error ~2^-22) refined by one
+// third-order step  y = y0 + y0 e (1/2 + 3/8 e),  e = 1 - x y0^2  (error ~ (5/16) e^3 < 2^-66): 5 DFMA-class instructions instead
+// of the library rsqrt's range checks and two Newton steps.  x = 0 gives NaN, which the caller selects away.
+__device__ __forceinline__ double drsqrt(double x) {
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    const double t = x * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(y0 * e, p, y0);
+}
+
 // ---- fp64 near field: the same mapping (one target leaf, or one segment of its strong list, per warp; lanes = target groups x
 // source slices; TPT targets per lane in registers), plain scalar DFMA arithmetic.  The FP64 pipe runs at half the FP32 rate and
 // one (target, source) pair costs ~13 DFMA-class instructions plus a double-precision rsqrt (MUFU.RSQ64H + Newton steps), so a
@@ -311,8 +323,8 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
             for (int k = 0; k < TPT; ++k) {
                 const double dx = tx[k] - sv.x, dy = ty[k] - sv.y, dz = tz[k] - sv.z;
                 const double r2 = dx * dx + dy * dy + dz * dz;
-                double inv = rsqrt(r2);
-                inv = (r2 > 0.0) ? inv : 0.0;  // reading S3: self / coincident pairs contribute nothing
+                double inv = drsqrt(r2);
+                inv = (r2 > 0.0) ? inv : 0.0;  // reading S3: self / coincident pairs contribute nothing (selects away the NaN of r2 = 0)
                 const double qi = sv.w * inv;
                 ph[k] += qi;
                 if constexpr (WF) {
