@@ -288,11 +288,11 @@ def test_non_finite_positions_are_rejected():
 
 
 # ------------------------------------------------------------------------------------------- full-size configs (sampled oracle)
-def sampled_case(name, n_sample_leaves=12, seed=0, cross_level=0):
+def sampled_case(name, n_sample_leaves=12, seed=0, cross_level=0, workload=None):
     """BASELINE full-size configs in the configuration bench.py times: hierarchy/lists bit-exact on everything;
     potential/field compared on the particles of a random sample of leaves (the oracle computes exactly those,
     with the same arithmetic as a full run) and against the O(N^2) definition on the same particles."""
-    pos, q, c = inputs.make(name)
+    pos, q, c = inputs.make(name) if workload is None else workload
     dt = pos.dtype.type
     P = gpu_plan(pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=cross_level)
     Po = O.Plan(pos, c["p"], c["N_max"], c["s"], c["theta"], cross_level=cross_level)
@@ -338,3 +338,10 @@ def test_config3_full_size_sampled(name):
 
 def test_config4_full_size_sampled():
     sampled_case("cfg4_film_f32", n_sample_leaves=24)
+
+
+def test_config5_ten_million_sampled():
+    """Largest N of BASELINE config 5 (N = 1e7, uniform cube, fp32, p = 8, N_max = 128, s = 3): 2.4e5 leaves, 5.6e7 weak pairs --
+    hierarchy and both lists bit-exact, potential/field on the particles of 4 sampled leaves."""
+    pos, q = inputs.uniform_cube(10**7, 57, np.float32)
+    sampled_case("cfg5_cube1e7_f32", n_sample_leaves=4, workload=(pos, q, dict(p=8, N_max=128, s=3, theta=0.77)))
