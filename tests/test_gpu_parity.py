@@ -345,3 +345,18 @@ def test_config5_ten_million_sampled():
     hierarchy and both lists bit-exact, potential/field on the particles of 4 sampled leaves."""
     pos, q = inputs.uniform_cube(10**7, 57, np.float32)
     sampled_case("cfg5_cube1e7_f32", n_sample_leaves=4, workload=(pos, q, dict(p=8, N_max=128, s=3, theta=0.77)))
+
+
+def test_config5_sphere_one_million_sampled():
+    """Config 5, points on the unit-sphere surface, N = 1e6, fp32, p = 8."""
+    pos, q = inputs.sphere_surface(10**6, 56, np.float32)
+    sampled_case("cfg5_sphere1e6_f32", n_sample_leaves=8, workload=(pos, q, dict(p=8, N_max=128, s=3, theta=0.77)))
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("N,N_max,s,p", [(20000, 512, 3, 6), (5000, 512, 1, 4), (3000, 3000, 2, 5)])
+def test_large_leaves(dtype, N, N_max, s, p):
+    """Config 5's N_max = 512: leaves of 300+ particles are cut into chunks of 32 x TPT targets per warp (P2P), several
+    P2M / L2P passes per leaf; N_max >= N gives a single leaf (L = 0, everything is P2P)."""
+    pos, q = inputs.uniform_cube(N, 58, dtype)
+    run_case(pos, q, p, N_max, s, direct=N_max < N)  # a single leaf: the oracle IS the direct sum, nothing to compare the error with
