@@ -20,6 +20,10 @@
  *  - fmm_plan_create and the fmm_plan_copy_* / fmm_plan_info calls synchronise the stream before
  *    returning; fmm_evaluate only enqueues work on the stream (asynchronous).  Evaluations on one plan
  *    must be serialised by stream order (the plan owns the coefficient scratch arrays).
+ *  - One device per process: the operator tables, constant memory and kernel attributes are set up once, on the device that
+ *    is current at the first call; every later call must run with the same current device (bench.py: one process per GPU).
+ *  - Plan memory comes from the device's default stream-ordered memory pool (cudaMallocAsync); up to 8 GiB of freed blocks stay
+ *    cached there for the next plan (cudaMemPoolTrimTo on the default pool returns them).
  *  - Outputs are in INPUT order.
  *  - No exception or abort crosses this boundary: every failure is a status code, *out_plan is NULL on
  *    failure, fmm_last_error() returns a thread-local message.
