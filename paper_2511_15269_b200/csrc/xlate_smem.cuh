@@ -12,6 +12,10 @@
 #pragma once
 #include "xlate_reg.cuh"
 
+#ifndef FMM_SMEM_SYNC
+#define FMM_SMEM_SYNC 1
+#endif
+
 namespace fmm {
 namespace {
 
@@ -34,9 +38,16 @@ struct SArgs {
 // compiler-only barrier between two blocks: keeps the loads of the next block behind the stores of this one, so that
 // only one block (plus the trig / power tables) is live in registers at a time
 __device__ __forceinline__ void fence_block() { asm volatile("" ::: "memory"); }
+// SYNC: the warps of a CTA meet after every block, so that they walk the (100+ KB, straight-line) code together and share
+// instruction-cache lines
+template <bool SYNC>
+__device__ __forceinline__ void meet() {
+    if constexpr (SYNC) __syncthreads();
+    else fence_block();
+}
 
 // state element idx of this thread: col[idx * LD]
-template <typename T, int P, int KIND, int LD>
+template <typename T, int P, int KIND, int LD, bool SYNC>
 __device__ __forceinline__ void translate_blocked(T* __restrict__ col, T bx, T by, T bz, T a_old, T a_new) {
     constexpr int P1 = P + 1, K = P1 * P1;
     const T rxy2 = bx * bx + by * by;
@@ -71,7 +82,7 @@ __device__ __forceinline__ void translate_blocked(T* __restrict__ col, T bx, T b
             apply_az<T, n, +1>(v, cth, sth);
             apply_B<T, n, false>(v);
             sfor<2 * n + 1>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = v[n * n + decltype(ic)::value]; });
-            fence_block();
+            meet<SYNC>();
         });
     }
 
@@ -131,7 +142,7 @@ __device__ __forceinline__ void translate_blocked(T* __restrict__ col, T bx, T b
                 col[(n * n + n + m) * LD] = acc * pw2[n];
             });
         }
-        fence_block();
+        meet<SYNC>();
     });
 
     // inverse rotation
@@ -143,7 +154,7 @@ __device__ __forceinline__ void translate_blocked(T* __restrict__ col, T bx, T b
         apply_B<T, n, false>(v);
         apply_az<T, n, -1>(v, cph, sph);
         sfor<2 * n + 1>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = v[n * n + decltype(ic)::value]; });
-        fence_block();
+        meet<SYNC>();
     });
 }
 
@@ -165,8 +176,9 @@ __global__ void __launch_bounds__(NT) xlate_smem_k(SArgs a) {
             }
         }
     }
+    constexpr bool SYNC = KIND == 1 && FMM_SMEM_SYNC;
     const unsigned vmask = __ballot_sync(0xffffffffu, gs >= 0);
-    if (vmask == 0) return;  // warps are independent (only __syncwarp below)
+    if (!SYNC && vmask == 0) return;  // warps are independent (only __syncwarp below) unless they walk the code in lockstep
 
     // stage in: the source rows of the warp's 32 translations, each read coalesced by the whole warp
     const T* in = reinterpret_cast<const T*>(a.in);
@@ -180,13 +192,14 @@ __global__ void __launch_bounds__(NT) xlate_smem_k(SArgs a) {
             if (lane + 32 * j < K) wcol[(lane + 32 * j) * LD + r] = row[lane + 32 * j];
     }
     __syncwarp();
-    if (gs >= 0) {
+    if (SYNC || gs >= 0) {
+        const int gs_ = gs >= 0 ? gs : 0, gt_ = gt >= 0 ? gt : 0;
         const T* sc = reinterpret_cast<const T*>(a.scale);
         const T* scs = reinterpret_cast<const T*>(a.scale_s);
-        const T bx = (T)(a.ctr_s[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
-        const T by = (T)(a.ctr_s[3 * (int64_t)gs + 1] - a.ctr[3 * (int64_t)gt + 1]);
-        const T bz = (T)(a.ctr_s[3 * (int64_t)gs + 2] - a.ctr[3 * (int64_t)gt + 2]);
-        translate_blocked<T, P, KIND, LD>(wcol + lane, bx, by, bz, scs[gs], sc[gt]);
+        const T bx = (T)(a.ctr_s[3 * (int64_t)gs_] - a.ctr[3 * (int64_t)gt_]);
+        const T by = (T)(a.ctr_s[3 * (int64_t)gs_ + 1] - a.ctr[3 * (int64_t)gt_ + 1]);
+        const T bz = (T)(a.ctr_s[3 * (int64_t)gs_ + 2] - a.ctr[3 * (int64_t)gt_ + 2]);
+        translate_blocked<T, P, KIND, LD, SYNC>(wcol + lane, bx, by, bz, scs[gs_], sc[gt_]);
     }
     __syncwarp();
 
