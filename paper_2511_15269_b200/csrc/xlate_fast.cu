@@ -173,10 +173,12 @@ void launch(const XArgs& a, cudaStream_t st) {
     xlate_fast_k<T, P, KIND, XW, SYNC><<<grid, XW * 32, smem, st>>>(a);
 }
 
+// fp64 M2L at p >= 7 (255 registers, 2 warps per scheduler): the warps of a CTA walk the code in lockstep (SYNC), which shares
+// instruction-cache lines: p = 8 2.48 -> 2.01 ms on B200; at p <= 6 and in fp32 (4 warps per scheduler) lockstep costs more than it saves.
 template <typename T, int KIND>
 bool dispatch(int p, const XArgs& a, cudaStream_t st) {
     switch (p) {
-#define FMM_CASE(PP) case PP: launch<T, PP, KIND>(a, st); return true;
+#define FMM_CASE(PP) case PP: launch<T, PP, KIND, 4, (sizeof(T) == 8 && KIND == 1 && PP >= 7)>(a, st); return true;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
         default: return false;
