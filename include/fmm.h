@@ -20,8 +20,10 @@
  *  - fmm_plan_create and the fmm_plan_copy_* / fmm_plan_info calls synchronise the stream before
  *    returning; fmm_evaluate only enqueues work on the stream (asynchronous).  Evaluations on one plan
  *    must be serialised by stream order (the plan owns the coefficient scratch arrays).
- *  - One device per process: the operator tables, constant memory and kernel attributes are set up once, on the device that
- *    is current at the first call; every later call must run with the same current device (bench.py: one process per GPU).
+ *  - A plan lives on the CUDA device that is current when it is created.  Every later call that takes the plan must run with
+ *    that device current (cudaSetDevice) and returns FMM_ERR_INVALID_ARG otherwise; fmm_plan_destroy switches by itself.
+ *    One process may hold plans on several devices (operator tables, constant memory and kernel attributes are kept per
+ *    device; their one-time setup is mutex-guarded).  Calls on ONE plan must not overlap in time on the host.
  *  - Plan memory comes from the device's default stream-ordered memory pool (cudaMallocAsync); up to 8 GiB of freed blocks stay
  *    cached there for the next plan (cudaMemPoolTrimTo on the default pool returns them).
  *  - Outputs are in INPUT order.
@@ -57,8 +59,9 @@ typedef struct {
     double theta;    /* 0 < theta < 1; the paper's default is 0.77 */
     int cross_level; /* 0 = same-level lists (the default).  1 = level-marching lists: weak
                       * pairs may join a target box with a source box one level below it; the march over (target level,
-                      * source level) is (0,0), (1,0), (1,1), (2,1), ..., (L,L) (reading S9).  Fewer M2L pairs
-                      * at the same eq. (4). */
+                      * source level) is (0,0), (0,1), (1,1), (1,2), ..., (L,L): on equal levels the SOURCE level is increased
+                      * first (reading S9), so a source box is never coarser than its target box.
+                      * Fewer M2L pairs at the same eq. (4). */
 } fmm_admissibility;
 
 /* Build hierarchy + lists for N charges (Listing 2; lists PAPER.md:72-74).
@@ -142,13 +145,9 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
 fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
 
 /* Selects the kernel family used by subsequent fmm_evaluate calls on this plan:
- * 0 = automatic (register translation kernels, one translation per thread, and the packed-f32x2 P2P kernel when available
- * for (p, dtype), else the generic kernels), 1 = force the generic kernels (any p <= FMM_P_MAX, both dtypes; used by the
- * tests to cross-check), 2 = as 0 but M2L by the two-pairs-per-thread packed-f32x2 kernel (m2l_packed.cu), 3 = as 0 but M2L by
- * the software-pipelined kernel over target-aligned batches (m2l_stream.cu; the batch copy of the weak list is built on the
- * first evaluate).  0 is the fastest measured on B200; 2 and 3 are kept as measured alternatives.
- * "Register translation kernels" covers p <= 8 (state in registers) and 9 <= p <= 12 (state in shared memory), fp32 and fp64;
- * 2 and 3 exist for fp32, p <= 8, single-hierarchy plans only and fall back to 0 elsewhere (separate-targets plans included). */
+ * 0 = automatic (the one-translation-per-thread kernels for M2M / M2L / L2L and the warp-per-leaf P2P kernels; the generic
+ * kernels where no specialised kernel exists for (p, dtype)), 1 = force the generic warp-per-box kernels (any p <= FMM_P_MAX,
+ * both dtypes; a second, independent implementation of App. B that the tests cross-check against the oracle). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
 /* Schedule of subsequent fmm_evaluate / fmm_evaluate_host calls on this plan.  0 (default) = concurrent: the call forks

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfmm_b200.so")
-SOURCES = ["api.cu", "plan.cu", "tables.cu", "evaluate.cu", "xlate_fast.cu", "xlate_smem.cu", "xlate_smem_f32.cu", "xlate_smem_f64.cu", "m2l_packed.cu", "m2l_stream.cu", "p2p_fast.cu"]
+SOURCES = ["api.cu", "plan.cu", "tables.cu", "evaluate.cu", "xlate_fast.cu", "xlate_smem.cu", "xlate_smem_f32.cu", "xlate_smem_f64.cu", "p2p_fast.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr", "--extended-lambda", "-Xptxas", "-v"]
 
@@ -56,15 +56,5 @@ def build(force=False, verbose=False):
     return LIB
 
 
-def build_ubench():
-    """Stand-alone FP32-pipe micro-benchmark (csrc/ubench_fp32_pipe.cu); not part of the library."""
-    exe = os.path.join(HERE, "ubench_fp32_pipe")
-    subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, os.path.join(CSRC, "ubench_fp32_pipe.cu")])
-    return exe
-
-
 if __name__ == "__main__":
-    if "--ubench" in sys.argv:
-        print(build_ubench())
-    else:
-        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

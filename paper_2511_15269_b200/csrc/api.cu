@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstring>
 #include <new>
+#include <string>
 #include <utility>
 
 #include "internal.cuh"
@@ -40,18 +41,34 @@ fmm_status guarded(F&& f) {
 
 size_t esize(fmm_dtype d) { return d == FMM_F32 ? 4 : 8; }
 
-// keep up to 8 GiB of freed blocks mapped in the device's default memory pool (see DevBuf)
-void init_pool() {
-    static bool done = false;
-    if (done) return;
-    int dev = 0;
-    cudaMemPool_t pool;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        unsigned long long thr = 8ull << 30;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+// per-device setup on plan creation: operator tables (device_ctx) and the memory pool -- keep up to 8 GiB of freed blocks mapped
+// in the device's default memory pool (see DevBuf).  Returns the current device.
+int init_device() {
+    const int dev = current_device();
+    DeviceCtx& ctx = device_ctx(dev);
+    std::lock_guard<std::mutex> lock(ctx.mu);
+    if (!ctx.pool_ready) {
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long thr = 8ull << 30;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+        cudaGetLastError();
+        ctx.pool_ready = true;
     }
-    cudaGetLastError();
-    done = true;
+    return dev;
+}
+
+// every entry point that touches device memory of a plan: the plan's device must be the current one
+bool on_plan_device(const Plan& P) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != P.device) {
+        cudaGetLastError();
+        set_error("the plan lives on device " + std::to_string(P.device) + " but the current device is " + std::to_string(dev) +
+                  " (call cudaSetDevice first)");
+        return false;
+    }
+    return true;
 }
 
 // N, p, N_max, s, dtype -> depth and box numbering of one hierarchy (rule T1 / T2); false if the tree is too large
@@ -121,14 +138,14 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
             return FMM_ERR_CUDA;
         }
         cudaStream_t st = (cudaStream_t)cuda_stream;
-        init_pool();
+        const int dev = init_device();
         AllocScope scope(st);
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
+            P.device = dev;
             P.cross_level = cross_level;
             if (!init_shape(P, N, p, N_max, s, dtype, theta)) { delete h; return FMM_ERR_UNSUPPORTED; }
-            tables();
             cudaEvent_t e0, e1;
             FMM_CUDA_CHECK(cudaEventCreate(&e0));
             FMM_CUDA_CHECK(cudaEventCreate(&e1));
@@ -179,17 +196,18 @@ fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void
             return FMM_ERR_CUDA;
         }
         cudaStream_t st = (cudaStream_t)cuda_stream;
-        init_pool();
+        const int dev = init_device();
         AllocScope scope(st);
         fmm_plan* h = new fmm_plan();
         Plan& P = h->P;
         try {
+            P.device = dev;
             P.cross_level = 1;
             P.S.reset(new Plan());
             Plan& S = *P.S;
+            S.device = dev;
             S.cross_level = 1;
             if (!init_shape(P, Nt, p, N_max, s, dtype, theta) || !init_shape(S, Ns, p, N_max, s, dtype, theta)) { delete h; return FMM_ERR_UNSUPPORTED; }
-            tables();
             cudaEvent_t e0, e1;
             FMM_CUDA_CHECK(cudaEventCreate(&e0));
             FMM_CUDA_CHECK(cudaEventCreate(&e1));
@@ -236,6 +254,7 @@ fmm_status fmm_plan_copy_source_tree(const fmm_plan* plan, int32_t* h_perm, int3
                                      void* h_box_hi, double* h_box_ctr, double* h_box_rad) {
     return guarded([&]() -> fmm_status {
         if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
         return copy_tree_impl(plan->P.S ? *plan->P.S : plan->P, h_perm, h_box_start, h_box_count, h_box_lo, h_box_hi, h_box_ctr, h_box_rad);
     });
 }
@@ -249,14 +268,25 @@ fmm_status fmm_plan_copy_march(const fmm_plan* plan, int32_t* h_steps, int32_t* 
 }
 
 fmm_status fmm_plan_destroy(fmm_plan* plan) {
-    if (plan) cudaDeviceSynchronize();  // nothing of the plan may still be in flight on any stream when its memory returns to the pool
-    delete plan;
-    return FMM_OK;
+    if (!plan) return FMM_OK;
+    return guarded([&]() -> fmm_status {
+        // the plan's memory goes back to the pool of ITS device: switch to it for the duration of the call if necessary
+        int cur = -1;
+        const int pdev = plan->P.device;
+        const bool have = cudaGetDevice(&cur) == cudaSuccess;
+        if (have && cur != pdev) cudaSetDevice(pdev);
+        cudaDeviceSynchronize();  // nothing of the plan may still be in flight on any stream when its memory returns to the pool
+        delete plan;
+        if (have && cur != pdev) cudaSetDevice(cur);
+        cudaGetLastError();
+        return FMM_OK;
+    });
 }
 
 fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream) {
     return guarded([&]() -> fmm_status {
         if (!plan || !d_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
         AllocScope scope((cudaStream_t)cuda_stream);
         run_evaluate(plan->P, d_charges, d_potential, d_field, (cudaStream_t)cuda_stream, nullptr);
         return FMM_OK;
@@ -267,6 +297,7 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
                                  double* h_stage_ms) {
     return guarded([&]() -> fmm_status {
         if (!plan || !d_charges || !h_stage_ms) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
         cudaEvent_t ev[8];
         for (auto& e : ev) FMM_CUDA_CHECK(cudaEventCreate(&e));
         cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -290,6 +321,7 @@ fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, vo
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream) {
     return guarded([&]() -> fmm_status {
         if (!plan || !h_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
         Plan& P = const_cast<Plan&>(plan->P);
         const size_t es = esize(P.dtype);
         cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -325,6 +357,7 @@ fmm_status fmm_plan_copy_tree(const fmm_plan* plan, int32_t* h_perm, int32_t* h_
                               void* h_box_hi, double* h_box_ctr, double* h_box_rad) {
     return guarded([&]() -> fmm_status {
         if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
         return copy_tree_impl(plan->P, h_perm, h_box_start, h_box_count, h_box_lo, h_box_hi, h_box_ctr, h_box_rad);
     });
 }
@@ -333,6 +366,7 @@ fmm_status fmm_plan_copy_lists(const fmm_plan* plan, int64_t* h_weak_off, int32_
     return guarded([&]() -> fmm_status {
         if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
         const Plan& P = plan->P;
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
         FMM_CUDA_CHECK(cudaDeviceSynchronize());
         if (h_weak_off) FMM_CUDA_CHECK(cudaMemcpy(h_weak_off, P.weak_off.p, (P.n_boxes + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost));
         if (h_weak_src && P.n_weak) FMM_CUDA_CHECK(cudaMemcpy(h_weak_src, P.weak_src.p, P.n_weak * sizeof(int32_t), cudaMemcpyDeviceToHost));
@@ -361,7 +395,7 @@ fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial) {
 }
 
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {
-    if (!plan || variant < 0 || variant > 3) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    if (!plan || variant < 0 || variant > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
     plan->P.m2l_variant = variant;
     return FMM_OK;
 }

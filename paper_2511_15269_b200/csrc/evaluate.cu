@@ -564,8 +564,6 @@ void dispatch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cuda
     }
 }
 
-bool g_const_uploaded = false;
-
 // Internal streams of a plan (created on first use).  s_far / s_up have the highest priority, s_near the lowest, so that
 // the latency-bound far-field kernels get SM resources as soon as they are launched and P2P fills whatever is left.
 void ensure_streams(const Plan& Pl) {
@@ -587,7 +585,7 @@ template <typename T>
 void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
     using T4 = typename V4<T>::type;
     const Plan& S = *Pl.S;
-    const Tables& tb = tables();
+    const Tables& tb = tables(Pl.device);
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
     const int p = Pl.p, s = Pl.s;
     const bool serial = ev != nullptr || Pl.serial;
@@ -669,7 +667,7 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
 template <typename T>
 void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
     using T4 = typename V4<T>::type;
-    const Tables& tb = tables();
+    const Tables& tb = tables(Pl.device);
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
     const int p = Pl.p, s = Pl.s, L = Pl.L;
     const int64_t N = Pl.N;
@@ -687,11 +685,8 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
         FMM_CUDA_CHECK(cudaEventRecord(e, producer));
         FMM_CUDA_CHECK(cudaStreamWaitEvent(waiter, e, 0));
     };
-    // m2l_variant: 0 = register kernels (one translation per thread), 1 = generic kernels, 2 = as 0 but M2L two pairs per thread (f32x2)
+    // m2l_variant: 0 = register / shared-memory kernels (one translation per thread), 1 = generic kernels (warp per box)
     const bool fast = Pl.m2l_variant != 1 && xlate_fast_available(p, Pl.dtype);
-    const bool packed = Pl.m2l_variant == 2 && m2l_packed_available(p, Pl.dtype);
-    const bool stream = Pl.m2l_variant == 3 && m2l_stream_available(p, Pl.dtype) && Pl.n_weak > 0;
-    if (stream && Pl.n_m2l_batches == 0) build_m2l_batches(const_cast<Plan&>(Pl), st);  // built on first use of variant 3
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
@@ -732,15 +727,9 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     if (Pl.n_weak > 0) {
         auto m2l_range = [&](int64_t e0, int64_t e1, cudaStream_t q) {
             if (e1 <= e0) return;
-            if (packed) m2l_packed_launch(Pl, q, e0, e1);
-            else xlate_fast_launch(Pl, 1, 0, q, e0, e1);
+            xlate_fast_launch(Pl, 1, 0, q, e0, e1);
         };
-        if (stream) {
-            if (split) {
-                m2l_stream_launch(Pl, sF, Pl.m2l_batch_leaf, Pl.n_m2l_batches);
-                m2l_stream_launch(Pl, sU, 0, Pl.m2l_batch_leaf);
-            } else m2l_stream_launch(Pl, sF, 0, Pl.n_m2l_batches);
-        } else if (split) {
+        if (split) {
             m2l_range(w_leaf, Pl.n_weak, sF);
             m2l_range(0, w_leaf, sU);
         } else if (fast) {
@@ -786,15 +775,18 @@ int64_t evaluate_launches(const Plan& P) {
 }
 
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
-    if (!g_const_uploaded) {
-        const Tables& tb = tables();
-        std::vector<double> g(KMAX);
-        std::vector<float> gf(KMAX);
-        FMM_CUDA_CHECK(cudaMemcpy(g.data(), tb.d_g, KMAX * sizeof(double), cudaMemcpyDeviceToHost));
-        for (int i = 0; i < KMAX; ++i) gf[i] = (float)g[i];
-        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_g, g.data(), KMAX * sizeof(double)));
-        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
-        g_const_uploaded = true;
+    {   // __constant__ copies of g_n^m: one upload per device
+        DeviceCtx& ctx = device_ctx(P.device);
+        std::lock_guard<std::mutex> lock(ctx.mu);
+        if (!ctx.const_uploaded) {
+            std::vector<double> g(KMAX);
+            std::vector<float> gf(KMAX);
+            FMM_CUDA_CHECK(cudaMemcpy(g.data(), ctx.tab.d_g, KMAX * sizeof(double), cudaMemcpyDeviceToHost));
+            for (int i = 0; i < KMAX; ++i) gf[i] = (float)g[i];
+            FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_g, g.data(), KMAX * sizeof(double)));
+            FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
+            ctx.const_uploaded = true;
+        }
     }
     if (P.S) {
         if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev);

@@ -4,7 +4,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <memory>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -66,7 +68,7 @@ struct DevBuf {
     DevBuf& operator=(const DevBuf&) = delete;
 };
 
-// Constant tables of the normalised operators (built once per process, host fp64 -> device):
+// Constant tables of the normalised operators (built once per DEVICE, host fp64 -> device):
 //   Bmat : per degree n a (2n+1)x(2n+1) row-major block at offset boff(n) = n(2n-1)(2n+1)/3;
 //          polar rotation Q_n(theta) = B_n Z_n(theta) B_n^T  (exact identity, B_n derived from d^n(pi/2))
 //   Hm2l : H[m][n][k] = (n+k)! / sqrt((n-m)!(n+m)!(k-m)!(k+m)!) * (-1)^(k+m)      (M2L z-shift weights)
@@ -80,7 +82,33 @@ struct Tables {
     double* d_g = nullptr;   // KMAX
     std::vector<double> h_B; // host copy (used by the unrolled-kernel self check)
 };
-const Tables& tables();  // throws CudaFail
+// Everything the library sets up once per device lives here (tables.cu): operator tables, the __constant__ copies of g_n^m,
+// the memory-pool threshold.  One process may hold plans on several devices; a plan remembers its device (Plan::device) and
+// every entry point checks that it is the current one.  Creation and the one-time steps are guarded by mutexes, so plans on
+// different devices may be created and used from different host threads.
+constexpr int MAX_DEVICES = 64;
+struct DeviceCtx {
+    int dev = -1;
+    Tables tab;
+    std::mutex mu;                // guards the lazy steps below
+    bool const_uploaded = false;  // evaluate.cu: c_g / c_gf
+    bool pool_ready = false;      // api.cu: release threshold of the default memory pool
+};
+DeviceCtx& device_ctx(int dev);   // throws CudaFail; builds and uploads the tables on first use (dev must be the current device)
+int current_device();             // cudaGetDevice or throws
+inline const Tables& tables(int dev) { return device_ctx(dev).tab; }
+
+// one-time, per-device cudaFuncSetAttribute of a kernel instantiation: `static AttrOnce once; once.ensure(dev, [&]{...});`
+struct AttrOnce {
+    std::atomic<unsigned long long> mask{0};
+    template <class F>
+    void ensure(int dev, F&& f) {
+        const unsigned long long bit = 1ull << (dev & (MAX_DEVICES - 1));
+        if (mask.load(std::memory_order_acquire) & bit) return;
+        f();  // idempotent: two threads racing here both set the same attribute
+        mask.fetch_or(bit, std::memory_order_release);
+    }
+};
 __host__ __device__ inline int boff(int n) { return n * (2 * n - 1) * (2 * n + 1) / 3; }
 
 // P2P work item (plan.cu p2p_segments_k, p2p_fast.cu): one segment of the strong list of a target leaf
@@ -91,6 +119,7 @@ struct P2PItem {
 };
 
 struct Plan {
+    int device = 0;  // the CUDA device the plan's memory lives on
     int64_t N = 0;
     int p = 0, N_max = 0, s = 0, L = 0;
     fmm_dtype dtype = FMM_F32;
@@ -125,9 +154,6 @@ struct Plan {
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
-    // weak list in batches of 32 pairs that never straddle two targets (m2l_stream.cu): sources padded with -1, one target per batch
-    DevBuf<int32_t> wpad_src, wpad_tgt;
-    int64_t n_m2l_batches = 0, m2l_batch_leaf = 0;  // m2l_batch_leaf: first batch whose target is a leaf-level box
     DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
     int64_t n_p2p_items = 0;
     bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
@@ -153,7 +179,6 @@ struct Plan {
 // plan.cu
 void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
 void build_lists(Plan& P, cudaStream_t st);
-void build_m2l_batches(Plan& P, cudaStream_t st);  // after build_lists; called on the first evaluate with m2l_variant 3
 // evaluate.cu
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
 int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evaluate
@@ -164,12 +189,6 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
 // xlate_smem.cu: the same three operators for 9 <= p <= 12, one thread per translation with the state vector in shared memory
 bool xlate_smem_available(int p, fmm_dtype dt);
 void xlate_smem_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1);
-// m2l_packed.cu: fp32 M2L with two weak pairs per thread in packed f32x2 arithmetic (p <= 8); results are ADDED to Lc
-bool m2l_packed_available(int p, fmm_dtype dt);
-void m2l_packed_launch(const Plan& P, cudaStream_t st, int64_t e0, int64_t e1);  // weak pairs [e0, e1)
-// m2l_stream.cu: fp32 M2L, one pair per thread, software-pipelined over the batches [b0, b1) of the padded weak list
-bool m2l_stream_available(int p, fmm_dtype dt);
-void m2l_stream_launch(const Plan& P, cudaStream_t st, int64_t b0, int64_t b1);
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
 void p2p_fast_launch(const Plan& P, cudaStream_t st, bool want_field);  // want_field = false: potential only (cheaper inner loop)
 void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field);  // fp64: same mapping, scalar DFMA arithmetic, sources read through L1

@@ -491,9 +491,11 @@ __global__ void p2p_segments_k(const int64_t* soff, const int32_t* ssrc, const i
     }
 }
 
-// ---- level-marching (cross-level) lists, reading S9: steps (lt, ls) = (0,0), (1,0), (1,1), (2,1), ..., (L,L).
+// ---- level-marching (cross-level) lists, reading S9: steps (lt, ls) = (0,0), (0,1), (1,1), (1,2), ..., (L,L).
 // Failing pairs (target box on level lt, source box on level ls; level-local indices) are refined on ONE side per step:
-// the sources when lt == ls, else the targets.  Invariant: for a fixed target the sources appear in ascending order, so a
+// the sources when lt == ls ("if equal, increase the source level"), else the targets.  A source box is therefore
+// never coarser than its target box, which the split schedule of evaluate.cu relies on (the leaf-level M2L reads only
+// leaf-level multipoles and may run beside the M2M pass).  Invariant: for a fixed target the sources appear in ascending order, so a
 // stable sort by target at the end gives the canonical CSR form (L4) that is compared bit by bit with the oracle.
 struct MarchArgs {
     const int32_t *ftgt, *fsrc;
@@ -552,47 +554,7 @@ struct CntLoad {
     __device__ int64_t operator()(int64_t i) const { return i < n ? (int64_t)p[i] : 0; }
 };
 
-// ---- batched copy of the weak list for m2l_stream.cu: every target's sources in batches of 32, padded with -1
-struct BatLoad {
-    const int64_t* woff;
-    int64_t n;
-    __device__ int64_t operator()(int64_t i) const { return i < n ? (woff[i + 1] - woff[i] + 31) / 32 : 0; }
-};
-__global__ void m2l_batches_fill_k(const int64_t* woff, const int32_t* wsrc, const int64_t* bat_off, int64_t n_boxes, int32_t* wpad_src,
-                                   int32_t* wpad_tgt) {
-    const int lane = threadIdx.x & 31;
-    const int64_t t = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (t >= n_boxes) return;
-    const int64_t w0 = woff[t], len = woff[t + 1] - w0, b0 = bat_off[t];
-    for (int64_t k = 0; k * 32 < len; ++k) {
-        const int64_t j = k * 32 + lane;
-        wpad_src[(b0 + k) * 32 + lane] = j < len ? wsrc[w0 + j] : -1;
-        if (lane == 0) wpad_tgt[b0 + k] = (int32_t)t;
-    }
-}
-
 }  // namespace
-
-void build_m2l_batches(Plan& P, cudaStream_t st) {
-    P.n_m2l_batches = 0;
-    P.m2l_batch_leaf = 0;
-    if (P.n_weak == 0) return;
-    DevBuf<int64_t> bat_off, scratch;
-    bat_off.alloc(P.n_boxes + 1);
-    scratch.alloc(scan_scratch_elems(P.n_boxes + 1));
-    exclusive_scan<int64_t>(BatLoad{P.weak_off.p, P.n_boxes}, bat_off.p, P.n_boxes + 1, scratch.p, st);
-    int64_t h[2] = {0, 0};
-    FMM_CUDA_CHECK(cudaMemcpyAsync(&h[0], bat_off.p + P.n_boxes, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-    FMM_CUDA_CHECK(cudaMemcpyAsync(&h[1], bat_off.p + P.level_off[P.L], sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-    P.n_m2l_batches = h[0];
-    P.m2l_batch_leaf = h[1];
-    P.wpad_src.alloc((size_t)h[0] * 32);
-    P.wpad_tgt.alloc((size_t)h[0]);
-    m2l_batches_fill_k<<<nblocks(P.n_boxes * 32, 128), 128, 0, st>>>(P.weak_off.p, P.weak_src.p, bat_off.p, P.n_boxes, P.wpad_src.p, P.wpad_tgt.p);
-    FMM_CUDA_CHECK(cudaGetLastError());
-    FMM_CUDA_CHECK(cudaStreamSynchronize(st));  // bat_off is freed on return
-}
 
 void build_tree(Plan& P, const void* d_positions, cudaStream_t st) {
     if (P.dtype == FMM_F32) build_tree_t<float, uint32_t>(P, (const float*)d_positions, st);

@@ -8,6 +8,12 @@
 //       B_n = Z_n(pi/2) Q_n(pi/2)  (a rotation about y is a rotation about z conjugated by a fixed quarter turn; this
 //       replaces the on-the-fly Wigner-d recursion of PAPER.md:154 / App. B.2).  Three quarters of
 //       the entries vanish (cos/sin-type decoupling and the parity d^n_{m',-m}(pi/2) = (-1)^(n+m') d^n_{m',m}(pi/2)).
+//   Q_n = the normalised real-basis polar rotation by pi/2 itself.  Because Q_n^T = Z_n(pi) Q_n Z_n(pi) (a rotation by -pi/2
+//       about y is the rotation by +pi/2 conjugated by a half turn about z), B_n^T = Z(pi) Q_n Z(pi/2) and therefore
+//           B Z(theta) B^T = Z(pi/2) Q Z(theta + pi) Q Z(pi/2):
+//       ONE constant matrix applied twice between azimuthal rotations.  The register kernels use this form, which lets the
+//       forward and the inverse rotation of a translation share one copy of the Q code and one copy of the Z code in a
+//       run-time loop (xlate_reg.cuh translate_qz) -- the whole kernel then fits the 32 KB instruction cache of an SM.
 //   H[m][n][k] = (-1)^(k+m) (n+k)! / sqrt((n-m)!(n+m)!(k-m)!(k+m)!)          M2L z-shift, App. B.3
 //   A[m][n][k] = sqrt((n-m)!(n+m)! / ((k-m)!(k+m)!)) / (n-k)!,  k <= n         M2M; L2L uses A[m][k][n]
 #pragma once
@@ -62,6 +68,7 @@ constexpr double dhalf(int j, int mp, int m) {
 
 struct RotTab {
     double B[NB];
+    double Q[NB];  // Q_n = normalised polar rotation by pi/2 (same layout as B); Q_n^T = Z_n(pi) Q_n Z_n(pi)
     double H[PF1][PF1][PF1];
     double A[PF1][PF1][PF1];
 };
@@ -83,6 +90,11 @@ constexpr RotTab make_rot_tab() {
             }
         for (int m = 1; m <= n; ++m)
             for (int k = 1; k <= n; ++k) Q[(n - m) * w + (n - k)] = dhalf(n, m, k) - ((k % 2) ? -1.0 : 1.0) * dhalf(n, m, -k);
+        for (int i = 0; i < w * w; ++i) {
+            double v = Q[(i / w) * w + (i % w)];
+            if (v < 1e-13 && v > -1e-13) v = 0.0;  // structural zeros
+            T.Q[boff(n) + i] = v;
+        }
         // B = Z(pi/2) Q : row m of B = cos(m pi/2) Q[m] - sin(m pi/2) Q[-m]
         for (int m = -n; m <= n; ++m) {
             const int r4 = ((m % 4) + 4) % 4;

@@ -1,5 +1,5 @@
 // tables.cu -- constant tables of the normalised operators, generated on the host in extended precision
-// once per process and uploaded.  Independent of oracle/ (different formulas: binomial form of d^n(pi/2)).
+// and uploaded once per device (DeviceCtx).  Independent of oracle/ (different formulas: binomial form of d^n(pi/2)).
 //
 // Normalisation used by every kernel of the CUDA path:
 //   regular functions   Rn_n^m(r) = g_n^m * R^_n^m(r),  g_n^m = sqrt((n-|m|)!(n+|m|)!) * (m != 0 ? sqrt2 : 1)
@@ -10,6 +10,7 @@
 // because a rotation about y is a rotation about z conjugated by a fixed quarter turn.  This replaces the
 // on-the-fly Wigner-d recursion of PAPER.md:154 by constant, half-empty matrices B_n.
 #include <cmath>
+#include <map>
 #include <mutex>
 
 #include "internal.cuh"
@@ -40,12 +41,8 @@ long double dhalf(int j, int mp, int m) {
     return sum * std::sqrt(fact(j + mp) * fact(j - mp) / (fact(j + m) * fact(j - m))) * std::pow(2.0L, -(long double)j);
 }
 
-Tables g_tables;
-std::once_flag g_once;
-fmm_status g_status = FMM_OK;
-
-void build() {
-    try {
+void build(Tables& T) {
+    {
         int nB = 0;
         for (int n = 0; n <= PMAX; ++n) nB += (2 * n + 1) * (2 * n + 1);
         std::vector<double> B(nB, 0.0);
@@ -95,7 +92,6 @@ void build() {
                 const int am = m < 0 ? -m : m;
                 g[n * n + n + m] = (double)(std::sqrt(fact(n - am) * fact(n + am)) * (m ? std::sqrt(2.0L) : 1.0L));
             }
-        Tables& T = g_tables;
         T.h_B = B;
         FMM_CUDA_CHECK(cudaMalloc((void**)&T.d_B, nB * sizeof(double)));
         FMM_CUDA_CHECK(cudaMalloc((void**)&T.d_Bf, nB * sizeof(float)));
@@ -107,17 +103,32 @@ void build() {
         FMM_CUDA_CHECK(cudaMemcpy(T.d_H, H.data(), H.size() * sizeof(double), cudaMemcpyHostToDevice));
         FMM_CUDA_CHECK(cudaMemcpy(T.d_A, A.data(), A.size() * sizeof(double), cudaMemcpyHostToDevice));
         FMM_CUDA_CHECK(cudaMemcpy(T.d_g, g.data(), g.size() * sizeof(double), cudaMemcpyHostToDevice));
-    } catch (CudaFail& f) {
-        g_status = f.st;
     }
 }
 
+std::mutex g_mu;
+std::map<int, std::unique_ptr<DeviceCtx>> g_ctx;
+
 }  // namespace
 
-const Tables& tables() {
-    std::call_once(g_once, build);
-    if (g_status != FMM_OK) throw CudaFail{g_status};
-    return g_tables;
+int current_device() {
+    int dev = 0;
+    FMM_CUDA_CHECK(cudaGetDevice(&dev));
+    return dev;
+}
+
+DeviceCtx& device_ctx(int dev) {
+    std::lock_guard<std::mutex> lock(g_mu);
+    auto it = g_ctx.find(dev);
+    if (it != g_ctx.end()) return *it->second;
+    if (dev < 0 || dev >= MAX_DEVICES) { set_error("device ordinal out of range"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+    if (current_device() != dev) { set_error("device_ctx: not the current device"); throw CudaFail{FMM_ERR_INVALID_ARG}; }
+    std::unique_ptr<DeviceCtx> c(new DeviceCtx());
+    c->dev = dev;
+    build(c->tab);  // throws on failure: nothing is cached then
+    DeviceCtx& ref = *c;
+    g_ctx[dev] = std::move(c);
+    return ref;
 }
 
 }  // namespace fmm

@@ -18,6 +18,11 @@
 #include "tma.cuh"
 #include "xlate_reg.cuh"
 
+// Form of the Q Z loop (xlate_reg.cuh translate_qz), measured on B200 (N = 1M, p = 8, M2L stage): fp32: MODE 0 (A / B trips, no
+// register copies) 0.691 ms, MODE 2 (Q in place) 0.700 ms, MODE 1 (one Q copy + identity trip) 0.75 ms; fp64: MODE 2 1.55 ms,
+// MODE 0 1.66 ms (255 registers either way; MODE 0 spills a little more).
+template <typename T> constexpr int qz_mode() { return sizeof(T) == 4 ? 0 : 2; }
+
 namespace fmm {
 namespace {
 
@@ -40,6 +45,7 @@ struct Geo {
 };
 
 struct XArgs {
+    int device;                   // host side only: the plan's device (per-device kernel attributes)
     int64_t n;                    // number of translations
     const int32_t *tgt, *src;     // KIND 1: global ids per pair
     int64_t off_parent, off_child;
@@ -121,7 +127,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
             if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
             else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
         });
-        translate_reg<T, P, KIND, SYNC>(v, bx, by, bz, a_old, a_new);
+        translate_qz<T, P, KIND, qz_mode<T>()>(v, bx, by, bz, a_old, a_new);
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             V x;
@@ -164,11 +170,8 @@ template <typename T, int P, int KIND, int XW = 4, bool SYNC = false>
 void launch(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
     constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;  // rows + one mbarrier per warp
-    static bool attr_set = false;
-    if (!attr_set) {
-        FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static AttrOnce once;
+    once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
     const unsigned grid = (unsigned)((a.n + XW * 32 - 1) / (XW * 32));
     xlate_fast_k<T, P, KIND, XW, SYNC><<<grid, XW * 32, smem, st>>>(a);
 }
@@ -178,7 +181,7 @@ void launch(const XArgs& a, cudaStream_t st) {
 template <typename T, int KIND>
 bool dispatch(int p, const XArgs& a, cudaStream_t st) {
     switch (p) {
-#define FMM_CASE(PP) case PP: launch<T, PP, KIND, 4, (sizeof(T) == 8 && KIND == 1 && PP >= 7)>(a, st); return true;
+#define FMM_CASE(PP) case PP: launch<T, PP, KIND, 4, false>(a, st); return true;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
         default: return false;
@@ -193,6 +196,7 @@ bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == 
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     if (P.p > 8) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }
     XArgs a{};
+    a.device = P.device;
     a.box_count = P.box_count.p;
     a.ctr = a.ctr_s = P.box_ctr.p;
     a.scale = a.scale_s = P.box_scale.p;

@@ -1,4 +1,4 @@
-// xlate_reg.cuh -- building blocks of the register ("fast") translation kernels (xlate_fast.cu, m2l_packed.cu):
+// xlate_reg.cuh -- building blocks of the register ("fast") translation kernels (xlate_fast.cu, xlate_smem.cuh):
 // compile-time loops, application of the constant matrices B_n / B_n^T of rot_tables.cuh with every entry an FFMA
 // immediate, azimuthal rotations (App. B.1 PAPER.md:441 in the normalised basis) and cos/sin(m x) tables.
 // translate_reg is the whole rotate / z-shift / rotate-back operator for one translation held in registers.
@@ -107,96 +107,131 @@ __device__ __forceinline__ void trig_table(T c1, T s1, T (&c)[P1], T (&s)[P1]) {
     });
 }
 
-// KIND 0 = M2M (b = child - parent), 1 = M2L (b = source - target), 2 = L2L (b = parent - child)   [DESIGN.md reading G3]
-// v: input coefficients of the old centre (length scale a_old) -> output coefficients about the new centre (a_new).
-// SYNC: the warps of a CTA meet at a barrier after every phase, so that they walk the (large, straight-line) code in
-// lockstep and share instruction-cache lines.
-template <typename T, int P, int KIND, bool SYNC, int KV>
-__device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
-    constexpr int P1 = P + 1;
-    const T rxy2 = bx * bx + by * by;
-    const T r2 = rxy2 + bz * bz;
-    const T r = sqrt(r2), rxy = sqrt(rxy2);
-    const T rinv = r > T(0) ? T(1) / r : T(0);
-    const T rxyinv = rxy > T(0) ? T(1) / rxy : T(0);
-    const T ct_ = r > T(0) ? bz * rinv : T(1), st_ = rxy * rinv;
-    const T cp_ = rxy > T(0) ? bx * rxyinv : T(1), sp_ = by * rxyinv;
-    T x1, x2;
-    if constexpr (KIND == 0) { x1 = r / a_new; x2 = a_old / a_new; }
-    else if constexpr (KIND == 1) { x1 = a_new * rinv; x2 = a_old * rinv; }
-    else { x1 = -r / a_old; x2 = a_new / a_old; }
+// ------------------------------------------------------------------------------------------------------------------------
+// The translation operator in "Q Z loop" form.  KIND 0 = M2M (b = child - parent), 1 = M2L (b = source - target),
+// 2 = L2L (b = parent - child) [DESIGN.md reading G3]; v: coefficients about the old centre (length scale a_old) -> coefficients
+// about the new centre (a_new).  With Q_n the (constant) polar rotation by pi/2 and Q_n^T = Z(pi) Q_n Z(pi)
+// (rot_tables.cuh), B Z(theta) B^T = Z(pi/2) Q Z(theta + pi) Q Z(pi/2), so that one translation is
+//     Z(pi/2 - phi) Q Z(pi - theta) Q  [ Z(pi/2) S Z(pi/2) ]  Q Z(theta + pi) Q Z(phi + pi/2),
+// S = z-shift.  S acts on the orders +m and -m alike, hence commutes with the azimuthal rotations and
+// Z(pi/2) S Z(pi/2) = Z(pi) S = (-1)^m S: a sign that is folded into the shift constants.  What is left is the sequence
+//     Z  Q Z  Q S  Q Z  Q Z
+// i.e. five trips of a RUN-TIME loop whose body holds ONE copy of the Q code (bnnz(p) FMAs), one copy of the azimuthal
+// code and one copy of the shift.  The straight-line form (round 1) needs four copies of the constant-matrix code and four of
+// the azimuthal code (35 KB of SASS at p = 8, 48 KB with prologue and epilogue); this form is 20 KB, so the whole kernel
+// stays inside the 32 KB instruction cache of an SM.  Measured on B200 with a synthetic FFMA stream (4 warps per
+// scheduler): bodies up to 32 KB issue at 0.97 instructions per clock and scheduler, bodies of 48 KB and more at 0.5.
+template <int n>
+constexpr double qent(int i, int j) {
+    return ct::kTab.Q[ct::boff(n) + i * (2 * n + 1) + j];
+}
+template <int n>
+constexpr bool qfirst(int i, int j) {
+    for (int jj = 0; jj < j; ++jj)
+        if (qent<n>(i, jj) != 0.0) return false;
+    return true;
+}
 
-    T cph[P1], sph[P1], cth[P1], sth[P1];
-    trig_table<T, P1>(cp_, sp_, cph, sph);
-    trig_table<T, P1>(ct_, st_, cth, sth);
-
-    // forward rotation, degree by degree; M2M / M2L fold the source scaling x2^k in
-    {
-        T pw = T(1);
-        sfor<P>([&](auto nc) {
-            constexpr int n = decltype(nc)::value + 1;
-            if constexpr (KIND != 2) {
-                pw *= x2;
-                sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
+// dst[od .. od+2n] <- Q_n src[os .. os+2n]   (src and dst must be different register sets)
+template <typename T, int n, int os, int od, int NS, int ND>
+__device__ __forceinline__ void q_from_to(const T (&src)[NS], T (&dst)[ND]) {
+    constexpr int w = 2 * n + 1;
+    sfor<w>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        T acc = T(0.f);
+        sfor<w>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            constexpr double b = qent<n>(i, j);
+            if constexpr (b != 0.0) {
+                if constexpr (qfirst<n>(i, j)) acc = T(b) * src[os + j];
+                else acc = fma(T(b), src[os + j], acc);
             }
-            apply_az<T, n, +1>(v, cph, sph);
-            apply_B<T, n, true>(v);
-            apply_az<T, n, +1>(v, cth, sth);
-            apply_B<T, n, false>(v);
-            if constexpr (SYNC && n >= 3) __syncthreads();
         });
-    }
+        dst[od + i] = acc;
+    });
+}
 
-    // z-shift (App. B.3), order by order; only equal m couple
+// dst <- Z_n(angle) src for one degree (App. B.1 PAPER.md:441 in the normalised basis, forward sense); order 0 is copied
+template <typename T, int n, int os, int od, int NS, int ND, int P1>
+__device__ __forceinline__ void az_from_to(const T (&src)[NS], T (&dst)[ND], const T (&c)[P1], const T (&s)[P1]) {
+    dst[od + n] = src[os + n];
+    sfor<n>([&](auto mc) {
+        constexpr int m = decltype(mc)::value + 1;
+        const T a = src[os + n + m], b = src[os + n - m];
+        dst[od + n + m] = fmsub(a, c[m], b * s[m]);
+        dst[od + n - m] = fma(b, c[m], a * s[m]);
+    });
+}
+
+// z-shift of App. B.3 in the normalised, scaled representation, times (-1)^m (see above); in place.
+// M2L expects v already scaled by x2^k and applies x1^n / r; M2M expects v scaled by x2^k; L2L applies x2^n itself.
+template <typename T, int P, int KIND, bool FUSE, int KV>
+__device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
+    constexpr int P1 = P + 1;
     if constexpr (KIND == 1) {
+        T pwo[P1];
+        if constexpr (FUSE) {
+            pwo[0] = rinv;
+            sfor<P>([&](auto jc) { pwo[decltype(jc)::value + 1] = pwo[decltype(jc)::value] * x1; });
+        }
         sfor<2 * P + 1>([&](auto mi) {
             constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+            constexpr double sg = (am & 1) ? -1.0 : 1.0;
             T t[cnt];
             sfor<cnt>([&](auto ni) {
                 constexpr int n = am + decltype(ni)::value;
-                constexpr double h0 = ct::kTab.H[am][n][am];
+                constexpr double h0 = sg * ct::kTab.H[am][n][am];
                 T acc = T(h0) * v[am * am + am + m];
                 sfor<cnt - 1>([&](auto ki) {
                     constexpr int k = am + 1 + decltype(ki)::value;
-                    constexpr double h = ct::kTab.H[am][n][k];
+                    constexpr double h = sg * ct::kTab.H[am][n][k];
                     acc = fma(T(h), v[k * k + k + m], acc);
                 });
                 t[decltype(ni)::value] = acc;
             });
-            sfor<cnt>([&](auto ni) { v[(am + decltype(ni)::value) * (am + decltype(ni)::value + 1) + m] = t[decltype(ni)::value]; });
+            // the output scaling x1^n / r is also the write-back (no register copies inside the run-time loop of translate_qz)
+            sfor<cnt>([&](auto ni) {
+                constexpr int n = am + decltype(ni)::value;
+                if constexpr (FUSE) v[n * n + n + m] = t[decltype(ni)::value] * pwo[n];
+                else v[n * n + n + m] = t[decltype(ni)::value];
+            });
         });
-        T pw = rinv;
-        sfor<P1>([&](auto nc) {
-            constexpr int n = decltype(nc)::value;
-            sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
-            pw *= x1;
-        });
+        if constexpr (!FUSE) {
+            T pw = rinv;
+            sfor<P1>([&](auto nc) {
+                constexpr int n = decltype(nc)::value;
+                sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
+                pw *= x1;
+            });
+        }
     } else {
         T pw1[P1];
         pw1[0] = T(1);
         sfor<P>([&](auto jc) { pw1[decltype(jc)::value + 1] = pw1[decltype(jc)::value] * x1; });
         if constexpr (KIND == 0) {
-            // out[n] = sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (v already scaled by x2^k): in place, n descending
+            // out[n] = (-1)^m sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (A[m][n][n] = 1): in place, n descending
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+                constexpr double sg = (am & 1) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = P - decltype(ni)::value;
-                    T acc = v[n * n + n + m];  // A[m][n][n] = 1
+                    T acc = (am & 1) ? T(0) - v[n * n + n + m] : v[n * n + n + m];
                     sfor<n - am>([&](auto ki) {
                         constexpr int k = am + decltype(ki)::value;
-                        constexpr double aa = ct::kTab.A[am][n][k];
+                        constexpr double aa = sg * ct::kTab.A[am][n][k];
                         acc = fma(T(aa) * pw1[n - k], v[k * k + k + m], acc);
                     });
                     v[n * n + n + m] = acc;
                 });
             });
         } else {
-            // out[n] = x2^n sum_{k=n..p} A[|m|][k][n] x1^(k-n) v[k]: in place, n ascending
+            // out[n] = (-1)^m x2^n sum_{k=n..p} A[|m|][k][n] x1^(k-n) v[k]: in place, n ascending
             T pw2[P1];
             pw2[0] = T(1);
             sfor<P>([&](auto jc) { pw2[decltype(jc)::value + 1] = pw2[decltype(jc)::value] * x2; });
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
+                constexpr double sg = (am & 1) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = am + decltype(ni)::value;
                     T acc = v[n * n + n + m];
@@ -205,22 +240,106 @@ __device__ __forceinline__ void translate_reg(T (&v)[KV], T bx, T by, T bz, T a_
                         constexpr double aa = ct::kTab.A[am][k][n];
                         acc = fma(T(aa) * pw1[k - n], v[k * k + k + m], acc);
                     });
-                    v[n * n + n + m] = acc * pw2[n];
+                    v[n * n + n + m] = acc * (T(sg) * pw2[n]);
                 });
             });
         }
     }
+}
 
-    // inverse rotation
-    if constexpr (SYNC) __syncthreads();
-    sfor<P>([&](auto nc) {
-        constexpr int n = decltype(nc)::value + 1;
-        apply_B<T, n, true>(v);
-        apply_az<T, n, -1>(v, cth, sth);
-        apply_B<T, n, false>(v);
-        apply_az<T, n, -1>(v, cph, sph);
-        if constexpr (SYNC && n >= 3) __syncthreads();
-    });
+// direction of b, scale ratios:  x1, x2 as in translate_reg
+template <typename T, int KIND>
+__device__ __forceinline__ void xlate_geometry(T bx, T by, T bz, T a_old, T a_new, T& ct_, T& st_, T& cp_, T& sp_, T& rinv, T& x1, T& x2) {
+    const T rxy2 = bx * bx + by * by;
+    const T r2 = rxy2 + bz * bz;
+    const T r = sqrt(r2), rxy = sqrt(rxy2);
+    rinv = r > T(0) ? T(1) / r : T(0);
+    const T rxyinv = rxy > T(0) ? T(1) / rxy : T(0);
+    ct_ = r > T(0) ? bz * rinv : T(1);
+    st_ = rxy * rinv;
+    cp_ = rxy > T(0) ? bx * rxyinv : T(1);
+    sp_ = by * rxyinv;
+    if constexpr (KIND == 0) { x1 = r / a_new; x2 = a_old / a_new; }
+    else if constexpr (KIND == 1) { x1 = a_new * rinv; x2 = a_old * rinv; }
+    else { x1 = -r / a_old; x2 = a_new / a_old; }
+}
+
+// Register copies would be real instructions inside a run-time loop (the state must sit in the same registers at every
+// back edge), so Q never works in place: it is always paired with an azimuthal rotation that moves the degree between the state v
+// and a per-degree temporary -- "A(alpha)": t = Z_n(alpha) v_n, v_n = Q_n t  and  "B(alpha)": t = Q_n v_n, v_n = Z_n(alpha) t.
+// MODE 0: trips A(phi + pi/2), A(theta + pi), S, B(pi - theta), B(pi/2 - phi): no wasted work, two copies of the Q / Z code.
+// MODE 1: trips A(phi + pi/2), A(theta + pi), S, A(0), A(pi - theta), Z(pi/2 - phi) in place: one copy of the Q code, one
+//         identity rotation (2 p (p+1) extra FMAs).
+template <typename T>
+__device__ __forceinline__ void qz_angle(int k, T ct_, T st_, T cp_, T sp_, T& c1, T& s1) {
+    // k: 0: phi + pi/2   1: theta + pi   2: pi - theta   3: pi/2 - phi   4: 0
+    c1 = k == 0 ? T(0) - sp_ : (k == 3 ? sp_ : (k == 4 ? T(1) : T(0) - ct_));
+    s1 = (k == 0 || k == 3) ? cp_ : (k == 1 ? T(0) - st_ : (k == 2 ? st_ : T(0)));
+}
+
+template <typename T, int P, int KIND, int MODE, int KV>
+__device__ __forceinline__ void translate_qz(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
+    constexpr int P1 = P + 1;
+    T ct_, st_, cp_, sp_, rinv, x1, x2;
+    xlate_geometry<T, KIND>(bx, by, bz, a_old, a_new, ct_, st_, cp_, sp_, rinv, x1, x2);
+    if constexpr (KIND != 2) {  // M2M / M2L: the source scaling x2^n commutes with the rotations
+        T pw = T(1);
+        sfor<P>([&](auto nc) {
+            constexpr int n = decltype(nc)::value + 1;
+            pw *= x2;
+            sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
+        });
+    }
+    if constexpr (MODE == 2) {  // experiment: Z | Q Z | Q S | Q Z | Q Z with Q in place (register copies at the back edge)
+#pragma unroll 1
+        for (int t = 0; t < 5; ++t) {
+            if (t > 0)
+                sfor<P>([&](auto nc) {
+                    constexpr int n = decltype(nc)::value + 1;
+                    T tt[2 * n + 1];
+                    q_from_to<T, n, n * n, 0>(v, tt);
+                    sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] = tt[decltype(ic)::value]; });
+                });
+            if (t == 2) {
+                shift_signed<T, P, KIND, (MODE != 2)>(v, x1, x2, rinv);
+            } else {
+                T c1, s1, c[P1], s[P1];
+                qz_angle<T>(t < 2 ? t : t - 1, ct_, st_, cp_, sp_, c1, s1);
+                trig_table<T, P1>(c1, s1, c, s);
+                sfor<P>([&](auto nc) { apply_az<T, decltype(nc)::value + 1, +1>(v, c, s); });
+            }
+        }
+        return;
+    }
+    constexpr int NT = MODE == 0 ? 5 : 6;
+#pragma unroll 1
+    for (int t = 0; t < NT; ++t) {
+        if (t == 2) {
+            shift_signed<T, P, KIND, (MODE != 2)>(v, x1, x2, rinv);
+            continue;
+        }
+        T c1, s1, c[P1], s[P1];
+        const int k = MODE == 0 ? (t < 2 ? t : t - 1) : (t < 2 ? t : (t == 3 ? 4 : t - 2));
+        qz_angle<T>(k, ct_, st_, cp_, sp_, c1, s1);
+        trig_table<T, P1>(c1, s1, c, s);
+        if (MODE == 1 && t == 5) {
+            sfor<P>([&](auto nc) { apply_az<T, decltype(nc)::value + 1, +1>(v, c, s); });
+        } else if (MODE == 1 || t < 2) {
+            sfor<P>([&](auto nc) {
+                constexpr int n = decltype(nc)::value + 1;
+                T tt[2 * n + 1];
+                az_from_to<T, n, n * n, 0>(v, tt, c, s);
+                q_from_to<T, n, 0, n * n>(tt, v);
+            });
+        } else {
+            sfor<P>([&](auto nc) {
+                constexpr int n = decltype(nc)::value + 1;
+                T tt[2 * n + 1];
+                q_from_to<T, n, n * n, 0>(v, tt);
+                az_from_to<T, n, 0, n * n>(tt, v, c, s);
+            });
+        }
+    }
 }
 
 }  // namespace xr

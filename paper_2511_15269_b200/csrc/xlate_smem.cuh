@@ -22,6 +22,7 @@ namespace {
 using namespace xr;
 
 struct SArgs {
+    int device;                   // host side only: the plan's device (per-device kernel attributes)
     int64_t n;                    // number of translations
     const int32_t *tgt, *src;     // KIND 1: global ids per pair
     int64_t off_parent, off_child;
@@ -232,11 +233,8 @@ void launch(const SArgs& a, cudaStream_t st) {
     constexpr int NT = sizeof(T) == 4 ? 128 : 64;
     constexpr int K = (P + 1) * (P + 1);
     constexpr size_t smem = (size_t)K * (NT + 1) * sizeof(T);
-    static bool attr_set = false;
-    if (!attr_set) {
-        FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_smem_k<T, P, KIND, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static AttrOnce once;
+    once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_smem_k<T, P, KIND, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
     const unsigned grid = (unsigned)((a.n + NT - 1) / NT);
     xlate_smem_k<T, P, KIND, NT><<<grid, NT, smem, st>>>(a);
 }
@@ -255,6 +253,7 @@ bool dispatch(int p, const SArgs& a, cudaStream_t st) {
 template <typename T>
 bool smem_launch_t(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     SArgs a{};
+    a.device = P.device;
     a.box_count = P.box_count.p;
     a.ctr = a.ctr_s = P.box_ctr.p;
     a.scale = a.scale_s = P.box_scale.p;

@@ -64,16 +64,17 @@ def test_wigner_d_textbook_low_degree(beta):
     assert abs(d(2, 1, -1, beta) - (-2 * c * c + c + 1) / 2) < 1e-15
 
 
-@pytest.mark.parametrize("j", [3, 6, 10, 12])
+@pytest.mark.parametrize("j", [3, 6, 10, 12, 14, 16])
 def test_wigner_d_m0_column_is_associated_legendre(j):
-    """d^j_{m,0}(b) = sqrt((j-m)!/(j+m)!) P_j^m(cos b) (P with Condon-Shortley phase)."""
+    """d^j_{m,0}(b) = sqrt((j-m)!/(j+m)!) P_j^m(cos b) (P with Condon-Shortley phase).  Up to j = FMM_P_MAX = 16: the explicit
+    sum (reading S6) cancels more and more digits with j; 1e-12 at j = 16 is still far inside the fp64 parity tolerance."""
     beta = 0.9
     for m in range(0, j + 1):
         want = math.sqrt(math.factorial(j - m) / math.factorial(j + m)) * lpmv(m, j, math.cos(beta))
-        assert abs(O.wigner_d(j, m, 0, beta) - want) < 1e-13
+        assert abs(O.wigner_d(j, m, 0, beta) - want) < (1e-13 if j <= 12 else 1e-12)
 
 
-@pytest.mark.parametrize("j", [1, 4, 8, 12])
+@pytest.mark.parametrize("j", [1, 4, 8, 12, 16])
 def test_wigner_d_identity_orthogonality_symmetries(j):
     beta = 0.77
     ms = range(-j, j + 1)
@@ -97,8 +98,9 @@ def test_wigner_d_identity_orthogonality_symmetries(j):
 
 
 # ---------------------------------------------------------------- rotations B.1 / B.2
-def _cloud(n, scale, centre):
-    return centre + scale * (RNG.random((n, 3)) - 0.5), RNG.uniform(-1, 1, n)
+def _cloud(n, scale, centre, rng=None):
+    rng = RNG if rng is None else rng
+    return centre + scale * (rng.random((n, 3)) - 0.5), rng.uniform(-1, 1, n)
 
 
 @pytest.mark.parametrize("ang", [0.4, -1.3, 2.9])
@@ -155,50 +157,51 @@ def test_polar_rotation_orthogonal_after_normalisation():
 DIRS = [np.array(v, dtype=float) for v in [(0.3, -0.5, 0.7), (0, 0, 1.3), (0, 0, -0.9), (1.1, 0.4, 0), (-0.2, -0.9, -0.6), (0.0, 0.7, 0.0)]]
 
 
+@pytest.mark.parametrize("p", [8, 16])
 @pytest.mark.parametrize("b", DIRS)
-def test_m2m_is_exact(b):
-    """M2M(P2M about c_old; b = c_old - c_new) == P2M about c_new, to round-off, for all n <= p."""
-    p = 8
+def test_m2m_is_exact(b, p):
+    """M2M(P2M about c_old; b = c_old - c_new) == P2M about c_new, to round-off, for all n <= p (p = 16 = FMM_P_MAX too)."""
     c_new = np.array([0.1, 0.2, -0.3])
     c_old = c_new + b
     pts, q = _cloud(9, 0.6, c_old)
     got = O.translate(O.M2M, p, _p2m(p, pts, q, c_old), b)
     want = _p2m(p, pts, q, c_new)
-    assert np.max(np.abs(got - want)) < 1e-13 * max(1.0, np.max(np.abs(want)))
+    assert np.max(np.abs(got - want)) < (1e-13 if p <= 8 else 2e-12) * max(1.0, np.max(np.abs(want)))
     # monopole only: C' = q R^(b)
     e0 = np.zeros(O.nk(p)); e0[0] = 2.5
     assert np.max(np.abs(O.translate(O.M2M, p, e0, b) - 2.5 * O.regular_basis(p, b))) < 1e-14
 
 
+@pytest.mark.parametrize("p", [8, 16])
 @pytest.mark.parametrize("b", DIRS)
-def test_l2l_is_exact(b):
+def test_l2l_is_exact(b, p):
     """same polynomial before and after: sum w D R^(x - c_old) == sum w D' R^(x - c_new)."""
-    p = 8
     c_new = np.array([0.1, 0.2, -0.3])
     c_old = c_new + b
     D = RNG.standard_normal(O.nk(p))
     Dn = O.translate(O.L2L, p, D, b)
     for x in (c_new + np.array([0.2, -0.1, 0.15]), c_new + np.array([-0.3, 0.25, 0.05])):
         a, bb = _eval_local(p, D, x - c_old), _eval_local(p, Dn, x - c_new)
-        assert abs(a - bb) < 1e-12 * max(1.0, abs(a))
+        assert abs(a - bb) < (1e-12 if p <= 8 else 2e-11) * max(1.0, abs(a))
 
 
+@pytest.mark.parametrize("p", [10, 16])
 @pytest.mark.parametrize("b", DIRS)
-def test_m2l_of_a_monopole_is_the_singular_basis(b):
+def test_m2l_of_a_monopole_is_the_singular_basis(b, p):
     """A charge sitting exactly on c_s has C = (q,0,...); M2L must return D = q S^(c_s - c_t) exactly (no truncation)."""
-    p = 10
     e0 = np.zeros(O.nk(p)); e0[0] = -1.7
     got = O.translate(O.M2L, p, e0, 3.0 * b)
     want = -1.7 * O.singular_basis(p, 3.0 * b)
     scale = np.array([math.factorial(n) / np.linalg.norm(3 * b) ** (n + 1) for n in range(p + 1) for _ in range(2 * n + 1)])
-    assert np.max(np.abs(got - want) / scale) < 1e-12
+    # at p = 16 the explicit Wigner sum (reading S6) has lost about five digits for directions in the xy-plane (beta = pi/2)
+    assert np.max(np.abs(got - want) / scale) < (1e-12 if p <= 10 else 5e-11)
 
 
 @pytest.mark.parametrize("b", DIRS)
 def test_m2l_converges_to_direct(b):
     c_t = np.array([0.1, 0.2, -0.3])
     c_s = c_t + 2.6 * b / np.linalg.norm(b)
-    pts, q = _cloud(12, 1.0, c_s)
+    pts, q = _cloud(12, 1.0, c_s, np.random.default_rng(77))  # own generator: the pointwise decay check must not depend on test order
     x = c_t + np.array([0.15, -0.2, 0.1])
     exact = sum(qi / np.linalg.norm(x - r) for r, qi in zip(pts, q))
     errs = []
