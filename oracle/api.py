@@ -47,8 +47,9 @@ def lib():
         L.orc_plan_copy_tree.argtypes = [C.c_void_p, _ip, _ip, _ip, _dp, _dp, _dp, _dp]
         L.orc_plan_copy_lists.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip]
         L.orc_lists_from_geometry.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_int, _ip, _ip]
-        L.orc_evaluate.argtypes = [C.c_void_p, _dp, _bp, _dp, _dp]
-        L.orc_direct.argtypes = [_dp, _dp, C.c_int64, _ip, C.c_int64, _dp, _dp]
+        L.orc_evaluate.argtypes = [C.c_void_p, _dp, _bp, _dp, _dp, C.c_int]
+        L.orc_evaluate_adjoint.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int]
+        L.orc_direct.argtypes = [_dp, _dp, C.c_int64, _ip, C.c_int64, _dp, _dp, C.c_int]
         L.orc_num_threads.restype = C.c_int
         _i32p = C.POINTER(C.c_int)
         L.orc_plan_st_create.argtypes = [_dp, C.c_int64, _dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double]
@@ -57,8 +58,9 @@ def lib():
         L.orc_plan_st_info.argtypes = [C.c_void_p, C.c_int, _i32p] + [_ip] * 5 + [_i32p]
         L.orc_plan_st_copy_tree.argtypes = [C.c_void_p, C.c_int, _ip, _ip, _ip, _dp, _dp, _dp, _dp]
         L.orc_plan_st_copy_lists.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, _i32p]
-        L.orc_evaluate_st.argtypes = [C.c_void_p, _dp, _dp, _dp]
-        L.orc_direct_st.argtypes = [_dp, _dp, C.c_int64, _dp, C.c_int64, _dp, _dp]
+        L.orc_evaluate_st.argtypes = [C.c_void_p, _dp, _bp, _dp, _dp, C.c_int]
+        L.orc_evaluate_st_adjoint.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int]
+        L.orc_direct_st.argtypes = [_dp, _dp, C.c_int64, _dp, C.c_int64, _dp, _dp, C.c_int]
         _lib = L
     return _lib
 
@@ -168,9 +170,10 @@ class Plan:
         lib().orc_plan_copy_lists(self._h, _i(ls["weak_off"]), _i(ls["weak_src"]), _i(ls["strong_off"]), _i(ls["strong_src"]))
         return ls
 
-    def evaluate(self, q, leaf_mask=None, want_field=True):
+    def evaluate(self, q, leaf_mask=None, want_field=True, fp32_rule=False):
         """potential (N,), field (N,3) in input order.  With leaf_mask (n_leaves uint8) only the particles of
-        the masked leaves are written; the others are NaN."""
+        the masked leaves are written; the others are NaN.  fp32_rule: coincidence (reading S3) is decided in binary32,
+        as the fp32 CUDA kernels decide it (pairs with r^2 < FLT_MIN are skipped); for comparisons with fp32 plans."""
         q = np.ascontiguousarray(q, dtype=np.float64)
         assert q.shape == (self.N,)
         pot = np.full(self.N, np.nan)
@@ -179,8 +182,19 @@ class Plan:
         if leaf_mask is not None:
             m = np.ascontiguousarray(leaf_mask, dtype=np.uint8)
             assert m.shape == (self.n_leaves,)
-        lib().orc_evaluate(self._h, _d(q), m.ctypes.data_as(_bp) if m is not None else None, _d(pot), _d(fld))
+        lib().orc_evaluate(self._h, _d(q), m.ctypes.data_as(_bp) if m is not None else None, _d(pot), _d(fld), int(fp32_rule))
         return pot, fld
+
+    def evaluate_adjoint(self, ubar=None, fbar=None, fp32_rule=False):
+        """qbar (N,) = A^T ubar + F^T fbar: the vector-Jacobian product of evaluate() with respect to the charges
+        (PAPER.md:281-310), every step transposed.  ubar (N,) and / or fbar (N,3): cotangents of potential and field."""
+        ub = None if ubar is None else np.ascontiguousarray(ubar, dtype=np.float64)
+        fb = None if fbar is None else np.ascontiguousarray(fbar, dtype=np.float64)
+        assert ub is None or ub.shape == (self.N,)
+        assert fb is None or fb.shape == (self.N, 3)
+        qbar = np.empty(self.N)
+        lib().orc_evaluate_adjoint(self._h, _d(ub), _d(fb), _d(qbar), int(fp32_rule))
+        return qbar
 
 
 def lists_from_geometry(s, L, ctr, rad, theta, cross_level=0):
@@ -193,7 +207,7 @@ def lists_from_geometry(s, L, ctr, rad, theta, cross_level=0):
     return nw, ns
 
 
-def direct(pos, q, targets=None):
+def direct(pos, q, targets=None, fp32_rule=False):
     """Plain definition eqs. (1)-(3): u_i = -(1/4pi) sum_{j!=i} q_j/|r_i-r_j|, field = -grad u, at `targets`."""
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     q = np.ascontiguousarray(q, dtype=np.float64)
@@ -201,7 +215,7 @@ def direct(pos, q, targets=None):
     tg = np.arange(N, dtype=np.int64) if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
     pot = np.empty(tg.shape[0])
     fld = np.empty((tg.shape[0], 3))
-    lib().orc_direct(_d(pos), _d(q), N, _i(tg), tg.shape[0], _d(pot), _d(fld))
+    lib().orc_direct(_d(pos), _d(q), N, _i(tg), tg.shape[0], _d(pot), _d(fld), int(fp32_rule))
     return pot, fld
 
 
@@ -251,22 +265,37 @@ class PlanST:
         ls["steps"] = steps.reshape(-1, 2)
         return ls
 
-    def evaluate(self, q):
-        """potential (Nt,), field (Nt,3) at the targets, in target input order."""
+    def evaluate(self, q, leaf_mask=None, fp32_rule=False):
+        """potential (Nt,), field (Nt,3) at the targets, in target input order.  With leaf_mask (uint8 per target leaf) only
+        the targets of the masked leaves are written; the others are NaN."""
         q = np.ascontiguousarray(q, dtype=np.float64)
         assert q.shape == (self.Ns,)
-        pot = np.empty(self.Nt)
-        fld = np.empty((self.Nt, 3))
-        lib().orc_evaluate_st(self._h, _d(q), _d(pot), _d(fld))
+        pot = np.full(self.Nt, np.nan)
+        fld = np.full((self.Nt, 3), np.nan)
+        m = None
+        if leaf_mask is not None:
+            m = np.ascontiguousarray(leaf_mask, dtype=np.uint8)
+            assert m.shape == (self.info["tgt"]["n_leaves"],)
+        lib().orc_evaluate_st(self._h, _d(q), m.ctypes.data_as(_bp) if m is not None else None, _d(pot), _d(fld), int(fp32_rule))
         return pot, fld
 
+    def evaluate_adjoint(self, ubar=None, fbar=None, fp32_rule=False):
+        """qbar (Ns,) = A^T ubar + F^T fbar for cotangents ubar (Nt,), fbar (Nt,3) of the outputs of evaluate()."""
+        ub = None if ubar is None else np.ascontiguousarray(ubar, dtype=np.float64)
+        fb = None if fbar is None else np.ascontiguousarray(fbar, dtype=np.float64)
+        assert ub is None or ub.shape == (self.Nt,)
+        assert fb is None or fb.shape == (self.Nt, 3)
+        qbar = np.empty(self.Ns)
+        lib().orc_evaluate_st_adjoint(self._h, _d(ub), _d(fb), _d(qbar), int(fp32_rule))
+        return qbar
 
-def direct_st(src_pos, q, tgt_pos):
+
+def direct_st(src_pos, q, tgt_pos, fp32_rule=False):
     """Plain definition at separate targets: u(t_i) = -(1/4pi) sum_j q_j/|t_i - s_j|, field = -grad u."""
     sp = np.ascontiguousarray(src_pos, dtype=np.float64)
     tp = np.ascontiguousarray(tgt_pos, dtype=np.float64)
     q = np.ascontiguousarray(q, dtype=np.float64)
     pot = np.empty(tp.shape[0])
     fld = np.empty((tp.shape[0], 3))
-    lib().orc_direct_st(_d(sp), _d(q), sp.shape[0], _d(tp), tp.shape[0], _d(pot), _d(fld))
+    lib().orc_direct_st(_d(sp), _d(q), sp.shape[0], _d(tp), tp.shape[0], _d(pot), _d(fld), int(fp32_rule))
     return pot, fld

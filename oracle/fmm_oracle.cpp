@@ -20,6 +20,8 @@
 // the theta=0.7637 cube pin; whole FMM vs O(N^2) direct sum.
 // Cross-level (level-marching) lists: partition identity over all level pairs, symmetry of
 // the covered particle pairs, accuracy vs the O(N^2) sum and the count reduction against same-level lists.
+// Adjoint evaluate: dot-product identity against the forward evaluate to round-off, the plain definition
+// with sources and targets exchanged, symmetry of the single-set same-level operator (tests/test_oracle_adjoint.py).
 // "parity unpinned": the interaction counts of Table I -- the helix point set is not given.
 //
 // Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py)
@@ -27,6 +29,7 @@
 // m>=0 <-> real part, m<0 <-> imaginary part.
 // =====================================================================================
 #include <algorithm>
+#include <cfloat>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -383,7 +386,7 @@ struct Lists {
 //   cross_level = 1: one side at a time.  "Increase the level with the larger average box radius; if equal, increase the
 //     source level; if there are no more source levels, increase the target level".  Sources and targets
 //     share one hierarchy here, whose mean box radius shrinks from level to level, so the rule yields the fixed sequence
-//     (0,0), (1,0), (1,1), (2,1), ..., (L,L-1), (L,L): refine the sources, then the targets, alternately.
+//     (lt, ls) = (0,0), (0,1), (1,1), (1,2), ..., (L-1,L), (L,L): refine the sources, then the targets, alternately.
 // Pairs still failing at (L,L) are the strong leaf pairs (L3).
 void build_lists(const Tree& T, double theta, Lists& Ls, int cross_level = 0) {
     const int s = T.s, L = T.L;
@@ -438,13 +441,25 @@ struct Plan {
     Tree T; Lists Ls;
 };
 
+// Reading S3: a pair at zero distance contributes nothing (eq. (3) is singular there).  rule = 0: zero distance
+// means r^2 == 0 in fp64.  rule = 1 ("fp32 rule", used when the inputs are fp32 and the result is compared with the fp32 CUDA
+// path): the decision is taken in the kernel's precision -- r^2 is formed in IEEE binary32 exactly as the fp32 kernels form it,
+// fma(dz, dz, fma(dy, dy, dx*dx)) from the binary32 differences, and every pair with r^2 below FLT_MIN (the smallest normal
+// binary32 number; |r| < 1.08e-19) counts as coincident: its 1/r^3 is not representable in binary32 anyway.
+inline bool coincident(int rule, double dx, double dy, double dz) {
+    if (rule == 0) return dx * dx + dy * dy + dz * dz == 0.0;
+    const float fx = (float)dx, fy = (float)dy, fz = (float)dz;  // exact: differences of binary32 inputs that close are binary32 numbers
+    const float r2 = std::fmaf(fz, fz, std::fmaf(fy, fy, fx * fx));
+    return r2 < FLT_MIN;
+}
+
 // -------------------------------------------------------------------------------------
 // Evaluate, stage order PAPER.md:251; steps E1-E7 of DESIGN.md.  If leaf_mask != nullptr only
 // the leaves with mask != 0 get results (all other outputs are left untouched): local
 // expansions are then computed only for those leaves and their ancestors, with the
 // same arithmetic and order as the full run, so sampled outputs equal the full ones.
 // -------------------------------------------------------------------------------------
-void evaluate(const Plan& P, const double* q, const uint8_t* leaf_mask, double* pot, double* field) {
+void evaluate(const Plan& P, const double* q, const uint8_t* leaf_mask, double* pot, double* field, int rule = 0) {
     const Tree& T = P.T; const Lists& Ls = P.Ls;
     const int p = P.p, K = (p + 1) * (p + 1), s = T.s, L = T.L;
     const int64_t nb = T.level_off[L + 1], n_leaves = (int64_t)1 << (s * L), nch = (int64_t)1 << s;
@@ -536,8 +551,8 @@ void evaluate(const Plan& P, const double* q, const uint8_t* leaf_mask, double* 
                     const int64_t j = T.perm[kk];
                     if (j == i) continue;  // S3
                     const double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+                    if (coincident(rule, dx, dy, dz)) continue;  // S3: coincident points contribute nothing
                     const double r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 == 0.0) continue;  // S3: coincident points contribute nothing
                     const double r = std::sqrt(r2);
                     phi_near += q[j] / r;
                     const double f = q[j] / (r2 * r);
@@ -631,8 +646,9 @@ struct PlanST {
     std::vector<int> steps;
 };
 
-// potential and field at the targets from charges q at the sources; steps E1-E7 with the two hierarchies
-void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
+// potential and field at the targets from charges q at the sources; steps E1-E7 with the two hierarchies.  leaf_mask (target
+// leaves) works as in evaluate(): only the masked leaves get results, computed with the same arithmetic as in a full run.
+void evaluate_st(const PlanST& P, const double* q, const uint8_t* leaf_mask, double* pot, double* field, int rule = 0) {
     const Tree& Ts = P.Ts; const Tree& Tt = P.Tt; const Lists& Ls = P.Ls;
     const int p = P.p, K = (p + 1) * (p + 1), s = Ts.s;
     const int64_t nch = (int64_t)1 << s;
@@ -641,6 +657,13 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
     const int64_t sleaf0 = Ts.level_off[Ts.L], tleaf0 = Tt.level_off[Tt.L];
     const double* spos = P.spos.data(); const double* tpos = P.tpos.data();
     std::vector<double> C((size_t)nbs * K, 0.0), D((size_t)nbt * K, 0.0);
+    std::vector<uint8_t> need(nbt, leaf_mask ? 0 : 1);
+    if (leaf_mask) {
+        for (int64_t t = 0; t < n_tleaves; ++t) if (leaf_mask[t]) need[tleaf0 + t] = 1;
+        for (int l = Tt.L; l >= 1; --l)
+            for (int64_t b = 0; b < ((int64_t)1 << (s * l)); ++b)
+                if (need[Tt.level_off[l] + b]) need[Tt.level_off[l - 1] + b / nch] = 1;
+    }
     // E1: P2M at the source leaves, eq. (13)
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t t = 0; t < n_sleaves; ++t) {
@@ -671,6 +694,7 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
     // E3: M2L over the weak list; b = source centre - target centre
 #pragma omp parallel for schedule(dynamic, 4)
     for (int64_t gt = 0; gt < nbt; ++gt) {
+        if (!need[gt]) continue;
         std::vector<double> tmp(K);
         for (int64_t e = Ls.weak_off[gt]; e < Ls.weak_off[gt + 1]; ++e) {
             const int64_t gs = Ls.weak_src[e];
@@ -685,7 +709,7 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
 #pragma omp parallel for schedule(dynamic, 16)
         for (int64_t bc = 0; bc < nbl; ++bc) {
             const int64_t gc = Tt.level_off[l] + bc, gp = Tt.level_off[l - 1] + bc / nch;
-            if (Tt.box_count[gc] == 0) continue;
+            if (!need[gc] || Tt.box_count[gc] == 0) continue;
             std::vector<double> tmp(K);
             const double b[3] = {Tt.ctr[3 * gp] - Tt.ctr[3 * gc], Tt.ctr[3 * gp + 1] - Tt.ctr[3 * gc + 1], Tt.ctr[3 * gp + 2] - Tt.ctr[3 * gc + 2]};
             translate(2, p, &D[(size_t)gp * K], b, tmp.data());
@@ -696,6 +720,7 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
     const double inv4pi = 1.0 / (4.0 * M_PI);
 #pragma omp parallel for schedule(dynamic, 4)
     for (int64_t t = 0; t < n_tleaves; ++t) {
+        if (leaf_mask && !leaf_mask[t]) continue;
         const int64_t g = tleaf0 + t;
         std::vector<double> R(K), G(3 * K);
         for (int64_t k = Tt.box_start[g]; k < Tt.box_start[g] + Tt.box_count[g]; ++k) {
@@ -716,8 +741,8 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
                 for (int64_t kk = Ts.box_start[gs]; kk < Ts.box_start[gs] + Ts.box_count[gs]; ++kk) {
                     const int64_t j = Ts.perm[kk];
                     const double dx = tpos[3 * i] - spos[3 * j], dy = tpos[3 * i + 1] - spos[3 * j + 1], dz = tpos[3 * i + 2] - spos[3 * j + 2];
+                    if (coincident(rule, dx, dy, dz)) continue;  // S3
                     const double r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 == 0.0) continue;  // S3
                     const double r = std::sqrt(r2);
                     phi_near += q[j] / r;
                     const double f = q[j] / (r2 * r);
@@ -726,6 +751,133 @@ void evaluate_st(const PlanST& P, const double* q, double* pot, double* field) {
             }
             if (pot) pot[i] = -(phi_far + phi_near) * inv4pi;
             if (field) for (int c = 0; c < 3; ++c) field[3 * i + c] = (gfar[c] + gnear[c]) * inv4pi;
+        }
+    }
+}
+
+
+// -------------------------------------------------------------------------------------
+// Adjoint evaluate.  The paper differentiates eval_potential with respect to the charges by JAX autodiff;
+// the evaluate is linear in q -- potential = A q, field = F q with the FMM operators A, F of evaluate() / evaluate_st() -- so the
+// vector-Jacobian product autodiff returns for cotangents (ubar, fbar) is  qbar = A^T ubar + F^T fbar:  every step E1-E7
+// transposed and run in reverse order.  Nothing clever: the transposed translation operators are formed literally, column k of
+// T = translate(e_k), and applied as T^T x.  Tt / tpos: hierarchy and points of the targets, Ts / spos: of the sources (the same
+// objects for a single point set, where the pair i == j is excluded as in evaluate()).
+// -------------------------------------------------------------------------------------
+void translate_transposed(int kind, int p, const double* in, const double b[3], double* out) {
+    const int K = (p + 1) * (p + 1);
+    std::vector<double> e(K, 0.0), col(K);
+    for (int k = 0; k < K; ++k) {
+        e[k] = 1.0;
+        translate(kind, p, e.data(), b, col.data());  // column k of T
+        e[k] = 0.0;
+        double acc = 0.0;
+        for (int c = 0; c < K; ++c) acc += col[c] * in[c];
+        out[k] = acc;  // (T^T in)_k = sum_c T[c][k] in[c]
+    }
+}
+
+void adjoint_impl(int p, const Tree& Tt, const double* tpos, const Tree& Ts, const double* spos, const Lists& Ls, bool same_set,
+                  const double* ubar, const double* fbar, double* qbar, int rule) {
+    const int K = (p + 1) * (p + 1), s = Ts.s;
+    const int64_t nch = (int64_t)1 << s;
+    const int64_t nbs = Ts.level_off[Ts.L + 1], nbt = Tt.level_off[Tt.L + 1];
+    const int64_t n_sleaves = (int64_t)1 << (s * Ts.L), n_tleaves = (int64_t)1 << (s * Tt.L);
+    const int64_t sleaf0 = Ts.level_off[Ts.L], tleaf0 = Tt.level_off[Tt.L];
+    const int64_t Ns = (int64_t)Ts.perm.size();
+    const double inv4pi = 1.0 / (4.0 * M_PI);
+    std::vector<double> Cbar((size_t)nbs * K, 0.0), Dbar((size_t)nbt * K, 0.0);
+    for (int64_t j = 0; j < Ns; ++j) qbar[j] = 0.0;
+    // E7^T: u = -(phi_far + phi_near)/4pi, field = (g_far + g_near)/4pi  =>  phibar = -ubar/4pi, gbar = fbar/4pi (both parts)
+    // E6^T (P2P) and E5^T (L2P), target leaf by target leaf (serial: the P2P part scatters into the sources)
+    for (int64_t t = 0; t < n_tleaves; ++t) {
+        const int64_t g = tleaf0 + t;
+        std::vector<double> R(K), G(3 * K);
+        for (int64_t k = Tt.box_start[g]; k < Tt.box_start[g] + Tt.box_count[g]; ++k) {
+            const int64_t i = Tt.perm[k];
+            const double phibar = ubar ? -ubar[i] * inv4pi : 0.0;
+            const double gbar[3] = {fbar ? fbar[3 * i] * inv4pi : 0.0, fbar ? fbar[3 * i + 1] * inv4pi : 0.0, fbar ? fbar[3 * i + 2] * inv4pi : 0.0};
+            const double x = tpos[3 * i] - Tt.ctr[3 * g], y = tpos[3 * i + 1] - Tt.ctr[3 * g + 1], z = tpos[3 * i + 2] - Tt.ctr[3 * g + 2];
+            regular_basis(p, x, y, z, R.data());
+            regular_grad(p, x, y, z, R.data(), G.data());
+            // E5^T: phi_far = sum w D R, g_far = sum w D G   =>   Dbar += w (phibar R + gbar . G)
+            for (int n = 0; n <= p; ++n)
+                for (int m = -n; m <= n; ++m) {
+                    const double w = ((m == 0) ? 1.0 : 2.0) * sgn(m);
+                    const int c = IDX(n, m);
+                    Dbar[(size_t)g * K + c] += w * (phibar * R[c] + gbar[0] * G[3 * c] + gbar[1] * G[3 * c + 1] + gbar[2] * G[3 * c + 2]);
+                }
+            // E6^T: phi_near += q_j / r, g_near -= q_j d / r^3   =>   qbar_j += phibar / r - (gbar . d) / r^3
+            for (int64_t e = Ls.strong_off[t]; e < Ls.strong_off[t + 1]; ++e) {
+                const int64_t gs = sleaf0 + Ls.strong_src[e];
+                for (int64_t kk = Ts.box_start[gs]; kk < Ts.box_start[gs] + Ts.box_count[gs]; ++kk) {
+                    const int64_t j = Ts.perm[kk];
+                    if (same_set && j == i) continue;  // S3
+                    const double dx = tpos[3 * i] - spos[3 * j], dy = tpos[3 * i + 1] - spos[3 * j + 1], dz = tpos[3 * i + 2] - spos[3 * j + 2];
+                    if (coincident(rule, dx, dy, dz)) continue;  // S3
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    const double r = std::sqrt(r2);
+                    qbar[j] += phibar / r - (gbar[0] * dx + gbar[1] * dy + gbar[2] * dz) / (r2 * r);
+                }
+            }
+        }
+    }
+    // E4^T: D_child += T_L2L(b = parent - child) D_parent for l = 1..L   =>   Dbar_parent += T^T Dbar_child, l = L..1
+    for (int l = Tt.L; l >= 1; --l) {
+        const int64_t nbp = (int64_t)1 << (s * (l - 1));
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t bp = 0; bp < nbp; ++bp) {
+            const int64_t gp = Tt.level_off[l - 1] + bp;
+            std::vector<double> tmp(K);
+            for (int64_t j = 0; j < nch; ++j) {
+                const int64_t gc = Tt.level_off[l] + bp * nch + j;
+                if (Tt.box_count[gc] == 0) continue;
+                const double b[3] = {Tt.ctr[3 * gp] - Tt.ctr[3 * gc], Tt.ctr[3 * gp + 1] - Tt.ctr[3 * gc + 1], Tt.ctr[3 * gp + 2] - Tt.ctr[3 * gc + 2]};
+                translate_transposed(2, p, &Dbar[(size_t)gc * K], b, tmp.data());
+                for (int c = 0; c < K; ++c) Dbar[(size_t)gp * K + c] += tmp[c];
+            }
+        }
+    }
+    // E3^T: D_t += T_M2L(b = c_s - c_t) C_s over the weak list   =>   Cbar_s += T^T Dbar_t.  Rows of the transposed list (by
+    // source box) are independent, so the loop runs over sources; targets of a source in ascending order.
+    {
+        std::vector<std::vector<int64_t>> by_src(nbs);
+        for (int64_t gt = 0; gt < nbt; ++gt)
+            for (int64_t e = Ls.weak_off[gt]; e < Ls.weak_off[gt + 1]; ++e) by_src[Ls.weak_src[e]].push_back(gt);
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t gs = 0; gs < nbs; ++gs) {
+            std::vector<double> tmp(K);
+            for (int64_t gt : by_src[gs]) {
+                const double b[3] = {Ts.ctr[3 * gs] - Tt.ctr[3 * gt], Ts.ctr[3 * gs + 1] - Tt.ctr[3 * gt + 1], Ts.ctr[3 * gs + 2] - Tt.ctr[3 * gt + 2]};
+                translate_transposed(1, p, &Dbar[(size_t)gt * K], b, tmp.data());
+                for (int c = 0; c < K; ++c) Cbar[(size_t)gs * K + c] += tmp[c];
+            }
+        }
+    }
+    // E2^T: C_parent += T_M2M(b = child - parent) C_child for l = L..1   =>   Cbar_child += T^T Cbar_parent, l = 1..L
+    for (int l = 1; l <= Ts.L; ++l) {
+        const int64_t nbl = (int64_t)1 << (s * l);
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t bc = 0; bc < nbl; ++bc) {
+            const int64_t gc = Ts.level_off[l] + bc, gp = Ts.level_off[l - 1] + bc / nch;
+            if (Ts.box_count[gc] == 0) continue;
+            std::vector<double> tmp(K);
+            const double b[3] = {Ts.ctr[3 * gc] - Ts.ctr[3 * gp], Ts.ctr[3 * gc + 1] - Ts.ctr[3 * gp + 1], Ts.ctr[3 * gc + 2] - Ts.ctr[3 * gp + 2]};
+            translate_transposed(0, p, &Cbar[(size_t)gp * K], b, tmp.data());
+            for (int c = 0; c < K; ++c) Cbar[(size_t)gc * K + c] += tmp[c];
+        }
+    }
+    // E1^T: C_leaf += q_i R^(r_i - c)   =>   qbar_i += sum_c Cbar_leaf[c] R^_c(r_i - c)
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < n_sleaves; ++t) {
+        const int64_t g = sleaf0 + t;
+        std::vector<double> R(K);
+        for (int64_t k = Ts.box_start[g]; k < Ts.box_start[g] + Ts.box_count[g]; ++k) {
+            const int64_t i = Ts.perm[k];
+            regular_basis(p, spos[3 * i] - Ts.ctr[3 * g], spos[3 * i + 1] - Ts.ctr[3 * g + 1], spos[3 * i + 2] - Ts.ctr[3 * g + 2], R.data());
+            double acc = 0.0;
+            for (int c = 0; c < K; ++c) acc += Cbar[(size_t)g * K + c] * R[c];
+            qbar[i] += acc;
         }
     }
 }
@@ -805,12 +957,17 @@ void orc_lists_from_geometry(int s, int L, const double* ctr, const double* rad,
     const int64_t nl = (int64_t)1 << (s * L);
     for (int64_t t = 0; t < nl; ++t) n_strong_per_leaf[t] = Ls.strong_off[t + 1] - Ls.strong_off[t];
 }
-void orc_evaluate(void* h, const double* q, const uint8_t* leaf_mask, double* pot, double* field) {
-    evaluate(*(Plan*)h, q, leaf_mask, pot, field);
+void orc_evaluate(void* h, const double* q, const uint8_t* leaf_mask, double* pot, double* field, int rule) {
+    evaluate(*(Plan*)h, q, leaf_mask, pot, field, rule);
+}
+// qbar (N) = A^T ubar + F^T fbar for the FMM operators of orc_evaluate (ubar: N or NULL, fbar: N x 3 or NULL)
+void orc_evaluate_adjoint(void* h, const double* ubar, const double* fbar, double* qbar, int rule) {
+    Plan* P = (Plan*)h;
+    adjoint_impl(P->p, P->T, P->pos.data(), P->T, P->pos.data(), P->Ls, true, ubar, fbar, qbar, rule);
 }
 // plain definition, eqs. (1)-(3) PAPER.md:19-28: u_i = -(1/4pi) sum_{j != i} q_j/|r_i - r_j|, field = -grad u;
 // evaluated at the targets listed in tgt (indices into pos), against all N sources.
-void orc_direct(const double* pos, const double* q, int64_t N, const int64_t* tgt, int64_t n_tgt, double* pot, double* field) {
+void orc_direct(const double* pos, const double* q, int64_t N, const int64_t* tgt, int64_t n_tgt, double* pot, double* field, int rule) {
     const double inv4pi = 1.0 / (4.0 * M_PI);
 #pragma omp parallel for schedule(static)
     for (int64_t a = 0; a < n_tgt; ++a) {
@@ -819,8 +976,8 @@ void orc_direct(const double* pos, const double* q, int64_t N, const int64_t* tg
         for (int64_t j = 0; j < N; ++j) {
             if (j == i) continue;
             const double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+            if (coincident(rule, dx, dy, dz)) continue;
             const double r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 == 0.0) continue;
             const double r = std::sqrt(r2);
             ph += q[j] / r;
             const double f = q[j] / (r2 * r);
@@ -873,17 +1030,24 @@ void orc_plan_st_copy_lists(void* h, int64_t* weak_off, int64_t* weak_src, int64
     if (strong_src) std::copy(Ls.strong_src.begin(), Ls.strong_src.end(), strong_src);
     if (steps) std::copy(P->steps.begin(), P->steps.end(), steps);
 }
-void orc_evaluate_st(void* h, const double* q, double* pot, double* field) { evaluate_st(*(PlanST*)h, q, pot, field); }
+void orc_evaluate_st(void* h, const double* q, const uint8_t* leaf_mask, double* pot, double* field, int rule) {
+    evaluate_st(*(PlanST*)h, q, leaf_mask, pot, field, rule);
+}
+// qbar (Ns) = A^T ubar + F^T fbar for the operators of orc_evaluate_st (ubar: Nt or NULL, fbar: Nt x 3 or NULL)
+void orc_evaluate_st_adjoint(void* h, const double* ubar, const double* fbar, double* qbar, int rule) {
+    PlanST* P = (PlanST*)h;
+    adjoint_impl(P->p, P->Tt, P->tpos.data(), P->Ts, P->spos.data(), P->Ls, false, ubar, fbar, qbar, rule);
+}
 // plain definition at separate targets: u(t_i) = -(1/4pi) sum_j q_j/|t_i - s_j|, field = -grad u; zero-distance pairs skipped (S3)
-void orc_direct_st(const double* spos, const double* q, int64_t Ns, const double* tpos, int64_t Nt, double* pot, double* field) {
+void orc_direct_st(const double* spos, const double* q, int64_t Ns, const double* tpos, int64_t Nt, double* pot, double* field, int rule) {
     const double inv4pi = 1.0 / (4.0 * M_PI);
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < Nt; ++i) {
         double ph = 0.0, g[3] = {0, 0, 0};
         for (int64_t j = 0; j < Ns; ++j) {
             const double dx = tpos[3 * i] - spos[3 * j], dy = tpos[3 * i + 1] - spos[3 * j + 1], dz = tpos[3 * i + 2] - spos[3 * j + 2];
+            if (coincident(rule, dx, dy, dz)) continue;
             const double r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 == 0.0) continue;
             const double r = std::sqrt(r2);
             ph += q[j] / r;
             const double f = q[j] / (r2 * r);

@@ -138,3 +138,32 @@ def test_accuracy_order_of_paper_set1(golden_dir):
     ud, _ = O.direct(pos, q)
     err = np.max(np.abs(u - ud)) / np.max(np.abs(ud))
     assert vals["set1_err_cube"] / 30 < err < vals["set1_err_cube"] * 3
+
+
+def test_p2p_pair_count_is_the_sum_over_the_strong_list():
+    """orc_plan_info's n_p2p_pairs (used for the P2P roofline accounting): recomputed here from the copied lists and tree."""
+    pos, _ = inputs.gaussian_clusters(6000, 8)
+    for cross in (0, 1):
+        P = O.Plan(pos, 4, 24, 3, 0.77, cross_level=cross)
+        t, ls = P.tree(), P.lists()
+        leaf0 = P.n_boxes - P.n_leaves
+        cnt = t["box_count"][leaf0:]
+        want = sum(int(cnt[a]) * int(cnt[ls["strong_src"][ls["strong_off"][a]:ls["strong_off"][a + 1]]].sum()) for a in range(P.n_leaves))
+        assert P.n_p2p_pairs == want
+
+
+def test_fp32_coincidence_rule():
+    """Reading S3 for fp32 plans: the zero-distance decision is taken in binary32 (r^2 < FLT_MIN counts as coincident).  Distinct
+    points 1e-23 apart: the fp64 rule sums 1/r = 1e23, the fp32 rule skips the pair; well separated points are unaffected."""
+    pos = np.array([[0.0, 0.0, 0.0], [1e-23, 0.0, 0.0], [0.5, 0.25, 0.125], [0.5, 0.25, 0.125 + 2e-19]], dtype=np.float32).astype(np.float64)
+    q = np.array([1.0, 2.0, -1.0, 3.0])
+    u64, _ = O.direct(pos, q)
+    u32, f32 = O.direct(pos, q, fp32_rule=True)
+    assert abs(u64[0]) > 1e21 and abs(u32[0]) < 10 and np.all(np.isfinite(f32))
+    # points 2 and 3 are 2e-19 apart in z only after rounding to binary32?  0.125 + 2e-19 rounds to 0.125: truly coincident under both rules
+    assert pos[2, 2] == pos[3, 2] and abs(u64[2]) < 10
+    far, qq = inputs.uniform_cube(50, 9, np.float32)
+    a, b = O.direct(far, qq), O.direct(far, qq, fp32_rule=True)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    P = O.Plan(pos, 3, 2, 1, 0.77)
+    assert abs(P.evaluate(q, fp32_rule=True)[0][0]) < 10 and abs(P.evaluate(q)[0][0]) > 1e21

@@ -94,18 +94,46 @@ def test_march_follows_the_mean_radius_rule_and_partitions_all_leaf_pairs(Ns, Nt
             assert not any(_adm(tt, anc_t(a, lt), ts, anc_s(b, lsrc), theta) for (lt, lsrc) in steps[:hits[0]])
 
 
-def test_identical_sets_reduce_to_the_single_hierarchy_cross_level_lists():
+@pytest.mark.parametrize("N,N_max,s", [(3000, 32, 2), (37, 1, 2), (150, 1, 3), (9, 1, 1)])
+def test_identical_sets_reduce_to_the_single_hierarchy_cross_level_lists(N, N_max, s):
     """Sources == targets: both hierarchies coincide, mean radii tie on equal levels (-> source first), so the march is the fixed
-    sequence of the single-hierarchy cross-level plan and lists and results must be identical."""
-    pos, q = inputs.uniform_cube(3000, 5)
-    P1 = O.Plan(pos, 5, 32, 2, 0.77, cross_level=1)
-    P2 = O.PlanST(pos, pos, 5, 32, 2, 0.77)
+    sequence (l_trg, l_src) = (0,0), (0,1), (1,1), (1,2), ... of the single-hierarchy cross-level plan and lists and results must
+    be identical -- also on ragged trees (N < 2^(sL): empty boxes, levels whose mean radius is taken over the non-empty boxes only)."""
+    pos, q = inputs.uniform_cube(N, 5)
+    P1 = O.Plan(pos, 5, N_max, s, 0.77, cross_level=1)
+    P2 = O.PlanST(pos, pos, 5, N_max, s, 0.77)
+    assert N_max > 1 or N < 2 ** (s * P1.L)  # the small cases are ragged
     l1, l2 = P1.lists(), P2.lists()
     for k in ("weak_off", "weak_src", "strong_off", "strong_src"):
         assert np.array_equal(l1[k], l2[k])
+    want = [(0, 0)]
+    while want[-1] != (P1.L, P1.L):
+        lt, ls = want[-1]
+        want.append((lt, ls + 1) if lt == ls else (lt + 1, ls))
+    assert [tuple(x) for x in l2["steps"]] == want
     u1, f1 = P1.evaluate(q)
     u2, f2 = P2.evaluate(q)
+    # the single-set evaluate skips the pair i == j by index, the two-set evaluate by distance: same terms, same order
     assert np.array_equal(u1, u2) and np.array_equal(f1, f2)
+
+
+def test_masked_evaluation_st_equals_full():
+    """leaf mask of evaluate_st (used by the full-size GPU parity tests): the masked target leaves get bit-for-bit the values of a
+    full run, every other target stays untouched."""
+    sp, q = inputs.uniform_cube(3000, 61)
+    tp = _targets(2200, 62)
+    P = O.PlanST(sp, tp, 6, 16, 2, 0.77)
+    u, f = P.evaluate(q)
+    nl = P.info["tgt"]["n_leaves"]
+    mask = np.zeros(nl, np.uint8)
+    mask[np.random.default_rng(3).choice(nl, 9, replace=False)] = 1
+    um, fm = P.evaluate(q, leaf_mask=mask)
+    t = P.tree("tgt")
+    off = _offsets(2, P.info["tgt"]["L"])[P.info["tgt"]["L"]]
+    sel = np.concatenate([t["perm"][t["box_start"][off + l]: t["box_start"][off + l] + t["box_count"][off + l]] for l in np.flatnonzero(mask)])
+    assert sel.size > 0 and np.array_equal(um[sel], u[sel]) and np.array_equal(fm[sel], f[sel])
+    rest = np.setdiff1d(np.arange(tp.shape[0]), sel)
+    assert np.all(np.isnan(um[rest])) and np.all(np.isnan(fm[rest]))
 
 
 @pytest.mark.parametrize("Ns,Nt,N_max,s", [(3000, 2000, 32, 2), (1024, 4096, 16, 3)])
