@@ -163,6 +163,13 @@ fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial);
  * concurrent schedule with the register kernels), P2P, L2P (which also finalizes).  cudaMemset nodes are not counted. */
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h_launches_per_evaluate);
 
+/* Floating-point instructions that ONE translation executes in the kernels selected for (p, dtype) with m2l_variant 0
+ * (HOST outputs, any may be NULL): fused multiply-adds, multiplies, adds of the rotate / z-shift / rotate-back operator
+ * (App. B) in the factorised form of DESIGN.md section 5 -- geometry, addressing, staging and the sums over equal
+ * targets are not counted.  kind: 0 = M2M, 1 = M2L, 2 = L2L.  All zero where only the generic kernels exist (p = 0, p > 12).
+ * This is the per-unit work behind bench.py's roofline line: executed flop = 2 * fma + mul + add.  No device needed. */
+fmm_status fmm_translation_work(int p, fmm_dtype dtype, int kind, int64_t* h_fma, int64_t* h_mul, int64_t* h_add);
+
 /* Thread-local, NUL-terminated description of the last failure on the calling thread ("" if none). */
 const char* fmm_last_error(void);
 

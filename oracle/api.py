@@ -51,6 +51,7 @@ def lib():
         L.orc_evaluate_adjoint.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int]
         L.orc_direct.argtypes = [_dp, _dp, C.c_int64, _ip, C.c_int64, _dp, _dp, C.c_int]
         L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
         _i32p = C.POINTER(C.c_int)
         L.orc_plan_st_create.argtypes = [_dp, C.c_int64, _dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double]
         L.orc_plan_st_create.restype = C.c_void_p
@@ -133,6 +134,11 @@ def tree_depth(N, N_max, s):
 
 def num_threads():
     return lib().orc_num_threads()
+
+
+def set_num_threads(n):
+    """OpenMP threads of the following oracle calls (n < 1: all processors).  Timing control only -- results do not depend on it."""
+    lib().orc_set_num_threads(int(n))
 
 
 class Plan:

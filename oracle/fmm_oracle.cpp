@@ -1057,6 +1057,14 @@ void orc_direct_st(const double* spos, const double* q, int64_t Ns, const double
         if (field) for (int c = 0; c < 3; ++c) field[3 * i + c] = g[c] * inv4pi;
     }
 }
+// number of OpenMP threads used by the following calls (bench.py's one-thread cpu_baseline leg); n < 1 restores the default
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    omp_set_num_threads(n >= 1 ? n : omp_get_num_procs());
+#else
+    (void)n;
+#endif
+}
 int orc_num_threads() {
     int n = 1;
 #ifdef _OPENMP

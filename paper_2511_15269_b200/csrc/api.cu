@@ -152,6 +152,7 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
             FMM_CUDA_CHECK(cudaEventRecord(e0, st));
             build_tree(P, d_positions, st);
             build_lists(P, st);
+            if (m2l_geo_wanted(p, dtype) && P.n_weak > 0) m2l_geo_prepare(P, st);
             const size_t es = esize(dtype);
             P.pq.alloc((size_t)N * 4 * es);
             P.near.alloc((size_t)N * 4 * es);
@@ -217,6 +218,7 @@ fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void
             build_tree(P, d_targets, st);
             P.plan_ms[0] += sort_s; P.plan_ms[1] += tree_s;
             build_lists(P, st);
+            if (m2l_geo_wanted(p, dtype) && P.n_weak > 0) m2l_geo_prepare(P, st);
             const size_t es = esize(dtype);
             S.pq.alloc((size_t)Ns * 4 * es);
             S.Mc.alloc((size_t)S.n_boxes * S.Kp * es);
@@ -385,6 +387,16 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms) {
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h) {
     if (!plan || !h) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
     *h = evaluate_launches(plan->P);
+    return FMM_OK;
+}
+
+fmm_status fmm_translation_work(int p, fmm_dtype dtype, int kind, int64_t* h_fma, int64_t* h_mul, int64_t* h_add) {
+    if (p < 0 || p > PMAX || kind < 0 || kind > 2 || (dtype != FMM_F32 && dtype != FMM_F64)) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    int64_t w[3];
+    xlate_work(p, dtype, kind, w);
+    if (h_fma) *h_fma = w[0];
+    if (h_mul) *h_mul = w[1];
+    if (h_add) *h_add = w[2];
     return FMM_OK;
 }
 

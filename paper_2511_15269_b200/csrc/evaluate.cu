@@ -26,6 +26,10 @@ template <typename T> __device__ inline T rsqrt_t(T x);
 template <> __device__ inline float rsqrt_t<float>(float x) { return rsqrtf(x); }
 template <> __device__ inline double rsqrt_t<double>(double x) { return rsqrt(x); }
 
+template <typename T> __device__ inline T r2_min();
+template <> __device__ inline float r2_min<float>() { return 1.17549435e-38f; }  // FLT_MIN
+template <> __device__ inline double r2_min<double>() { return 4.9406564584124654e-324; }  // any r^2 > 0
+
 inline unsigned nblocks(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
 
 // ------------------------------------------------------------------------------------------------ permute (a3)
@@ -501,9 +505,11 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
 #pragma unroll
                 for (int t = 0; t < P2P_TPT; ++t) {
                     const T dx = tx[t] - sv.x, dy = ty[t] - sv.y, dz = tz[t] - sv.z;
-                    const T r2 = dx * dx + dy * dy + dz * dz;
+                    const T r2 = fma(dz, dz, fma(dy, dy, dx * dx));  // the same order as the packed kernel (p2p_fast.cu)
                     T inv = rsqrt_t<T>(r2);
-                    inv = (r2 > T(0)) ? inv : T(0);  // S3: self / coincident pairs contribute nothing
+                    // S3: self / coincident pairs contribute nothing; in fp32 every pair with r^2 below the smallest normal number
+                    // counts as coincident (its 1/r^3 is not representable), in fp64 only r^2 == 0
+                    inv = (r2 >= r2_min<T>()) ? inv : T(0);
                     const T inv2 = inv * inv;
                     const T q3 = sv.w * inv * inv2;
                     ph[t] += sv.w * inv;

@@ -154,6 +154,8 @@ struct Plan {
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
+    DevBuf<float> m2l_geo;   // xlate_fast.cu: per batch of 32 weak pairs a 1 KB geometry record (fp32, p <= 8)
+    int64_t m2l_seg_e0[2] = {0, 0}, m2l_seg_rec[2] = {0, 0};  // the two segments of the weak list the records are batched by: first pair, first record
     DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
     int64_t n_p2p_items = 0;
     bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
@@ -185,10 +187,13 @@ int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evalua
 // xlate_fast.cu: register kernels (one thread per translation).  kind 0 = M2M into level-1 from `level`, 1 = M2L (all
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
 bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
+void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]);  // {FMA, MUL, ADD} instructions of one translation (0 if generic only)
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0 = 0, int64_t e1 = -1);  // kind 1: weak pairs [e0, e1)
 // xlate_smem.cu: the same three operators for 9 <= p <= 12, one thread per translation with the state vector in shared memory
 bool xlate_smem_available(int p, fmm_dtype dt);
 void xlate_smem_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1);
+bool m2l_geo_wanted(int p, fmm_dtype dt);        // fp32, p <= 8: the M2L kernel reads per-pair geometry records
+void m2l_geo_prepare(Plan& P, cudaStream_t st);  // plan time, after build_lists: writes Plan::m2l_geo
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
 void p2p_fast_launch(const Plan& P, cudaStream_t st, bool want_field);  // want_field = false: potential only (cheaper inner loop)
 void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field);  // fp64: same mapping, scalar DFMA arithmetic, sources read through L1

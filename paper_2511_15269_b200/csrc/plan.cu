@@ -424,8 +424,8 @@ __global__ void expand_offsets_k(ExpandArgs A, const unsigned long long* S, int6
     foff2[t] = (int64_t)(sv >> 32);
 }
 
-// strong_touch[e] = 1 iff the tight bounding boxes of the target leaf and the source leaf of entry e touch or overlap (exact
-// comparisons in the plan's dtype): only then can a target coincide with a source (reading S3)
+// strong_touch[e] = 1 iff the tight bounding boxes of the target leaf and the source leaf of entry e touch or overlap (comparisons
+// in the plan's dtype): only then can a target coincide with a source (reading S3)
 template <typename T>
 __global__ void strong_touch_k(const int64_t* soff, const int32_t* ssrc, const T* tlo, const T* thi, const T* slo, const T* shi, int64_t n_leaves, uint8_t* touch) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -433,7 +433,11 @@ __global__ void strong_touch_k(const int64_t* soff, const int32_t* ssrc, const T
     const T a0 = tlo[3 * t], a1 = tlo[3 * t + 1], a2 = tlo[3 * t + 2], b0 = thi[3 * t], b1 = thi[3 * t + 1], b2 = thi[3 * t + 2];
     for (int64_t e = soff[t]; e < soff[t + 1]; ++e) {
         const int64_t s = ssrc[e];
-        const bool hit = a0 <= shi[3 * s] && slo[3 * s] <= b0 && a1 <= shi[3 * s + 1] && slo[3 * s + 1] <= b1 && a2 <= shi[3 * s + 2] && slo[3 * s + 2] <= b2;
+        // fp32: pairs with r^2 < FLT_MIN count as coincident (reading S3), so boxes closer than sqrt(FLT_MIN) ~ 1.08e-19 along every
+        // axis are flagged as well (tol is conservative); fp64: exact comparisons
+        const T tol = sizeof(T) == 4 ? (T)2e-19 : (T)0;
+        const bool hit = a0 - shi[3 * s] <= tol && slo[3 * s] - b0 <= tol && a1 - shi[3 * s + 1] <= tol && slo[3 * s + 1] - b1 <= tol &&
+                         a2 - shi[3 * s + 2] <= tol && slo[3 * s + 2] - b2 <= tol;
         touch[e] = hit ? 1 : 0;
     }
 }

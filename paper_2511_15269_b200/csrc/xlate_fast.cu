@@ -57,11 +57,15 @@ struct XArgs {
     const void* scale_s;          //     a source hierarchy to a separate target hierarchy)
     const void* in;
     void* out;
+    const float* geo;             // KIND 1, GEO kernels: geometry records of the pairs (m2l_geo_prepare), 1 KB per batch of 32
 };
 
-// XW warps per CTA; SYNC = lockstep barriers (all warps then run the operator, also on padding lanes)
-template <typename T, int P, int KIND, int XW, bool SYNC>
+// XW warps per CTA; GEO (fp32 M2L only): target ids and the geometry of every pair (cos / sin of the two angles, 1/r, scale ratios)
+// come from records written at plan time (m2l_geo_prepare) -- one coalesced load per word instead of a gather of fp64 centres
+// that depends on the ids, and no square roots or divisions in the kernel
+template <typename T, int P, int KIND, int XW, bool GEO>
 __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (XW == 4 ? 4 : 1))) xlate_fast_k(XArgs a) {
+    constexpr bool SYNC = false;
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -69,7 +73,15 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
     V* sm = reinterpret_cast<V*>(smraw) + (size_t)warp * 32 * G::KSB;
     const int64_t e = ((int64_t)blockIdx.x * XW + warp) * 32 + lane;
     int gs = -1, gt = -1;
-    if (e < a.n) {
+    float rec[7];  // GEO: ct, st, cp, sp, 1/r, x1, x2
+    if constexpr (GEO) {
+        // the record block of this warp's batch: word w of pair `lane` at rec[w * 32 + lane]; padding pairs carry gt = -1
+        const float* r = a.geo + (e >> 5) * 256 + lane;
+#pragma unroll
+        for (int w = 0; w < 7; ++w) rec[w] = r[32 * w];
+        gt = reinterpret_cast<const int*>(r)[224];
+        if (e < a.n) gs = a.src[e];
+    } else if (e < a.n) {
         if constexpr (KIND == 1) { gs = a.src[e]; gt = a.tgt[e]; }
         else {
             const int64_t gc = a.off_child + e, gp = a.off_parent + (e >> a.s);
@@ -107,7 +119,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
     }
     if (lane == 0) mbar_expect_tx(bar, (uint32_t)__popc(vmask) * ROWB);
     T bx = T(0), by = T(0), bz = T(1), a_old = T(1), a_new = T(1);
-    if (gs >= 0) {
+    if (!GEO && gs >= 0) {
         const T* sc = reinterpret_cast<const T*>(a.scale);
         const T* scs = reinterpret_cast<const T*>(a.scale_s);
         bx = (T)(a.ctr_s[3 * (int64_t)gs] - a.ctr[3 * (int64_t)gt]);
@@ -127,7 +139,8 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
             if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
             else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
         });
-        translate_qz<T, P, KIND, qz_mode<T>()>(v, bx, by, bz, a_old, a_new);
+        if constexpr (GEO) translate_qz_geo<T, P, KIND, qz_mode<T>()>(v, (T)rec[0], (T)rec[1], (T)rec[2], (T)rec[3], (T)rec[4], (T)rec[5], (T)rec[6]);
+        else translate_qz<T, P, KIND, qz_mode<T>()>(v, bx, by, bz, a_old, a_new);
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             V x;
@@ -166,22 +179,22 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
     }
 }
 
-template <typename T, int P, int KIND, int XW = 4, bool SYNC = false>
+template <typename T, int P, int KIND, int XW = 4, bool GEO = false>
 void launch(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
     constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;  // rows + one mbarrier per warp
     static AttrOnce once;
-    once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, SYNC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
+    once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_fast_k<T, P, KIND, XW, GEO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
     const unsigned grid = (unsigned)((a.n + XW * 32 - 1) / (XW * 32));
-    xlate_fast_k<T, P, KIND, XW, SYNC><<<grid, XW * 32, smem, st>>>(a);
+    xlate_fast_k<T, P, KIND, XW, GEO><<<grid, XW * 32, smem, st>>>(a);
 }
 
-// fp64 M2L at p >= 7 (255 registers, 2 warps per scheduler): the warps of a CTA walk the code in lockstep (SYNC), which shares
-// instruction-cache lines: p = 8 2.48 -> 2.01 ms on B200; at p <= 6 and in fp32 (4 warps per scheduler) lockstep costs more than it saves.
 template <typename T, int KIND>
 bool dispatch(int p, const XArgs& a, cudaStream_t st) {
     switch (p) {
-#define FMM_CASE(PP) case PP: launch<T, PP, KIND, 4, false>(a, st); return true;
+#define FMM_CASE(PP) case PP: \
+        if constexpr (sizeof(T) == 4 && KIND == 1) { if (a.geo) { launch<T, PP, KIND, 4, true>(a, st); return true; } } \
+        launch<T, PP, KIND, 4, false>(a, st); return true;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
         default: return false;
@@ -189,6 +202,77 @@ bool dispatch(int p, const XArgs& a, cudaStream_t st) {
 }
 
 }  // namespace
+
+// plan time (fp32, p <= 8): the geometry record of every weak pair, 1 KB per batch of 32 pairs: ct[32], st[32], cp[32], sp[32],
+// 1/r[32], x1[32], x2[32] (float) and the target id[32] (int; -1 for the padding of the last batch) -- what xlate_geometry computes
+namespace {
+__global__ void m2l_geo_prepare_k(int64_t n, const int32_t* __restrict__ tgt, const int32_t* __restrict__ src, const double* __restrict__ ctr,
+                                  const float* __restrict__ scale, const double* __restrict__ ctr_s, const float* __restrict__ scale_s, float* __restrict__ geo) {
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nb = (n + 31) >> 5;
+    if (e >= (nb << 5)) return;
+    float ct_ = 1.f, st_ = 0.f, cp_ = 1.f, sp_ = 0.f, rinv = 0.f, x1 = 0.f, x2 = 0.f;
+    int gt = -1;
+    if (e < n) {
+        const int gs = src[e];
+        gt = tgt[e];
+        const float bx = (float)(ctr_s[3 * (int64_t)gs] - ctr[3 * (int64_t)gt]);
+        const float by = (float)(ctr_s[3 * (int64_t)gs + 1] - ctr[3 * (int64_t)gt + 1]);
+        const float bz = (float)(ctr_s[3 * (int64_t)gs + 2] - ctr[3 * (int64_t)gt + 2]);
+        xr::xlate_geometry<float, 1>(bx, by, bz, scale_s[gs], scale[gt], ct_, st_, cp_, sp_, rinv, x1, x2);
+    }
+    float* rec = geo + (e >> 5) * 256 + (e & 31);
+    rec[0] = ct_; rec[32] = st_; rec[64] = cp_; rec[96] = sp_; rec[128] = rinv; rec[160] = x1; rec[192] = x2;
+    reinterpret_cast<int*>(rec)[224] = gt;
+}
+}  // namespace
+
+bool m2l_geo_wanted(int p, fmm_dtype dt) { return dt == FMM_F32 && p >= 1 && p <= 8; }
+
+// Geometry records of the weak list (28 + 4 bytes per pair; they depend on the positions only, so they are written once per plan).
+// The list is cut into the two segments that the evaluate schedule launches separately -- the pairs whose target is above the leaf
+// level, [0, w_leaf), and the leaf-level pairs [w_leaf, n_weak) -- each with its own batches of 32.
+void m2l_geo_prepare(Plan& P, cudaStream_t st) {
+    const int64_t w_leaf = (!P.S && (int64_t)P.weak_level_off.size() > P.L) ? P.weak_level_off[P.L] : 0;
+    const int64_t seg_e0[2] = {0, w_leaf}, seg_n[2] = {w_leaf, P.n_weak - w_leaf};
+    P.m2l_seg_e0[0] = 0; P.m2l_seg_e0[1] = w_leaf;
+    P.m2l_seg_rec[0] = 0; P.m2l_seg_rec[1] = (seg_n[0] + 31) >> 5;
+    const int64_t nb = P.m2l_seg_rec[1] + ((seg_n[1] + 31) >> 5);
+    P.m2l_geo.alloc((size_t)nb * 256);
+    const Plan& PS = P.S ? *P.S : P;
+    for (int g = 0; g < 2; ++g) {
+        if (seg_n[g] <= 0) continue;
+        const int64_t nbg = (seg_n[g] + 31) >> 5;
+        m2l_geo_prepare_k<<<(unsigned)((nbg * 32 + 255) / 256), 256, 0, st>>>(seg_n[g], P.weak_tgt.p + seg_e0[g], P.weak_src.p + seg_e0[g], P.box_ctr.p,
+                                                                              reinterpret_cast<const float*>(P.box_scale.p), PS.box_ctr.p,
+                                                                              reinterpret_cast<const float*>(PS.box_scale.p), P.m2l_geo.p + P.m2l_seg_rec[g] * 256);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+}
+
+// FP32 / FP64 arithmetic instructions of ONE translation as these kernels execute it (operator arithmetic only: the geometry,
+// addressing, staging and run sums are not counted) -- the flop count behind bench.py's roofline line.  w = {FMA, MUL, ADD}.
+void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]) {
+    w[0] = w[1] = w[2] = 0;
+    if (p < 1 || p > ct::PF) return;
+    const int64_t K = (int64_t)(p + 1) * (p + 1), rows = K - 1, nnz = ct::bnnz(p) - 1;  // degree 0 is never touched
+    const int64_t zpairs = (int64_t)p * (p + 1) / 2;                                    // (m, -m) pairs of all degrees
+    const bool qz = p <= 8;                                                            // register kernels: Q Z loop
+    const int n_trig = qz ? 4 : 2;                                                     // cos / sin tables built per translation
+    int64_t fma = 0, mul = 0;
+    fma += (int64_t)n_trig * p * 2; mul += (int64_t)n_trig * p * 2;                      // addition-theorem recurrences
+    fma += 4 * zpairs * 2; mul += 4 * zpairs * 2;                                      // four azimuthal rotations
+    fma += 4 * (nnz - rows); mul += 4 * rows;                                          // four applications of Q (or B, B^T)
+    if (kind != 2) mul += rows + p;                                                    // source scaling x2^n
+    for (int m = -p; m <= p; ++m) {
+        const int64_t cnt = p - (m < 0 ? -m : m) + 1;
+        if (kind == 1) { mul += cnt; fma += cnt * (cnt - 1); }                         // M2L z-shift: dense cnt x cnt block
+        else { fma += cnt * (cnt - 1) / 2; mul += cnt * (cnt - 1) / 2; }               // M2M / L2L: triangular, weight = const * power
+    }
+    mul += p + (kind == 0 ? 0 : K);                                                    // powers of x1; output scaling (M2L, L2L)
+    (void)dt;
+    w[0] = fma; w[1] = mul; w[2] = 0;
+}
 
 // p <= 8: state vector in registers (this file); 9 <= p <= 12: state vector in shared memory (xlate_smem.cu)
 bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && ((p >= 1 && p <= 8) || xlate_smem_available(p, dt)); }
@@ -209,6 +293,17 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
         a.in = P.Mc.p;
         a.out = P.Lc.p;
         if (P.S) { a.ctr_s = P.S->box_ctr.p; a.scale_s = P.S->box_scale.p; a.in = P.S->Mc.p; }  // sources in their own hierarchy
+        // geometry records: usable when [e0, e1) starts at a segment start and does not straddle the two segments
+        if (P.m2l_geo.p) {
+            const int64_t w = P.m2l_seg_e0[1];
+            if (e0 == 0 && (e1 <= w || w == 0)) a.geo = P.m2l_geo.p + P.m2l_seg_rec[w == 0 ? 1 : 0] * 256;
+            else if (e0 == w) a.geo = P.m2l_geo.p + P.m2l_seg_rec[1] * 256;
+            else if (e0 == 0 && e1 > w) {  // both segments: two launches
+                xlate_fast_launch(P, 1, level, st, 0, w);
+                xlate_fast_launch(P, 1, level, st, w, e1);
+                return;
+            }
+        }
     } else {
         a.n = (int64_t)1 << (P.s * level);  // children on `level`
         a.off_parent = P.level_off[level - 1];

@@ -277,11 +277,20 @@ __device__ __forceinline__ void qz_angle(int k, T ct_, T st_, T cp_, T sp_, T& c
     s1 = (k == 0 || k == 3) ? cp_ : (k == 1 ? T(0) - st_ : (k == 2 ? st_ : T(0)));
 }
 
+// translate_qz with the geometry of the translation given (xlate_geometry): cos / sin of the polar and azimuthal angle, 1/r, x1, x2
+template <typename T, int P, int KIND, int MODE, int KV>
+__device__ __forceinline__ void translate_qz_geo(T (&v)[KV], T ct_, T st_, T cp_, T sp_, T rinv, T x1, T x2);
+
 template <typename T, int P, int KIND, int MODE, int KV>
 __device__ __forceinline__ void translate_qz(T (&v)[KV], T bx, T by, T bz, T a_old, T a_new) {
-    constexpr int P1 = P + 1;
     T ct_, st_, cp_, sp_, rinv, x1, x2;
     xlate_geometry<T, KIND>(bx, by, bz, a_old, a_new, ct_, st_, cp_, sp_, rinv, x1, x2);
+    translate_qz_geo<T, P, KIND, MODE>(v, ct_, st_, cp_, sp_, rinv, x1, x2);
+}
+
+template <typename T, int P, int KIND, int MODE, int KV>
+__device__ __forceinline__ void translate_qz_geo(T (&v)[KV], T ct_, T st_, T cp_, T sp_, T rinv, T x1, T x2) {
+    constexpr int P1 = P + 1;
     if constexpr (KIND != 2) {  // M2M / M2L: the source scaling x2^n commutes with the rotations
         T pw = T(1);
         sfor<P>([&](auto nc) {

@@ -18,7 +18,7 @@ FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
-           "fmm_version", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
+           "fmm_version", "fmm_translation_work", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
 
 class fmm_admissibility(C.Structure):
@@ -58,6 +58,7 @@ def lib():
         L.fmm_plan_set_m2l_variant.argtypes = [vp, C.c_int]
         L.fmm_plan_set_schedule.argtypes = [vp, C.c_int]
         L.fmm_plan_launches.argtypes = [vp, i64p]
+        L.fmm_translation_work.argtypes = [C.c_int, C.c_int, C.c_int, i64p, i64p, i64p]
         L.fmm_last_error.restype = C.c_char_p
         L.fmm_version.restype = C.c_char_p
         for name in EXPORTS:
@@ -95,6 +96,43 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
+# handle -> (torch dtype, number of charges, number of outputs, device): the C side sees raw pointers only, so the binding checks
+# every tensor it marshals against the plan it is passed with
+_PLANS = {}
+
+
+def _check_io(plan, charges, potential, field, host=False):
+    meta = _PLANS.get(plan.value)
+    if meta is None:
+        raise ValueError("unknown or destroyed plan handle")
+    tdtype, Nq, Nt, device = meta
+
+    def one(name, t, shape):
+        if t is None:
+            return
+        if isinstance(t, np.ndarray):
+            if not host:
+                raise ValueError("%s must be a CUDA tensor" % name)
+            ok_dtype = t.dtype == (np.float32 if str(tdtype).endswith("float32") else np.float64)
+            contiguous, on_dev = t.flags["C_CONTIGUOUS"], True
+        else:
+            ok_dtype = t.dtype == tdtype
+            contiguous = t.is_contiguous()
+            on_dev = (not t.is_cuda) if host else (t.is_cuda and t.device == device)
+        if not ok_dtype:
+            raise ValueError("%s has dtype %s but the plan was built for %s" % (name, t.dtype, tdtype))
+        if tuple(t.shape) != shape:
+            raise ValueError("%s has shape %s, expected %s" % (name, tuple(t.shape), shape))
+        if not contiguous:
+            raise ValueError("%s must be contiguous" % name)
+        if not on_dev:
+            raise ValueError("%s must live %s" % (name, "in host memory" if host else "on the plan's device %s" % device))
+
+    one("charges", charges, (Nq,))
+    one("potential", potential, (Nt,))
+    one("field", field, (Nt, 3))
+
+
 def fmm_plan_create(positions, p, N_max, s, theta=0.77, cross_level=0, stream=None):
     """positions: CUDA tensor (N,3), contiguous, float32/float64.  Returns an opaque plan handle (c_void_p)."""
     if not positions.is_cuda or not positions.is_contiguous() or positions.dim() != 2 or positions.shape[1] != 3:
@@ -103,6 +141,7 @@ def fmm_plan_create(positions, p, N_max, s, theta=0.77, cross_level=0, stream=No
     h = C.c_void_p()
     _check(lib().fmm_plan_create(C.c_void_p(positions.data_ptr()), positions.shape[0], int(p), int(N_max), int(s), C.byref(adm),
                                  _dtype_code(positions), _stream_ptr(stream), C.byref(h)))
+    _PLANS[h.value] = (positions.dtype, positions.shape[0], positions.shape[0], positions.device)
     return h
 
 
@@ -117,6 +156,7 @@ def fmm_plan_create_targets(sources, targets, p, N_max, s, theta=0.77, stream=No
     h = C.c_void_p()
     _check(lib().fmm_plan_create_targets(C.c_void_p(sources.data_ptr()), sources.shape[0], C.c_void_p(targets.data_ptr()), targets.shape[0], int(p),
                                          int(N_max), int(s), C.byref(adm), _dtype_code(sources), _stream_ptr(stream), C.byref(h)))
+    _PLANS[h.value] = (sources.dtype, sources.shape[0], targets.shape[0], sources.device)
     return h
 
 
@@ -149,19 +189,20 @@ def fmm_plan_copy_march(plan):
 
 
 def fmm_plan_destroy(plan):
+    _PLANS.pop(plan.value, None)
     _check(lib().fmm_plan_destroy(plan))
 
 
 def fmm_evaluate(plan, charges, potential=None, field=None, stream=None):
-    """charges (N,), potential (N,) or None, field (N,3) or None: contiguous CUDA tensors of the plan's dtype."""
-    for t in (charges, potential, field):
-        if t is not None and (not t.is_cuda or not t.is_contiguous()):
-            raise ValueError("tensors must be contiguous CUDA tensors")
+    """charges (N,), potential (N,) or None, field (N,3) or None: contiguous CUDA tensors of the plan's dtype on the plan's device
+    (N = number of sources for the charges, number of targets for the outputs)."""
+    _check_io(plan, charges, potential, field)
     _check(lib().fmm_evaluate(plan, C.c_void_p(charges.data_ptr()), C.c_void_p(potential.data_ptr()) if potential is not None else None,
                               C.c_void_p(field.data_ptr()) if field is not None else None, _stream_ptr(stream)))
 
 
 def fmm_evaluate_profiled(plan, charges, potential=None, field=None, stream=None):
+    _check_io(plan, charges, potential, field)
     ms = (C.c_double * 8)()
     _check(lib().fmm_evaluate_profiled(plan, C.c_void_p(charges.data_ptr()), C.c_void_p(potential.data_ptr()) if potential is not None else None,
                                        C.c_void_p(field.data_ptr()) if field is not None else None, _stream_ptr(stream), ms))
@@ -171,6 +212,8 @@ def fmm_evaluate_profiled(plan, charges, potential=None, field=None, stream=None
 
 def fmm_evaluate_host(plan, h_charges, h_potential=None, h_field=None, stream=None):
     """Host-buffer path: numpy arrays or pinned CPU tensors; H2D and D2H copies happen inside the call."""
+    _check_io(plan, h_charges, h_potential, h_field, host=True)
+
     def ptr(a):
         if a is None:
             return None
@@ -197,6 +240,13 @@ def fmm_plan_launches(plan):
     v = C.c_int64()
     _check(lib().fmm_plan_launches(plan, C.byref(v)))
     return v.value
+
+
+def fmm_translation_work(p, dtype, kind):
+    """(fma, mul, add) instructions of one translation (kind 0 = M2M, 1 = M2L, 2 = L2L) in the specialised kernels."""
+    a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+    _check(lib().fmm_translation_work(int(p), int(dtype), int(kind), C.byref(a), C.byref(b), C.byref(c)))
+    return a.value, b.value, c.value
 
 
 def fmm_plan_set_schedule(plan, serial):

@@ -90,13 +90,27 @@ CONFIGS = {
 }
 
 
+def config5(name):
+    """BASELINE config 5 (scaling sweep): `cfg5_<cube|sphere>_<N>_<f32|f64>_p<p>_n<N_max>[_s<s>]`, e.g. cfg5_cube_1000000_f32_p8_n128.
+    Seeds 50 + round(log10 N); theta = 0.77; s = 3 unless given (the paper's own sweep uses s = 2)."""
+    t = name.split("_")
+    if len(t) < 6 or t[0] != "cfg5" or t[1] not in ("cube", "sphere") or t[3] not in ("f32", "f64") or t[4][0] != "p" or t[5][0] != "n":
+        raise KeyError(name)
+    N = int(float(t[2]))
+    s = int(t[6][1:]) if len(t) > 6 else 3
+    return dict(gen="uniform_cube" if t[1] == "cube" else "sphere_surface", N=N, seed=50 + int(round(np.log10(N))), dtype=t[3],
+                p=int(t[4][1:]), s=s, N_max=int(t[5][1:]), theta=0.77)
+
+
 def make(name):
-    """Return (pos, q, params) for a named BASELINE config."""
-    c = dict(CONFIGS[name])
+    """Return (pos, q, params) for a named BASELINE config (CONFIGS, or a config-5 sweep point, see config5)."""
+    c = dict(CONFIGS[name]) if name in CONFIGS else config5(name)
     dt = np.float32 if c["dtype"] == "f32" else np.float64
     g = c["gen"]
     if g == "uniform_cube":
         pos, q = uniform_cube(c["N"], c["seed"], dt)
+    elif g == "sphere_surface":
+        pos, q = sphere_surface(c["N"], c["seed"], dt)
     elif g == "gaussian_clusters":
         pos, q = gaussian_clusters(c["N"], c["seed"], dt)
     elif g == "thin_film":

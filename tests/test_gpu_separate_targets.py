@@ -45,7 +45,8 @@ def run_st(sp, q, tp, p, N_max, s, theta=0.77, direct=True, variants=(0,)):
     assert (P.info["n_weak"], P.info["n_strong"], P.info["n_p2p_pairs"]) == (Po.n_weak, Po.n_strong, Po.n_p2p_pairs)
     for k in ("weak_off", "weak_src", "strong_off", "strong_src"):
         assert np.array_equal(lg[k].astype(np.int64), lo_[k]), k
-    uo, fo = Po.evaluate(q)
+    f32 = dt == np.float32
+    uo, fo = Po.evaluate(q, fp32_rule=f32)
     tq = torch.from_numpy(np.ascontiguousarray(q)).cuda()
     res = None
     for v in variants:
@@ -60,9 +61,12 @@ def run_st(sp, q, tp, p, N_max, s, theta=0.77, direct=True, variants=(0,)):
             assert eu <= TOL[dt] and ef <= TOL[dt], (v, serial, eu, ef)
             res = (u, f)
     if direct:
-        ud, fd = O.direct_st(sp, q, tp)
-        # + TOL: where the oracle is exact to rounding (all-P2P cases) the GPU result can only be as close as its own arithmetic
-        assert rel2(res[0], ud) <= 1.5 * rel2(uo, ud) + TOL[dt] and rel2(res[1], fd) <= 1.5 * rel2(fo, fd) + TOL[dt]
+        ud, fd = O.direct_st(sp, q, tp, fp32_rule=f32)
+        # north_star: GPU error <= 1.5 x the oracle's own.  The slack is the unit roundoff of the plan's dtype times 8 -- where the oracle is
+        # exact to fp64 rounding (all-P2P cases) an fp32 result can only be as close to the definition as binary32 arithmetic allows;
+        # it never dominates a truncation error (>= 1e-6 in every far-field case here), so the 1.5x clause keeps its meaning
+        slack = 8 * (6e-8 if f32 else 1.2e-16)
+        assert rel2(res[0], ud) <= 1.5 * rel2(uo, ud) + slack and rel2(res[1], fd) <= 1.5 * rel2(fo, fd) + slack
     st = fmm.fmm_evaluate_profiled(P.handle, tq, *P.evaluate(tq))
     assert st["total"] > 0
     P.close()
@@ -142,14 +146,33 @@ def test_host_path_and_partial_outputs():
 
 
 def test_one_million_sources_sampled_targets():
-    """Config-2 sources (N = 1M, fp32, p = 8) evaluated at 200 000 separate targets; checked against the definition on a sample."""
+    """Config-2 sources (N = 1M, fp32, p = 8) evaluated at 200 000 separate targets: both hierarchies, the march and both lists
+    bit-exact against the oracle at full size; potential / field on the targets of 128 random target leaves against the oracle
+    (leaf mask: same arithmetic as a full run) at the north_star tolerance and element by element, and against the definition."""
     sp, q, c = inputs.make("cfg2_cube1M_f32")
     tp = targets(200000, 75, np.float32, 0.0, 1.0)
     P = fmm.PlanTargets(torch.from_numpy(sp).cuda(), torch.from_numpy(tp).cuda(), c["p"], c["N_max"], c["s"], c["theta"])
+    Po = O.PlanST(sp, tp, c["p"], c["N_max"], c["s"], c["theta"])
+    same_tree(P.tree("tgt"), Po.tree("tgt"))
+    same_tree(P.tree("src"), Po.tree("src"))
+    lg, lo_ = P.lists(), Po.lists()
+    assert lg["steps"].tolist() == lo_["steps"].tolist()
+    assert (P.info["n_weak"], P.info["n_strong"], P.info["n_p2p_pairs"]) == (Po.n_weak, Po.n_strong, Po.n_p2p_pairs)
+    for k in ("weak_off", "weak_src", "strong_off", "strong_src"):
+        assert np.array_equal(lg[k].astype(np.int64), lo_[k]), k
     u, f = P.evaluate(torch.from_numpy(q).cuda())
     torch.cuda.synchronize()
-    sel = np.random.default_rng(0).choice(tp.shape[0], 512, replace=False)
-    ud, fd = O.direct_st(sp, q, tp[sel])
-    eu, ef = rel2(u.cpu().numpy()[sel], ud), rel2(f.cpu().numpy()[sel], fd)
-    assert eu < 2e-4 and ef < 2e-3, (eu, ef)  # truncation error of p = 8 at theta = 0.77 (same order as config 2 itself)
+    u, f = u.cpu().numpy(), f.cpu().numpy()
+    nl = Po.info["tgt"]["n_leaves"]
+    mask = np.zeros(nl, np.uint8)
+    mask[np.random.default_rng(0).choice(nl, 128, replace=False)] = 1
+    uo, fo = Po.evaluate(q, leaf_mask=mask, fp32_rule=True)
+    sel = np.flatnonzero(np.isfinite(uo))
+    assert sel.size > 1000
+    eu, ef = rel2(u[sel], uo[sel]), rel2(f[sel], fo[sel])
+    assert eu <= 1e-5 and ef <= 1e-5, (eu, ef)
+    assert np.max(np.abs(u[sel] - uo[sel])) <= 1e-4 * np.max(np.abs(uo[sel])) and np.max(np.abs(f[sel] - fo[sel])) <= 1e-4 * np.max(np.abs(fo[sel]))
+    dsel = sel[:1024]
+    ud, fd = O.direct_st(sp, q, tp[dsel], fp32_rule=True)
+    assert rel2(u[dsel], ud) <= 1.5 * rel2(uo[dsel], ud) and rel2(f[dsel], fd) <= 1.5 * rel2(fo[dsel], fd)
     P.close()
