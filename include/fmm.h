@@ -82,6 +82,22 @@ fmm_status fmm_plan_create(const void* d_positions, int64_t N, int p, int N_max,
  * Asynchronous on cuda_stream. */
 fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream);
 
+/* Adjoint evaluate: the vector-Jacobian product of fmm_evaluate with respect to the charges (where JAX autodiff
+ * differentiates a loss on the potential with respect to the charges).  fmm_evaluate is linear in the charges -- potential = A q,
+ * field = F q with the FMM operators A, F of this plan -- so for cotangents ubar (of the potential) and fbar (of the field)
+ *     charge_grad = A^T ubar + F^T fbar .
+ * It is computed as the TRANSPOSE OF THE FORWARD OPERATOR on the same plan, stage by stage: L2P^T is a P2M at the targets (with
+ * dipole moments -fbar for the field part), L2L^T = M2M and M2M^T = L2L run on the other hierarchy, M2L^T is the M2L over the
+ * transposed weak list, P2P^T the near field over the transposed strong list.  The transposed lists are built on the first call
+ * (which synchronises the stream) and kept in the plan; a plan over one point set with same-level lists needs none (its lists
+ * are symmetric).  <ubar, A q> + <fbar, F q> = <charge_grad, q> holds to rounding, not just to the truncation error of the FMM.
+ *   d_cotangent_potential : DEVICE, Nt (N), target input order, dtype; may be NULL (zero).
+ *   d_cotangent_field     : DEVICE, Nt x 3 (N x 3), dtype; may be NULL (zero); at least one of the two must be given.
+ *   d_charge_grad         : DEVICE, Ns (N), source input order, dtype (overwritten).
+ * Asynchronous on cuda_stream after the first call. */
+fmm_status fmm_evaluate_adjoint(fmm_plan* plan, const void* d_cotangent_potential, const void* d_cotangent_field, void* d_charge_grad,
+                                void* cuda_stream);
+
 /* Same operation with HOST buffers: copies charges host->device, evaluates, copies the results back and
  * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);

@@ -295,6 +295,24 @@ fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_pot
     });
 }
 
+fmm_status fmm_evaluate_adjoint(fmm_plan* plan, const void* d_cotangent_potential, const void* d_cotangent_field, void* d_charge_grad, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !d_charge_grad || (!d_cotangent_potential && !d_cotangent_field)) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        Plan& P = plan->P;
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
+        // one point set with same-level lists: the lists are symmetric and the FMM potential operator is its own transpose
+        // (M2M^T = L2L, M2L(t<-s)^T = M2L(s<-t), P2M^T = L2P in the normalised basis), so the plan is its own adjoint view
+        const bool self_adjoint = !P.S && !P.cross_level;
+        if (!self_adjoint) build_adjoint_view(P, st);
+        const Plan& V = self_adjoint ? P : *P.adj;
+        if (!self_adjoint) { P.adj->m2l_variant = P.m2l_variant; P.adj->serial = P.serial; }
+        run_evaluate(V, d_cotangent_potential, d_charge_grad, nullptr, st, nullptr, d_cotangent_field);
+        return FMM_OK;
+    });
+}
+
 fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream,
                                  double* h_stage_ms) {
     return guarded([&]() -> fmm_status {

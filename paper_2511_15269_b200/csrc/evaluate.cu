@@ -260,6 +260,73 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) l2p_k(const typename V4<
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------ dipole sources (adjoint of the field)
+// fmm_evaluate_adjoint with a field cotangent fbar: field = -grad u, so its transpose makes every target a DIPOLE source of moment
+// -fbar_i: the potential it causes at x is fbar_i . grad_y (1/|x - y|) ... with the overall sign bookkeeping of evaluate():
+//     phi(x) += -fbar_i . (x - y_i) / |x - y_i|^3        (near field, p2p_k<T, true>)
+//     M_n^m  += -fbar_i . grad Rn_n^m((y_i - c)/a) / a   (far field, p2m_dipole_k: the transposed "L2P with gradient")
+// grad R^ comes from the ladder identities of App. A.3 (the same ones l2p_k uses, pinned in tests/test_oracle_basis.py):
+//     d/dz R^_n^(+-j) = R^_(n-1)^(+-j)
+//     d/dx R^_n^j  = (j >= 1 ? 1/2 R^_(n-1)^(j-1) : 0) - (j >= 1 ? 1/2 : 1) R^_(n-1)^(j+1)              (j >= 0)
+//     d/dx R^_n^-j = (j >= 2 ? 1/2 R^_(n-1)^-(j-1) : 0) - 1/2 R^_(n-1)^-(j+1)                            (j >= 1)
+//     d/dy R^_n^j  = (j >= 2 ? 1/2 R^_(n-1)^-(j-1) : 0) + (j >= 1 ? 1/2 : 1) R^_(n-1)^-(j+1)            (j >= 0)
+//     d/dy R^_n^-j = -1/2 R^_(n-1)^(j-1) - 1/2 R^_(n-1)^(j+1)                                            (j >= 1)
+// with R^_(n-1)^k := 0 for |k| > n-1.
+template <typename T>
+__global__ void permute_dip_k(const T* __restrict__ fbar, const int32_t* __restrict__ perm, typename V4<T>::type* __restrict__ dip, int64_t N) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int64_t i = perm[k];
+    dip[k] = make4<T>(fbar[3 * i], fbar[3 * i + 1], fbar[3 * i + 2], T(0));
+}
+
+template <typename T, int P>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) p2m_dipole_k(const typename V4<T>::type* __restrict__ pq, const typename V4<T>::type* __restrict__ dip,
+                                                                     const int32_t* __restrict__ box_start, const int32_t* __restrict__ box_count,
+                                                                     const double* __restrict__ ctr, const T* __restrict__ scale, int64_t leaf0, int64_t n_leaves,
+                                                                     int Kp, T* __restrict__ Mc) {
+    constexpr int KD = P > 0 ? P * P : 1;  // R^ of degree <= P-1
+    const int lane = threadIdx.x & 31;
+    const int64_t leaf = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
+    if (leaf >= n_leaves || P == 0) return;
+    const int64_t g = leaf0 + leaf;
+    const int st = box_start[g], cnt = box_count[g];
+    const double cx = ctr[3 * g], cy = ctr[3 * g + 1], cz = ctr[3 * g + 2];
+    const T inva = T(1) / scale[g];
+    for (int base = 0; base < cnt; base += 32) {
+        const int i = base + lane;
+        T x = 0, y = 0, z = 0, fx = 0, fy = 0, fz = 0;
+        if (i < cnt) {
+            const typename V4<T>::type v = pq[st + i], d = dip[st + i];
+            x = (T)((double)v.x - cx) * inva; y = (T)((double)v.y - cy) * inva; z = (T)((double)v.z - cz) * inva;
+            fx = d.x; fy = d.y; fz = d.z;
+        }
+        T R[KD];
+        regular_rec<(P > 0 ? P - 1 : 0), T>(x, y, z, [&](int n, int m, T val) { R[n * n + n + m] = val; });
+        auto Rl = [&](int n1, int k) -> T { return (k >= -n1 && k <= n1) ? R[n1 * n1 + n1 + k] : T(0); };
+        for (int n = 1; n <= P; ++n)
+            for (int m = -n; m <= n; ++m) {
+                const int j = m < 0 ? -m : m, n1 = n - 1;
+                T gx, gy, gz;
+                if (m >= 0) {
+                    gx = (j >= 1 ? T(0.5) * Rl(n1, j - 1) : T(0)) - (j >= 1 ? T(0.5) : T(1)) * Rl(n1, j + 1);
+                    gy = (j >= 2 ? T(0.5) * Rl(n1, -(j - 1)) : T(0)) + (j >= 1 ? T(0.5) : T(1)) * Rl(n1, -(j + 1));
+                    gz = Rl(n1, j);
+                } else {
+                    gx = (j >= 2 ? T(0.5) * Rl(n1, -(j - 1)) : T(0)) - T(0.5) * Rl(n1, -(j + 1));
+                    gy = -T(0.5) * Rl(n1, j - 1) - T(0.5) * Rl(n1, j + 1);
+                    gz = Rl(n1, -j);
+                }
+                T v = -(fx * gx + fy * gy + fz * gz);
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+                const int idx = n * n + n + m;
+                if (lane == 0) Mc[g * Kp + idx] += v * inva * gnorm<T>(idx);
+            }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ generic translations
 // One warp per translation; state vectors in shared memory; rotation = Z(-phi) B Z(-theta) B^T [shift] B Z(theta) B^T Z(phi).
 template <typename T>
@@ -450,14 +517,17 @@ constexpr int P2P_THREADS = 128;
 constexpr int P2P_TPT = 4;
 constexpr int P2P_TILE = 512;
 
-template <typename T>
+// DIP: every source also carries a dipole (dip_s, see above); potential only
+template <typename T, bool DIP>
 __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type* __restrict__ pq, const int32_t* __restrict__ leaf_start,
                                                      const int32_t* __restrict__ leaf_cnt, const typename V4<T>::type* __restrict__ pq_s,
                                                      const int32_t* __restrict__ sleaf_start, const int32_t* __restrict__ sleaf_cnt,
                                                      const int64_t* __restrict__ strong_off, const int32_t* __restrict__ strong_src,
-                                                     typename V4<T>::type* __restrict__ near) {  // *_s: the sources' hierarchy (== the targets' unless PAPER.md:82)
+                                                     typename V4<T>::type* __restrict__ near,  // *_s: the sources' hierarchy (== the targets' unless PAPER.md:82)
+                                                     const typename V4<T>::type* __restrict__ dip_s) {
     using T4 = typename V4<T>::type;
     __shared__ T4 sh[P2P_TILE];
+    __shared__ T4 shd[DIP ? P2P_TILE : 1];
     __shared__ T red[P2P_THREADS * P2P_TPT * 4];
     const int tid = threadIdx.x;
     const int64_t leaf = blockIdx.x;
@@ -492,7 +562,10 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
                 const int sleaf = strong_src[e];
                 const int sst = sleaf_start[sleaf], sc = sleaf_cnt[sleaf];
                 const int take = min(sc - sub, P2P_TILE - tile_n);
-                for (int i = tid; i < take; i += P2P_THREADS) sh[tile_n + i] = pq_s[sst + sub + i];
+                for (int i = tid; i < take; i += P2P_THREADS) {
+                    sh[tile_n + i] = pq_s[sst + sub + i];
+                    if constexpr (DIP) shd[tile_n + i] = dip_s[sst + sub + i];
+                }
                 tile_n += take;
                 sub += take;
                 if (sub >= sc) { ++e; sub = 0; }
@@ -513,7 +586,12 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
                     const T inv2 = inv * inv;
                     const T q3 = sv.w * inv * inv2;
                     ph[t] += sv.w * inv;
-                    gx[t] -= q3 * dx; gy[t] -= q3 * dy; gz[t] -= q3 * dz;
+                    if constexpr (DIP) {
+                        const T4 dv = shd[j];
+                        ph[t] -= (dv.x * dx + dv.y * dy + dv.z * dz) * (inv * inv2);
+                    } else {
+                        gx[t] -= q3 * dx; gy[t] -= q3 * dy; gz[t] -= q3 * dz;
+                    }
                 }
             }
         }
@@ -561,6 +639,20 @@ void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaSt
 }
 
 template <typename T>
+void dispatch_p2m_dipole(const Plan& Pl, cudaStream_t st) {
+    using T4 = typename V4<T>::type;
+    const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK);
+    switch (Pl.p) {
+#define FMM_CASE(PP) case PP: p2m_dipole_k<T, PP><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, (const T4*)Pl.dip.p, Pl.box_start.p, Pl.box_count.p, \
+            Pl.box_ctr.p, (const T*)Pl.box_scale.p, Pl.level_off[Pl.L], Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p); break;
+        FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
+        FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12) FMM_CASE(13) FMM_CASE(14) FMM_CASE(15) FMM_CASE(16)
+#undef FMM_CASE
+        default: break;  // p = 0: a dipole has no monopole moment
+    }
+}
+
+template <typename T>
 void dispatch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
     switch (Pl.p) {
 #define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, d_pot, d_field, st); break;
@@ -588,7 +680,7 @@ void ensure_streams(const Plan& Pl) {
 // source leaves into target leaves.  Weak pairs may join any two levels, so the whole upward pass precedes the M2L; the P2P
 // still runs beside the far-field chain on its own stream.  ev != nullptr: serial, one event per stage (same order as run_t).
 template <typename T>
-void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
     using T4 = typename V4<T>::type;
     const Plan& S = *Pl.S;
     const Tables& tb = tables(Pl.device);
@@ -612,10 +704,15 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[Pl.L], sleaf0 = S.level_off[S.L];
     auto launch_p2p = [&](cudaStream_t q) {
-        if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
+        if (d_dip)
+            p2p_k<T, true><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
+                                                                        S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p,
+                                                                        (T4*)Pl.near.p, (const T4*)S.dip.p);
+        else if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
         else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q, d_field != nullptr);
-        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
-                                                                  S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
+        else p2p_k<T, false><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)S.pq.p,
+                                                                         S.box_start.p + sleaf0, S.box_count.p + sleaf0, Pl.strong_off.p, Pl.strong_src.p,
+                                                                         (T4*)Pl.near.p, nullptr);
         FMM_CUDA_CHECK(cudaGetLastError());
     };
     mark(0);
@@ -624,11 +721,17 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     FMM_CUDA_CHECK(cudaGetLastError());
     permute_k<T><<<nblocks(Pl.N, 256), 256, 0, sF>>>((const T*)Pl.pos_tree.p, nullptr, Pl.perm.p, (T4*)Pl.pq.p, nullptr, nullptr, Pl.N);
     FMM_CUDA_CHECK(cudaGetLastError());
+    if (d_dip) {
+        if (!S.dip.p) S.dip.alloc((size_t)S.N * 4 * sizeof(T));
+        permute_dip_k<T><<<nblocks(S.N, 256), 256, 0, sF>>>((const T*)d_dip, S.perm.p, (T4*)S.dip.p, S.N);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
     after(sN, sF, Pl.e_perm);
     if (!serial) launch_p2p(sN);
     FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, sF));
     mark(1);
     dispatch_p2m_l2p<T>(S, false, nullptr, nullptr, sF);
+    if (d_dip) dispatch_p2m_dipole<T>(S, sF);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(2);
     if (fast && S.L > 0) FMM_CUDA_CHECK(cudaMemsetAsync(S.Mc.p, 0, (size_t)S.level_off[S.L] * S.Kp * sizeof(T), sF));
@@ -671,7 +774,7 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
 // the L2L levels, all concurrent with the leaf-level M2L) and near field (P2P, concurrent with everything between permute and L2P).
 // ev != nullptr: the same kernels back to back on the caller's stream with an event after every stage (profiling).
 template <typename T>
-void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
     using T4 = typename V4<T>::type;
     const Tables& tb = tables(Pl.device);
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
@@ -696,10 +799,15 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const bool fast_p2p = sizeof(T) == 4 && Pl.m2l_variant != 1;
     const int64_t leaf0 = Pl.level_off[L];
     auto launch_p2p = [&](cudaStream_t q) {
-        if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
+        if (d_dip)
+            p2p_k<T, true><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
+                                                                        Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p,
+                                                                        (T4*)Pl.near.p, (const T4*)Pl.dip.p);
+        else if (fast_p2p) p2p_fast_launch(Pl, q, d_field != nullptr);
         else if (sizeof(T) == 8 && Pl.m2l_variant != 1) p2p_fast64_launch(Pl, q, d_field != nullptr);
-        else p2p_k<T><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
-                                                                  Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p, (T4*)Pl.near.p);
+        else p2p_k<T, false><<<(unsigned)Pl.n_leaves, P2P_THREADS, 0, q>>>((const T4*)Pl.pq.p, Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, (const T4*)Pl.pq.p,
+                                                                         Pl.box_start.p + leaf0, Pl.box_count.p + leaf0, Pl.strong_off.p, Pl.strong_src.p,
+                                                                         (T4*)Pl.near.p, nullptr);
         FMM_CUDA_CHECK(cudaGetLastError());
     };
 
@@ -707,11 +815,17 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     permute_k<T><<<nblocks(N, 256), 256, 0, sF>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, Pl.src_slot.p,
                                                   sizeof(T) == 4 ? Pl.srcg.p : nullptr, N);
     FMM_CUDA_CHECK(cudaGetLastError());
+    if (d_dip) {
+        if (!Pl.dip.p) Pl.dip.alloc((size_t)N * 4 * sizeof(T));
+        permute_dip_k<T><<<nblocks(N, 256), 256, 0, sF>>>((const T*)d_dip, Pl.perm.p, (T4*)Pl.dip.p, N);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
     after(sN, sF, Pl.e_perm);
     if (!serial) launch_p2p(sN);
     FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, sF));
     mark(1);
     dispatch_p2m_l2p<T>(Pl, false, nullptr, nullptr, sF);
+    if (d_dip) dispatch_p2m_dipole<T>(Pl, sF);
     FMM_CUDA_CHECK(cudaGetLastError());
     mark(2);
     if (fast && L > 0)  // the register kernels accumulate into the parents
@@ -719,7 +833,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     // the M2L of the leaf level needs only the P2M output: with the register kernels it runs on sF while M2M and the upper
     // levels' M2L run on sU (weak pairs are sorted by target id, hence by level; rows of different levels are disjoint)
     const int64_t w_leaf = (int64_t)Pl.weak_level_off.size() > L ? Pl.weak_level_off[L] : 0;
-    const bool split = !serial && fast && L > 0;
+    const bool split = !serial && fast && L > 0 && !Pl.no_split;
     if (split) after(sU, sF, Pl.e_p2m);
     cudaStream_t sM = split ? sU : sF;
     for (int l = L; l >= 1; --l) {
@@ -780,7 +894,7 @@ int64_t evaluate_launches(const Plan& P) {
     return 4 + 2 * (int64_t)P.L + m2l;  // permute, P2M, P2P, L2P(+finalize) + M2M/L2L per level + M2L
 }
 
-void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev) {
+void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
     {   // __constant__ copies of g_n^m: one upload per device
         DeviceCtx& ctx = device_ctx(P.device);
         std::lock_guard<std::mutex> lock(ctx.mu);
@@ -795,10 +909,10 @@ void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cu
         }
     }
     if (P.S) {
-        if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev);
-        else run_st<double>(P, d_q, d_pot, d_field, st, ev);
-    } else if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev);
-    else run_t<double>(P, d_q, d_pot, d_field, st, ev);
+        if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev, d_dip);
+        else run_st<double>(P, d_q, d_pot, d_field, st, ev, d_dip);
+    } else if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev, d_dip);
+    else run_t<double>(P, d_q, d_pot, d_field, st, ev, d_dip);
 }
 
 }  // namespace fmm

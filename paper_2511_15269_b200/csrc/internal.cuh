@@ -52,15 +52,23 @@ template <typename T>
 struct DevBuf {
     T* p = nullptr;
     size_t n = 0;
+    bool owned = true;  // false: an alias of another buffer (adjoint view of a plan); never freed here
     void alloc(size_t count) {
         release();
         n = count;
         if (count) FMM_CUDA_CHECK(cudaMallocAsync((void**)&p, count * sizeof(T), alloc_stream()));
     }
+    void alias(const DevBuf& o) {
+        release();
+        p = o.p;
+        n = o.n;
+        owned = false;
+    }
     void release() {
-        if (p) cudaFreeAsync(p, alloc_stream());
+        if (p && owned) cudaFreeAsync(p, alloc_stream());
         p = nullptr;
         n = 0;
+        owned = true;
     }
     ~DevBuf() { release(); }
     DevBuf() = default;
@@ -135,6 +143,11 @@ struct Plan {
     // the local coefficients Lc, `near` and both lists (weak: target box id here -> source box id in S; strong: target leaf ->
     // source leaf of S); S holds the hierarchy of the sources, their permuted particles (pq, srcg) and the multipoles Mc.
     std::unique_ptr<Plan> S;
+    // Adjoint evaluate (fmm_evaluate_adjoint): a view of this plan with the roles of sources and targets exchanged --
+    // aliases of the hierarchy arrays plus the transposed interaction lists -- built on first use (plan.cu build_adjoint_view).
+    // Declared after S: it is destroyed first, while the buffers it aliases are still alive.
+    std::unique_ptr<Plan> adj;
+    bool no_split = false;  // evaluate schedule: never run the leaf-level M2L beside the M2M pass (sources may be coarser than targets)
     std::vector<int> march_steps;  // (l_trg, l_src) pairs visited by the level march (cross_level = 1 or separate targets)
 
     DevBuf<int32_t> perm;                 // N: tree order -> input index
@@ -153,6 +166,7 @@ struct Plan {
     DevBuf<char> pq;      // N x 4 dtype: (x,y,z,q) tree order
     DevBuf<char> Mc, Lc;  // n_boxes x Kp dtype: multipole / local coefficients (normalised, scaled)
     DevBuf<char> near;    // N x 4 dtype: (phi_near, grad phi_near) tree order, P2P -> L2P (which finalizes)
+    mutable DevBuf<char> dip;  // N x 4 dtype: dipole moments of the sources in tree order (adjoint of the field), allocated on first use
     // fp32 P2P source groups (p2p_fast.cu): per leaf src_G groups of (-x[4], -y[4], -z[4], q[4]); src_slot[k] = 4*group + (i & 3)
     DevBuf<float> m2l_geo;   // xlate_fast.cu: per batch of 32 weak pairs a 1 KB geometry record (fp32, p <= 8)
     int64_t m2l_seg_e0[2] = {0, 0}, m2l_seg_rec[2] = {0, 0};  // the two segments of the weak list the records are batched by: first pair, first record
@@ -181,8 +195,11 @@ struct Plan {
 // plan.cu
 void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
 void build_lists(Plan& P, cudaStream_t st);
+void build_adjoint_view(Plan& P, cudaStream_t st);  // fills P.adj (transposed lists; synchronises the stream)
 // evaluate.cu
-void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/);
+// d_q: charges (may be null = zero charges), d_dip: optional dipole moments (N_sources x 3, input order): the sources then also
+// carry the potential -d . grad_source(1/|x - y|) (the transposed field operator of fmm_evaluate_adjoint); potential only
+void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev /*8 or null*/, const void* d_dip = nullptr);
 int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evaluate
 // xlate_fast.cu: register kernels (one thread per translation).  kind 0 = M2M into level-1 from `level`, 1 = M2L (all
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.

@@ -629,6 +629,35 @@ static void finish_lists(Plan& P, cudaStream_t st) {
     }
 }
 
+// stable LSD radix sort of (key, value) pairs by key in [0, n_keys) and the CSR offsets of the keys (n_keys + 1, device)
+static void sort_by_key(DevBuf<int32_t>& keys, DevBuf<int32_t>& vals, int64_t n, int64_t n_keys, int64_t* off_out, cudaStream_t st) {
+    DevBuf<unsigned long long> cnt;
+    DevBuf<int64_t> scr64;
+    cnt.alloc(n_keys + 1);
+    scr64.alloc(scan_scratch_elems(n_keys + 1));
+    FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, (n_keys + 1) * sizeof(unsigned long long), st));
+    if (n > 0) {
+        int bits = 8;
+        while (((int64_t)1 << bits) < n_keys) bits += 8;
+        DevBuf<int32_t> kb, vb, hist, scr;
+        kb.alloc(n); vb.alloc(n);
+        const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
+        hist.alloc((size_t)256 * nblk + 1);
+        scr.alloc(scan_scratch_elems((int64_t)256 * nblk));
+        const int where = radix_sort_pairs<uint32_t>(reinterpret_cast<uint32_t*>(keys.p), vals.p, reinterpret_cast<uint32_t*>(kb.p), vb.p, n, bits,
+                                                     hist.p, scr.p, st);
+        if (where == 1) {
+            FMM_CUDA_CHECK(cudaMemcpyAsync(keys.p, kb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+            FMM_CUDA_CHECK(cudaMemcpyAsync(vals.p, vb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        }
+        count_keys_k<<<nblocks(n, 256), 256, 0, st>>>(keys.p, n, cnt.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));  // temporaries are freed on scope exit
+    }
+    exclusive_scan<int64_t>(CntLoad{cnt.p, n_keys}, off_out, n_keys + 1, scr64.p, st);
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+}
+
 // mean radius of the non-empty boxes of every level, summed in box order on the host ("average box radius";
 // the oracle sums in the same order, so the comparison of two levels takes the same decision on both sides)
 static std::vector<double> mean_radii(const Plan& P, cudaStream_t st) {
@@ -735,34 +764,6 @@ static void build_lists_cross(Plan& P, cudaStream_t st) {
     (void)nch;
     if (n_weak > 0x7fffff00ll || nfail > 0x7fffff00ll) { set_error("interaction lists exceed 2^31 pairs"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
 
-    // canonical form: stable sort by target id (steps concatenated in chronological order), CSR offsets by counting
-    auto sort_by_key = [&](DevBuf<int32_t>& keys, DevBuf<int32_t>& vals, int64_t n, int64_t n_keys, int64_t* off_out /*n_keys + 1, device*/) {
-        DevBuf<unsigned long long> cnt;
-        DevBuf<int64_t> scr64;
-        cnt.alloc(n_keys + 1);
-        scr64.alloc(scan_scratch_elems(n_keys + 1));
-        FMM_CUDA_CHECK(cudaMemsetAsync(cnt.p, 0, (n_keys + 1) * sizeof(unsigned long long), st));
-        if (n > 0) {
-            int bits = 8;
-            while (((int64_t)1 << bits) < n_keys) bits += 8;
-            DevBuf<int32_t> kb, vb, hist, scr;
-            kb.alloc(n); vb.alloc(n);
-            const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
-            hist.alloc((size_t)256 * nblk + 1);
-            scr.alloc(scan_scratch_elems((int64_t)256 * nblk));
-            const int where = radix_sort_pairs<uint32_t>(reinterpret_cast<uint32_t*>(keys.p), vals.p, reinterpret_cast<uint32_t*>(kb.p), vb.p, n, bits,
-                                                         hist.p, scr.p, st);
-            if (where == 1) {
-                FMM_CUDA_CHECK(cudaMemcpyAsync(keys.p, kb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-                FMM_CUDA_CHECK(cudaMemcpyAsync(vals.p, vb.p, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-            }
-            count_keys_k<<<nblocks(n, 256), 256, 0, st>>>(keys.p, n, cnt.p);
-            FMM_CUDA_CHECK(cudaGetLastError());
-            FMM_CUDA_CHECK(cudaStreamSynchronize(st));  // temporaries are freed on scope exit
-        }
-        exclusive_scan<int64_t>(CntLoad{cnt.p, n_keys}, off_out, n_keys + 1, scr64.p, st);
-        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-    };
     P.n_weak = n_weak;
     P.weak_tgt.alloc(n_weak); P.weak_src.alloc(n_weak);
     {
@@ -774,14 +775,14 @@ static void build_lists_cross(Plan& P, cudaStream_t st) {
             o += wn[k];
         }
     }
-    sort_by_key(P.weak_tgt, P.weak_src, n_weak, P.n_boxes, P.weak_off.p);
+    sort_by_key(P.weak_tgt, P.weak_src, n_weak, P.n_boxes, P.weak_off.p, st);
     for (int l = 0; l <= L + 1; ++l)  // weak pairs are sorted by target id, hence by target level
         FMM_CUDA_CHECK(cudaMemcpyAsync(&P.weak_level_off[l], P.weak_off.p + P.level_off[l], sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     // strong list = pairs still failing at (L, L) (rule L3)
     P.n_strong = nfail;
     P.strong_off.alloc(P.n_leaves + 1);
     P.strong_src.alloc(nfail);
-    sort_by_key(ftgt, fsrc, nfail, P.n_leaves, P.strong_off.p);
+    sort_by_key(ftgt, fsrc, nfail, P.n_leaves, P.strong_off.p, st);
     FMM_CUDA_CHECK(cudaMemcpyAsync(P.strong_src.p, fsrc.p, nfail * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     FMM_CUDA_CHECK(cudaStreamSynchronize(st));
 }
@@ -890,6 +891,78 @@ void build_lists(Plan& P, cudaStream_t st) {
     cudaEventElapsedTime(&ms, e0, e1);
     P.plan_ms[2] = ms;
     cudaEventDestroy(e0); cudaEventDestroy(e1);
+}
+
+
+// ---------------------------------------------------------------------------------------------- adjoint view
+// The transposed evaluate runs the forward kernels on a VIEW of the plan with the roles of sources and targets exchanged: the view's
+// target hierarchy is the plan's source hierarchy and vice versa (all hierarchy arrays are aliases, nothing is copied), and its
+// interaction lists are the plan's lists transposed: weak pairs sorted by (source, target), strong list CSR by source leaf.
+namespace {
+__global__ void expand_rows_k(const int64_t* off, int64_t n_rows, int32_t* row_of) {  // CSR offsets -> row index per entry (warp per row)
+    const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (r >= n_rows) return;
+    for (int64_t e = off[r] + (threadIdx.x & 31); e < off[r + 1]; e += 32) row_of[e] = (int32_t)r;
+}
+
+void alias_hierarchy(Plan& V, const Plan& H) {
+    V.device = H.device;
+    V.N = H.N; V.p = H.p; V.N_max = H.N_max; V.s = H.s; V.L = H.L; V.dtype = H.dtype; V.theta = H.theta;
+    V.K = H.K; V.Kp = H.Kp; V.n_boxes = H.n_boxes; V.n_leaves = H.n_leaves; V.level_off = H.level_off; V.max_leaf = H.max_leaf;
+    V.perm.alias(H.perm); V.pos_tree.alias(H.pos_tree); V.box_start.alias(H.box_start); V.box_count.alias(H.box_count);
+    V.box_lo.alias(H.box_lo); V.box_hi.alias(H.box_hi); V.box_ctr.alias(H.box_ctr); V.box_rad.alias(H.box_rad); V.box_scale.alias(H.box_scale);
+    V.srcg.alias(H.srcg); V.src_slot.alias(H.src_slot); V.src_G = H.src_G;
+    V.pq.alias(H.pq);
+}
+}  // namespace
+
+void build_adjoint_view(Plan& P, cudaStream_t st) {
+    if (P.adj) return;
+    const Plan& HS = P.S ? *P.S : P;  // hierarchy of the plan's sources = the view's targets
+    std::unique_ptr<Plan> Vp(new Plan());
+    Plan& V = *Vp;
+    alias_hierarchy(V, HS);
+    V.cross_level = 1;
+    V.no_split = true;  // a transposed weak pair may join a target with a COARSER source: the whole upward pass must precede the M2L
+    V.m2l_variant = P.m2l_variant;
+    if (P.S) {
+        V.S.reset(new Plan());
+        alias_hierarchy(*V.S, P);
+        V.S->Mc.alias(P.Lc);   // multipoles of the view's sources live on the plan's target hierarchy: its local array is free
+        V.Lc.alias(P.S->Mc);   // and the other way round
+    } else {
+        V.Mc.alias(P.Lc);
+        V.Lc.alias(P.Mc);
+    }
+    const size_t es = P.dtype == FMM_F32 ? 4 : 8;
+    V.near.alloc((size_t)V.N * 4 * es);
+    // weak list: (target, source) pairs of the plan -> keys = source, values = target; the plan's order (target, source) and a
+    // stable sort by source give the canonical order (source, target) of the view
+    V.n_weak = P.n_weak;
+    V.weak_tgt.alloc(P.n_weak); V.weak_src.alloc(P.n_weak);
+    V.weak_off.alloc(V.n_boxes + 1);
+    if (P.n_weak > 0) {
+        FMM_CUDA_CHECK(cudaMemcpyAsync(V.weak_tgt.p, P.weak_src.p, P.n_weak * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(V.weak_src.p, P.weak_tgt.p, P.n_weak * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    }
+    sort_by_key(V.weak_tgt, V.weak_src, P.n_weak, V.n_boxes, V.weak_off.p, st);
+    // strong list: CSR by target leaf -> (target leaf, source leaf) pairs -> CSR by source leaf
+    V.n_strong = P.n_strong;
+    DevBuf<int32_t> keys, vals;
+    keys.alloc(P.n_strong); vals.alloc(P.n_strong);
+    V.strong_off.alloc(V.n_leaves + 1);
+    V.strong_src.alloc(P.n_strong);
+    if (P.n_strong > 0) {
+        FMM_CUDA_CHECK(cudaMemcpyAsync(keys.p, P.strong_src.p, P.n_strong * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        expand_rows_k<<<nblocks(P.n_leaves * 32, 256), 256, 0, st>>>(P.strong_off.p, P.n_leaves, vals.p);
+        FMM_CUDA_CHECK(cudaGetLastError());
+    }
+    sort_by_key(keys, vals, P.n_strong, V.n_leaves, V.strong_off.p, st);
+    if (P.n_strong > 0) FMM_CUDA_CHECK(cudaMemcpyAsync(V.strong_src.p, vals.p, P.n_strong * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    finish_lists(V, st);
+    if (m2l_geo_wanted(V.p, V.dtype) && V.n_weak > 0) m2l_geo_prepare(V, st);
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    P.adj = std::move(Vp);
 }
 
 }  // namespace fmm

@@ -16,7 +16,7 @@ FMM_OK, FMM_ERR_INVALID_ARG, FMM_ERR_ALLOC, FMM_ERR_CUDA, FMM_ERR_UNSUPPORTED = 
 FMM_F32, FMM_F64 = 0, 1
 FMM_P_MAX = 16
 
-EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
+EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
            "fmm_version", "fmm_translation_work", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
@@ -45,6 +45,7 @@ def lib():
         L.fmm_plan_create.argtypes = [vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
         L.fmm_evaluate.argtypes = [vp, vp, vp, vp, vp]
         L.fmm_evaluate_host.argtypes = [vp, vp, vp, vp, vp]
+        L.fmm_evaluate_adjoint.argtypes = [vp, vp, vp, vp, vp]
         L.fmm_evaluate_profiled.argtypes = [vp, vp, vp, vp, vp, dp]
         L.fmm_plan_destroy.argtypes = [vp]
         L.fmm_plan_info.argtypes = [vp, C.POINTER(C.c_int), i64p, i64p, i64p, i64p, i64p]
@@ -201,6 +202,16 @@ def fmm_evaluate(plan, charges, potential=None, field=None, stream=None):
                               C.c_void_p(field.data_ptr()) if field is not None else None, _stream_ptr(stream)))
 
 
+def fmm_evaluate_adjoint(plan, cot_potential, cot_field, charge_grad, stream=None):
+    """charge_grad (Ns,) = A^T cot_potential + F^T cot_field: the VJP of fmm_evaluate with respect to the charges.
+    cot_potential (Nt,) and / or cot_field (Nt,3): contiguous CUDA tensors of the plan's dtype; one of them may be None."""
+    if cot_potential is None and cot_field is None:
+        raise ValueError("at least one cotangent is needed")
+    _check_io(plan, charge_grad, cot_potential, cot_field)
+    p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().fmm_evaluate_adjoint(plan, p(cot_potential), p(cot_field), p(charge_grad), _stream_ptr(stream)))
+
+
 def fmm_evaluate_profiled(plan, charges, potential=None, field=None, stream=None):
     _check_io(plan, charges, potential, field)
     ms = (C.c_double * 8)()
@@ -300,6 +311,13 @@ class Plan:
         fmm_evaluate(self.handle, charges, pot, fld, stream)
         return pot, fld
 
+    def evaluate_adjoint(self, cot_potential=None, cot_field=None, stream=None):
+        """gradient of <cot_potential, potential> + <cot_field, field> with respect to the charges (N,)"""
+        import torch
+        g = torch.empty(self.N, dtype=self.tdtype, device=self.device)
+        fmm_evaluate_adjoint(self.handle, cot_potential, cot_field, g, stream)
+        return g
+
     def tree(self):
         return fmm_plan_copy_tree(self.handle, self.N, self.dtype)
 
@@ -340,6 +358,13 @@ class PlanTargets:
         fld = torch.empty((self.Nt, 3), dtype=self.tdtype, device=self.device) if want_field else None
         fmm_evaluate(self.handle, charges, pot, fld, stream)
         return pot, fld
+
+    def evaluate_adjoint(self, cot_potential=None, cot_field=None, stream=None):
+        """gradient of <cot_potential, potential> + <cot_field, field> with respect to the source charges (Ns,)"""
+        import torch
+        g = torch.empty(self.Ns, dtype=self.tdtype, device=self.device)
+        fmm_evaluate_adjoint(self.handle, cot_potential, cot_field, g, stream)
+        return g
 
     def tree(self, which):
         """which: 'tgt' or 'src'"""
