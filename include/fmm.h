@@ -118,6 +118,18 @@ fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* 
 fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void* d_targets, int64_t Nt, int p, int N_max, int s,
                                    const fmm_admissibility* adm, fmm_dtype dtype, void* cuda_stream, fmm_plan** out_plan);
 
+/* Re-plan for moved points (in jaxFMM every change of the positions costs a new gen_hierarchy, minutes with
+ * JIT): rebuilds hierarchy and interaction lists of an existing plan for new positions of the SAME number of points, with the
+ * plan's p, N_max, s, theta, list kind and dtype.  The result is exactly the plan fmm_plan_create would build for these positions
+ * (same kernels: hierarchy and lists bit-exact against the oracle); what is saved is every allocation -- all arrays whose size
+ * depends only on N stay in place, the evaluate scratch and the internal streams are kept -- and, for a plan with separate targets,
+ * the hierarchy of the side that did not move.
+ *   one point set   : d_positions = DEVICE, N x 3, dtype;  d_targets must be NULL.
+ *   separate targets: d_positions = new sources (Ns x 3) or NULL (unchanged), d_targets = new targets (Nt x 3) or NULL (unchanged).
+ * Waits for the device to be idle, then runs on cuda_stream and synchronises it.  On failure (e.g. non-finite positions ->
+ * FMM_ERR_INVALID_ARG) the plan is left without a valid hierarchy: update it again with valid positions or destroy it. */
+fmm_status fmm_plan_update(fmm_plan* plan, const void* d_positions, const void* d_targets, void* cuda_stream);
+
 /* Source hierarchy of a plan (HOST outputs, any may be NULL); for a plan made by fmm_plan_create it is the one hierarchy. */
 fmm_status fmm_plan_source_info(const fmm_plan* plan, int64_t* Ns, int* L, int64_t* n_boxes, int64_t* n_leaves);
 /* As fmm_plan_copy_tree, for the source hierarchy (sizes from fmm_plan_source_info). */

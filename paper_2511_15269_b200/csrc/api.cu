@@ -242,6 +242,45 @@ fmm_status fmm_plan_create_targets(const void* d_sources, int64_t Ns, const void
     });
 }
 
+fmm_status fmm_plan_update(fmm_plan* plan, const void* d_positions, const void* d_targets, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        g_err.clear();
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        Plan& P = plan->P;
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
+        if (!P.S && (!d_positions || d_targets)) { set_error("a plan over one point set takes d_positions and d_targets == NULL"); return FMM_ERR_INVALID_ARG; }
+        if (P.S && !d_positions && !d_targets) { set_error("nothing to update"); return FMM_ERR_INVALID_ARG; }
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
+        FMM_CUDA_CHECK(cudaDeviceSynchronize());  // no evaluate of this plan may still be reading the arrays that are rebuilt
+        cudaEvent_t e0, e1;
+        FMM_CUDA_CHECK(cudaEventCreate(&e0));
+        FMM_CUDA_CHECK(cudaEventCreate(&e1));
+        FMM_CUDA_CHECK(cudaEventRecord(e0, st));
+        P.adj.reset();  // the transposed lists belong to the old positions
+        double sort_ms = 0, tree_ms = 0;
+        if (P.S) {
+            if (d_positions) { build_tree(*P.S, d_positions, st); sort_ms += P.S->plan_ms[0]; tree_ms += P.S->plan_ms[1]; }
+            if (d_targets) { build_tree(P, d_targets, st); sort_ms += P.plan_ms[0]; tree_ms += P.plan_ms[1]; }
+        } else {
+            build_tree(P, d_positions, st);
+            sort_ms = P.plan_ms[0]; tree_ms = P.plan_ms[1];
+        }
+        P.plan_ms[0] = sort_ms; P.plan_ms[1] = tree_ms;
+        build_lists(P, st);
+        if (m2l_geo_wanted(P.p, P.dtype) && P.n_weak > 0) m2l_geo_prepare(P, st);
+        else P.m2l_geo.release();
+        FMM_CUDA_CHECK(cudaEventRecord(e1, st));
+        FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        P.plan_ms[3] = ms;
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+        return FMM_OK;
+    });
+}
+
 fmm_status fmm_plan_source_info(const fmm_plan* plan, int64_t* Ns, int* L, int64_t* n_boxes, int64_t* n_leaves) {
     if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
     const Plan& S = plan->P.S ? *plan->P.S : plan->P;

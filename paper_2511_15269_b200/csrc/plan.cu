@@ -138,6 +138,63 @@ __global__ void partition_k(const int32_t* ord_in, int32_t* ord_out, const int32
     ord_out[dest] = pt;
 }
 
+// ---- the four orderings (x, y, z, index) of one sub-split in ONE launch per phase (blockIdx.y = ordering): the rounds are
+// latency-bound (150 launches of ~10 us at N = 1M when every ordering has its own scan and partition kernels)
+struct Ord4 {
+    const int32_t* in[4];
+    int32_t* out[4];
+};
+__global__ void __launch_bounds__(SCAN_THREADS) flag4_reduce_k(const uint8_t* pflag, Ord4 o, int64_t N, int32_t* block_sums, int64_t nb) {
+    __shared__ int32_t sm[33];
+    const int32_t* ord = o.in[blockIdx.y];
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i)
+        if (base + i < N) s += pflag[ord[base + i]];
+    int32_t tot;
+    block_exclusive_scan<int32_t>(s, &tot, sm);
+    if (threadIdx.x == 0) block_sums[blockIdx.y * nb + blockIdx.x] = tot;
+}
+// exclusive scan of the nb <= SCAN_TILE block sums of each ordering, one block per ordering, in place
+__global__ void __launch_bounds__(SCAN_THREADS) flag4_sums_k(int32_t* block_sums, int64_t nb) {
+    __shared__ int32_t sm[33];
+    int32_t* b = block_sums + blockIdx.y * nb;
+    const int64_t base = (int64_t)threadIdx.x * SCAN_ITEMS;
+    int32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { v[i] = base + i < nb ? b[base + i] : 0; s += v[i]; }
+    int32_t off = block_exclusive_scan<int32_t>(s, nullptr, sm);
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { if (base + i < nb) b[base + i] = off; off += v[i]; }
+}
+// F[y][i] = number of flagged particles before position i of ordering y (i = 0..N; F has N + 1 entries per ordering)
+__global__ void __launch_bounds__(SCAN_THREADS) flag4_apply_k(const uint8_t* pflag, Ord4 o, int64_t N, const int32_t* block_offs, int64_t nb, int32_t* F) {
+    __shared__ int32_t sm[33];
+    const int32_t* ord = o.in[blockIdx.y];
+    int32_t* Fy = F + blockIdx.y * (N + 1);
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { v[i] = base + i < N ? (int32_t)pflag[ord[base + i]] : 0; s += v[i]; }
+    int32_t off = block_exclusive_scan<int32_t>(s, nullptr, sm) + block_offs[blockIdx.y * nb + blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { if (base + i <= N) Fy[base + i] = off; off += v[i]; }
+}
+__global__ void partition4_k(Ord4 o, const int32_t* F, const uint8_t* pflag, const int32_t* pnode, const int32_t* nstart, const int32_t* nstart2, int64_t N) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int32_t* Fy = F + blockIdx.y * (N + 1);
+    const int32_t pt = o.in[blockIdx.y][i];
+    const int32_t nd = pnode[pt];
+    const int32_t s0 = nstart[nd];
+    const int32_t ups = Fy[i] - Fy[s0];  // flagged elements of this node before position i
+    int32_t dest;
+    if (pflag[pt]) dest = nstart2[2 * nd + 1] + ups;
+    else dest = nstart2[2 * nd] + ((int32_t)i - s0) - ups;
+    o.out[blockIdx.y][dest] = pt;
+}
+
 __global__ void pnode_update_k(int32_t* pnode, const uint8_t* pflag, int64_t N) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) pnode[i] = 2 * pnode[i] + pflag[i];
@@ -211,7 +268,11 @@ void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
     scan_scratch.alloc((size_t)std::max(scan_scratch_elems((int64_t)256 * nblk), scan_scratch_elems(N + 1)));
     for (int a = 0; a < 3; ++a) rank[a].alloc(N);
     for (int a = 0; a < 4; ++a) { ordA[a].alloc(N); ordB[a].alloc(N); }
-    pnode.alloc(N); F.alloc(N + 1); pflag.alloc(N);
+    const int64_t nb_scan = (N + 1 + SCAN_TILE - 1) / SCAN_TILE;
+    const bool fused4 = nb_scan <= SCAN_TILE;  // the block sums of one ordering fit one scan block (N <= 4.19M); else one ordering at a time
+    DevBuf<int32_t> sums4;
+    if (fused4) sums4.alloc((size_t)4 * nb_scan);
+    pnode.alloc(N); F.alloc(fused4 ? 4 * (N + 1) : N + 1); pflag.alloc(N);
     bad.alloc(1);
     FMM_CUDA_CHECK(cudaMemsetAsync(bad.p, 0, sizeof(int), st));
 
@@ -265,12 +326,22 @@ void build_tree_t(Plan& P, const T* pos, cudaStream_t st) {
         if (is_last) break;
         pflag_k<<<nblocks(N, 256), 256, 0, st>>>(pnode.p, rank[0].p, rank[1].p, rank[2].p, naxis.p, npivot.p, pflag.p, N);
         FMM_CUDA_CHECK(cudaGetLastError());
-        for (int a = 0; a < 4; ++a) {
-            exclusive_scan<int32_t, FlagLoad>(FlagLoad{pflag.p, oa[a], N}, F.p, N + 1, scan_scratch.p, st);
-            partition_k<<<nblocks(N, 256), 256, 0, st>>>(oa[a], ob[a], F.p, pflag.p, pnode.p, nstart[cur].p, nstart[cur ^ 1].p, N);
+        if (fused4) {
+            Ord4 o4;
+            for (int a = 0; a < 4; ++a) { o4.in[a] = oa[a]; o4.out[a] = ob[a]; }
+            flag4_reduce_k<<<dim3((unsigned)nb_scan, 4), SCAN_THREADS, 0, st>>>(pflag.p, o4, N, sums4.p, nb_scan);
+            flag4_sums_k<<<dim3(1, 4), SCAN_THREADS, 0, st>>>(sums4.p, nb_scan);
+            flag4_apply_k<<<dim3((unsigned)nb_scan, 4), SCAN_THREADS, 0, st>>>(pflag.p, o4, N, sums4.p, nb_scan, F.p);
+            partition4_k<<<dim3(nblocks(N, 256), 4), 256, 0, st>>>(o4, F.p, pflag.p, pnode.p, nstart[cur].p, nstart[cur ^ 1].p, N);
             FMM_CUDA_CHECK(cudaGetLastError());
-            std::swap(oa[a], ob[a]);
-        }
+            for (int a = 0; a < 4; ++a) std::swap(oa[a], ob[a]);
+        } else
+            for (int a = 0; a < 4; ++a) {
+                exclusive_scan<int32_t, FlagLoad>(FlagLoad{pflag.p, oa[a], N}, F.p, N + 1, scan_scratch.p, st);
+                partition_k<<<nblocks(N, 256), 256, 0, st>>>(oa[a], ob[a], F.p, pflag.p, pnode.p, nstart[cur].p, nstart[cur ^ 1].p, N);
+                FMM_CUDA_CHECK(cudaGetLastError());
+                std::swap(oa[a], ob[a]);
+            }
         pnode_update_k<<<nblocks(N, 256), 256, 0, st>>>(pnode.p, pflag.p, N);
         FMM_CUDA_CHECK(cudaGetLastError());
         n_d = (n_d + 1) / 2;

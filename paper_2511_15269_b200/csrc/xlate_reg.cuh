@@ -121,6 +121,26 @@ __device__ __forceinline__ void trig_table(T c1, T s1, T (&c)[P1], T (&s)[P1]) {
 // the azimuthal code (35 KB of SASS at p = 8, 48 KB with prologue and epilogue); this form is 20 KB, so the whole kernel
 // stays inside the 32 KB instruction cache of an SM.  Measured on B200 with a synthetic FFMA stream (4 warps per
 // scheduler): bodies up to 32 KB issue at 0.97 instructions per clock and scheduler, bodies of 48 KB and more at 0.5.
+// Matrix entries are immediates of the FMA that uses them (fp32) or are materialised by two uniform moves (fp64).  Measured: taking
+// the fp64 entries from a 59 KB __constant__ table instead (one LDC / LDCU per one or two entries) makes the fp64 p = 8 M2L 1.7x
+// slower (2.64 vs 1.55 ms at N = 1M): the table does not fit the constant cache.
+template <typename T, int n, int i, int j>
+__device__ __forceinline__ T q_coef() {
+    constexpr double v = ct::kTab.Q[ct::boff(n) + i * (2 * n + 1) + j];
+    return T(v);
+}
+// sg * H[am][n][k] / sg * A[am][n][k] with sg = +-1 (the sign is an operand modifier of the instruction that uses it)
+template <typename T, int am, int n, int k, bool NEG>
+__device__ __forceinline__ T h_coef() {
+    constexpr double v = NEG ? -ct::kTab.H[am][n][k] : ct::kTab.H[am][n][k];
+    return T(v);
+}
+template <typename T, int am, int n, int k, bool NEG>
+__device__ __forceinline__ T a_coef() {
+    constexpr double v = NEG ? -ct::kTab.A[am][n][k] : ct::kTab.A[am][n][k];
+    return T(v);
+}
+
 template <int n>
 constexpr double qent(int i, int j) {
     return ct::kTab.Q[ct::boff(n) + i * (2 * n + 1) + j];
@@ -143,8 +163,8 @@ __device__ __forceinline__ void q_from_to(const T (&src)[NS], T (&dst)[ND]) {
             constexpr int j = decltype(jc)::value;
             constexpr double b = qent<n>(i, j);
             if constexpr (b != 0.0) {
-                if constexpr (qfirst<n>(i, j)) acc = T(b) * src[os + j];
-                else acc = fma(T(b), src[os + j], acc);
+                if constexpr (qfirst<n>(i, j)) acc = q_coef<T, n, i, j>() * src[os + j];
+                else acc = fma(q_coef<T, n, i, j>(), src[os + j], acc);
             }
         });
         dst[od + i] = acc;
@@ -180,12 +200,10 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
             T t[cnt];
             sfor<cnt>([&](auto ni) {
                 constexpr int n = am + decltype(ni)::value;
-                constexpr double h0 = sg * ct::kTab.H[am][n][am];
-                T acc = T(h0) * v[am * am + am + m];
+                T acc = h_coef<T, am, n, am, (sg < 0)>() * v[am * am + am + m];
                 sfor<cnt - 1>([&](auto ki) {
                     constexpr int k = am + 1 + decltype(ki)::value;
-                    constexpr double h = sg * ct::kTab.H[am][n][k];
-                    acc = fma(T(h), v[k * k + k + m], acc);
+                    acc = fma(h_coef<T, am, n, k, (sg < 0)>(), v[k * k + k + m], acc);
                 });
                 t[decltype(ni)::value] = acc;
             });
@@ -218,8 +236,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
                     T acc = (am & 1) ? T(0) - v[n * n + n + m] : v[n * n + n + m];
                     sfor<n - am>([&](auto ki) {
                         constexpr int k = am + decltype(ki)::value;
-                        constexpr double aa = sg * ct::kTab.A[am][n][k];
-                        acc = fma(T(aa) * pw1[n - k], v[k * k + k + m], acc);
+                        acc = fma(a_coef<T, am, n, k, (sg < 0)>() * pw1[n - k], v[k * k + k + m], acc);
                     });
                     v[n * n + n + m] = acc;
                 });
@@ -237,8 +254,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
                     T acc = v[n * n + n + m];
                     sfor<P - n>([&](auto ki) {
                         constexpr int k = n + 1 + decltype(ki)::value;
-                        constexpr double aa = ct::kTab.A[am][k][n];
-                        acc = fma(T(aa) * pw1[k - n], v[k * k + k + m], acc);
+                        acc = fma(a_coef<T, am, k, n, false>() * pw1[k - n], v[k * k + k + m], acc);
                     });
                     v[n * n + n + m] = acc * (T(sg) * pw2[n]);
                 });

@@ -18,7 +18,7 @@ FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
-           "fmm_version", "fmm_translation_work", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
+           "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
 
 class fmm_admissibility(C.Structure):
@@ -52,6 +52,7 @@ def lib():
         L.fmm_plan_copy_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
         L.fmm_plan_copy_lists.argtypes = [vp, i64p, i32p, i64p, i32p]
         L.fmm_plan_create_targets.argtypes = [vp, C.c_int64, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
+        L.fmm_plan_update.argtypes = [vp, vp, vp, vp]
         L.fmm_plan_source_info.argtypes = [vp, i64p, C.POINTER(C.c_int), i64p, i64p]
         L.fmm_plan_copy_source_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
         L.fmm_plan_copy_march.argtypes = [vp, i32p, i32p]
@@ -159,6 +160,20 @@ def fmm_plan_create_targets(sources, targets, p, N_max, s, theta=0.77, stream=No
                                          int(N_max), int(s), C.byref(adm), _dtype_code(sources), _stream_ptr(stream), C.byref(h)))
     _PLANS[h.value] = (sources.dtype, sources.shape[0], targets.shape[0], sources.device)
     return h
+
+
+def fmm_plan_update(plan, positions=None, targets=None, stream=None):
+    """Re-plan in place for moved points (same counts, dtype and parameters).  One point set: `positions`; separate targets:
+    `positions` = new sources and / or `targets` = new targets (None = unchanged)."""
+    meta = _PLANS.get(plan.value)
+    if meta is None:
+        raise ValueError("unknown or destroyed plan handle")
+    tdtype, Nq, Nt, device = meta
+    for t, n in ((positions, Nq), (targets, Nt)):
+        if t is not None and (not t.is_cuda or not t.is_contiguous() or t.dtype != tdtype or tuple(t.shape) != (n, 3) or t.device != device):
+            raise ValueError("new positions must be contiguous CUDA tensors of shape (%d, 3) and dtype %s on %s" % (n, tdtype, device))
+    p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().fmm_plan_update(plan, p(positions), p(targets), _stream_ptr(stream)))
 
 
 def fmm_plan_source_info(plan):
@@ -311,6 +326,11 @@ class Plan:
         fmm_evaluate(self.handle, charges, pot, fld, stream)
         return pot, fld
 
+    def update(self, positions, stream=None):
+        """re-plan in place for moved points (fmm_plan_update)"""
+        fmm_plan_update(self.handle, positions, None, stream)
+        self.info = fmm_plan_info(self.handle)
+
     def evaluate_adjoint(self, cot_potential=None, cot_field=None, stream=None):
         """gradient of <cot_potential, potential> + <cot_field, field> with respect to the charges (N,)"""
         import torch
@@ -358,6 +378,12 @@ class PlanTargets:
         fld = torch.empty((self.Nt, 3), dtype=self.tdtype, device=self.device) if want_field else None
         fmm_evaluate(self.handle, charges, pot, fld, stream)
         return pot, fld
+
+    def update(self, sources=None, targets=None, stream=None):
+        """re-plan in place for moved sources and / or targets (fmm_plan_update)"""
+        fmm_plan_update(self.handle, sources, targets, stream)
+        self.info = fmm_plan_info(self.handle)
+        self.source_info = fmm_plan_source_info(self.handle)
 
     def evaluate_adjoint(self, cot_potential=None, cot_field=None, stream=None):
         """gradient of <cot_potential, potential> + <cot_field, field> with respect to the source charges (Ns,)"""
