@@ -311,7 +311,10 @@ def run_ours(args):
     fmm.lib()  # fail loudly if the CUDA extension is missing
     peaks = load_peaks()
 
-    pos, q, c = make_workload(args.workload, rank)
+    # --sharded (N > 1): ONE problem, its targets sharded over the ranks (fmm.evaluate_sharded: upward pass of the own leaves, one NCCL
+    # all-gather of the leaf multipoles, downward pass of the own targets): "scaling": "strong".  Default: independent replicas.
+    sharded = bool(args.sharded) and world > 1
+    pos, q, c = make_workload(args.workload, 0 if sharded else rank)
     N = pos.shape[0]
     tdt = torch.float32 if pos.dtype == np.float32 else torch.float64
     esize = pos.dtype.itemsize
@@ -325,6 +328,12 @@ def run_ours(args):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
     launches = fmm.fmm_plan_launches(P.handle)
 
+    def step():
+        if sharded:
+            fmm.evaluate_sharded(P.handle, info["n_leaves"], d_q, d_u, d_f)
+        else:
+            fmm.fmm_evaluate(P.handle, d_q, d_u, d_f)
+
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
@@ -333,7 +342,7 @@ def run_ours(args):
 
     for _ in range(max(args.warmup, 3)):
         flush.zero_()
-        fmm.fmm_evaluate(P.handle, d_q, d_u, d_f)
+        step()
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -341,7 +350,7 @@ def run_ours(args):
     for a, b in ev:
         flush.zero_()
         a.record()
-        fmm.fmm_evaluate(P.handle, d_q, d_u, d_f)
+        step()
         b.record()
     barrier()
     t_wall = time.perf_counter() - t_wall0
@@ -426,6 +435,8 @@ def run_ours(args):
         del d_tgt, d_ut, d_ft
 
     ms_per_step, value, e2e_ms_max, e2e_value = aggregate_over_ranks(total_ms, e2e_ms, N, args.steps, world, "cuda")
+    if sharded:  # one problem of N particles, not `world` of them
+        value, e2e_value = value / world, e2e_value / world
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -488,11 +499,12 @@ def run_ours(args):
         cpu_baseline = oracle_baseline(pos, q, c, full=not args.cpu_sample)
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms_per_step,
-                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if esize == 4 else "f64", data="synthetic",
+                higher_is_better=True, scaling="strong" if sharded else "weak", vs_baseline=None, dtype="f32" if esize == 4 else "f64", data="synthetic",
                 config=dict(workload=args.workload, N=N, p=c["p"], s=c["s"], N_max=c["N_max"], theta=c["theta"], cross_level=args.cross_level,
                             outputs="potential+field",
                             L=info["L"], n_boxes=info["n_boxes"], n_weak=info["n_weak"], n_strong=info["n_strong"], n_p2p_pairs=info["n_p2p_pairs"],
-                            l2="flushed between timed steps (512 MiB memset outside the event pairs)", parallelism="replicas x%d" % world,
+                            l2="flushed between timed steps (512 MiB memset outside the event pairs)", parallelism=("targets sharded x%d (one all-gather of leaf multipoles per step; e2e is the unsharded host path of each rank)" % world) if sharded
+                            else "replicas x%d" % world,
                             schedule="concurrent: P2P, the tree passes (M2M, upper-level M2L, L2L) and the leaf-level M2L on three forked streams"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=N * esize, d2h_bytes_per_step=N * 4 * esize,
                                         ms_per_step=e2e_ms_max, steps=n_e2e),
@@ -572,6 +584,8 @@ def main():
                     help="interaction lists of the timed plan: 0 = same-level (paper default, PAPER.md:72-74), 1 = level marching (PAPER.md:82-89)")
     ap.add_argument("--no-extras", "--no-alt-lists", dest="no_extras", action="store_true",
                     help="skip the extra measurements (the other list kind, potential only, re-plan, separate targets)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: one problem with its targets sharded over the ranks (strong scaling) instead of independent replicas")
     ap.add_argument("--sweep", action="store_true", help="run the config-5 grid instead of the headline")
     ap.add_argument("--sweep-out", default=None, help="write the markdown table of --sweep here")
     ap.add_argument("--sweep-sets", default="cube,sphere")

@@ -98,6 +98,30 @@ fmm_status fmm_evaluate(const fmm_plan* plan, const void* d_charges, void* d_pot
 fmm_status fmm_evaluate_adjoint(fmm_plan* plan, const void* d_cotangent_potential, const void* d_cotangent_field, void* d_charge_grad,
                                 void* cuda_stream);
 
+/* Target-sharded evaluate for several GPUs (the paper has no multi-device support).  Every rank holds
+ * the same plan (the positions are replicated; building it costs milliseconds) and all charges, and owns the targets of a contiguous
+ * range of leaves -- a set of subtrees, because the tree order is a Z-order: shard r of n owns the leaves
+ * [n_leaves r / n, n_leaves (r+1) / n).  One evaluate is
+ *     fmm_evaluate_shard_upward   : permute, P2M for the shard's leaves (1/n of the work)
+ *     <all-gather of the leaf rows of the multipole array among the ranks>   -- the ONE data-path collective; the caller runs it
+ *                                   (paper_2511_15269_b200/fmm.py: NCCL through torch.distributed) on the rows that
+ *                                   fmm_plan_leaf_multipoles copies out of / into the plan
+ *     fmm_evaluate_shard_downward : M2M (all boxes, redundant: 0.05 ms), M2L and L2L for the shard's boxes and their ancestors,
+ *                                   P2P and L2P for its leaves; writes potential / field of the shard's particles ONLY (input order;
+ *                                   the other entries of the output arrays are not touched).
+ * Both calls are asynchronous on cuda_stream (the first downward call of a shard reads a few list offsets back and synchronises).
+ * Plans over one point set, orders 1..12 (the specialised kernels), m2l_variant 0; FMM_ERR_UNSUPPORTED otherwise.
+ * fmm_shard_box_range needs no device: the level-local range of boxes of `level` that a shard touches (its leaves for level = L,
+ * their ancestors above), for a tree of depth L with 2^s children per box. */
+fmm_status fmm_shard_box_range(int L, int s, int n_shards, int shard, int level, int64_t* h_begin, int64_t* h_end);
+fmm_status fmm_evaluate_shard_upward(const fmm_plan* plan, int n_shards, int shard, const void* d_charges, void* cuda_stream);
+fmm_status fmm_evaluate_shard_downward(const fmm_plan* plan, int n_shards, int shard, void* d_potential, void* d_field, void* cuda_stream);
+/* Leaf rows [leaf_begin, leaf_end) of the plan's multipole array, row = *h_row_elems elements of the plan's dtype ((p+1)^2 rounded up
+ * to a multiple of 4): copy_in = 0 copies them to d_rows (DEVICE), copy_in = 1 copies d_rows into the plan.  d_rows = NULL only
+ * queries the row length.  Asynchronous on cuda_stream. */
+fmm_status fmm_plan_leaf_multipoles(const fmm_plan* plan, int copy_in, int64_t leaf_begin, int64_t leaf_end, void* d_rows, int64_t* h_row_elems,
+                                    void* cuda_stream);
+
 /* Same operation with HOST buffers: copies charges host->device, evaluates, copies the results back and
  * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);

@@ -258,6 +258,7 @@ fmm_status fmm_plan_update(fmm_plan* plan, const void* d_positions, const void* 
         FMM_CUDA_CHECK(cudaEventCreate(&e1));
         FMM_CUDA_CHECK(cudaEventRecord(e0, st));
         P.adj.reset();  // the transposed lists belong to the old positions
+        P.shard_cache = Plan::Shard();
         double sort_ms = 0, tree_ms = 0;
         if (P.S) {
             if (d_positions) { build_tree(*P.S, d_positions, st); sort_ms += P.S->plan_ms[0]; tree_ms += P.S->plan_ms[1]; }
@@ -348,6 +349,54 @@ fmm_status fmm_evaluate_adjoint(fmm_plan* plan, const void* d_cotangent_potentia
         const Plan& V = self_adjoint ? P : *P.adj;
         if (!self_adjoint) { P.adj->m2l_variant = P.m2l_variant; P.adj->serial = P.serial; }
         run_evaluate(V, d_cotangent_potential, d_charge_grad, nullptr, st, nullptr, d_cotangent_field);
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_shard_box_range(int L, int s, int n_shards, int shard, int level, int64_t* h_begin, int64_t* h_end) {
+    if (L < 0 || s < 1 || (int64_t)s * L > 30 || n_shards < 1 || shard < 0 || shard >= n_shards || level < 0 || level > L || !h_begin || !h_end) {
+        set_error("bad argument");
+        return FMM_ERR_INVALID_ARG;
+    }
+    shard_box_range(L, s, n_shards, shard, level, h_begin, h_end);
+    return FMM_OK;
+}
+
+fmm_status fmm_evaluate_shard_upward(const fmm_plan* plan, int n_shards, int shard, const void* d_charges, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !d_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
+        AllocScope scope((cudaStream_t)cuda_stream);
+        run_shard_upward(plan->P, n_shards, shard, d_charges, (cudaStream_t)cuda_stream);
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_evaluate_shard_downward(const fmm_plan* plan, int n_shards, int shard, void* d_potential, void* d_field, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
+        AllocScope scope((cudaStream_t)cuda_stream);
+        run_shard_downward(plan->P, n_shards, shard, d_potential, d_field, (cudaStream_t)cuda_stream);
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_plan_leaf_multipoles(const fmm_plan* plan, int copy_in, int64_t leaf_begin, int64_t leaf_end, void* d_rows, int64_t* h_row_elems,
+                                    void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        const Plan& P = plan->P;
+        if (P.S) { set_error("plans with separate targets are not supported"); return FMM_ERR_UNSUPPORTED; }
+        if (h_row_elems) *h_row_elems = P.Kp;
+        if (!d_rows) return FMM_OK;  // query only
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
+        if (leaf_begin < 0 || leaf_end > P.n_leaves || leaf_begin > leaf_end) { set_error("leaf range out of bounds"); return FMM_ERR_INVALID_ARG; }
+        const size_t es = esize(P.dtype), row = (size_t)P.Kp * es;
+        char* blk = P.Mc.p + ((size_t)P.level_off[P.L] + (size_t)leaf_begin) * row;
+        const size_t bytes = (size_t)(leaf_end - leaf_begin) * row;
+        if (bytes) FMM_CUDA_CHECK(cudaMemcpyAsync(copy_in ? (void*)blk : d_rows, copy_in ? (const void*)d_rows : (const void*)blk, bytes, cudaMemcpyDeviceToDevice,
+                                                  (cudaStream_t)cuda_stream));
         return FMM_OK;
     });
 }

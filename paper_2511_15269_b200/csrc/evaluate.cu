@@ -615,27 +615,30 @@ __global__ void __launch_bounds__(P2P_THREADS) p2p_k(const typename V4<T>::type*
     }
 }
 
+// leaves [lo, hi) of the leaf level (hi < 0: all)
 template <typename T, int P, int LPL>
-void launch_p2m_l2p_t(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
+void launch_p2m_l2p_t(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st, int64_t lo, int64_t hi) {
     using T4 = typename V4<T>::type;
-    const int64_t leaf0 = Pl.level_off[Pl.L];
-    const unsigned grid = nblocks(Pl.n_leaves, WARPS_PER_BLOCK * (32 / LPL));
+    if (hi < 0) { lo = 0; hi = Pl.n_leaves; }
+    if (hi <= lo) return;
+    const int64_t leaf0 = Pl.level_off[Pl.L] + lo, nl = hi - lo;
+    const unsigned grid = nblocks(nl, WARPS_PER_BLOCK * (32 / LPL));
     if (!l2p)
         p2m_k<T, P, LPL><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
-                                                                (const T*)Pl.box_scale.p, leaf0, Pl.n_leaves, Pl.Kp, (T*)Pl.Mc.p);
+                                                                (const T*)Pl.box_scale.p, leaf0, nl, Pl.Kp, (T*)Pl.Mc.p);
     else
         l2p_k<T, P, LPL><<<grid, WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)Pl.pq.p, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
-                                                                (const T*)Pl.box_scale.p, leaf0, Pl.n_leaves, Pl.Kp, (const T*)Pl.Lc.p,
+                                                                (const T*)Pl.box_scale.p, leaf0, nl, Pl.Kp, (const T*)Pl.Lc.p,
                                                                 (const T4*)Pl.near.p, Pl.perm.p, (T*)d_pot, (T*)d_field);
 }
 
 template <typename T, int P>
-void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
+void launch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st, int64_t lo, int64_t hi) {
     // leaves of <= 16 particles (e.g. config 4: N_max = 64, s = 3): two leaves per warp.  fp32, p <= 8 only (compile time).
     if constexpr (sizeof(T) == 4 && P <= 8) {
-        if (Pl.max_leaf <= 16) { launch_p2m_l2p_t<T, P, 16>(Pl, l2p, d_pot, d_field, st); return; }
+        if (Pl.max_leaf <= 16) { launch_p2m_l2p_t<T, P, 16>(Pl, l2p, d_pot, d_field, st, lo, hi); return; }
     }
-    launch_p2m_l2p_t<T, P, 32>(Pl, l2p, d_pot, d_field, st);
+    launch_p2m_l2p_t<T, P, 32>(Pl, l2p, d_pot, d_field, st, lo, hi);
 }
 
 template <typename T>
@@ -653,12 +656,27 @@ void dispatch_p2m_dipole(const Plan& Pl, cudaStream_t st) {
 }
 
 template <typename T>
-void dispatch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st) {
+void dispatch_p2m_l2p(const Plan& Pl, bool l2p, void* d_pot, void* d_field, cudaStream_t st, int64_t lo = 0, int64_t hi = -1) {
     switch (Pl.p) {
-#define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, d_pot, d_field, st); break;
+#define FMM_CASE(PP) case PP: launch_p2m_l2p<T, PP>(Pl, l2p, d_pot, d_field, st, lo, hi); break;
         FMM_CASE(0) FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
         FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12) FMM_CASE(13) FMM_CASE(14) FMM_CASE(15) FMM_CASE(16)
 #undef FMM_CASE
+    }
+}
+
+// __constant__ copies of g_n^m: one upload per device
+void ensure_constants(const Plan& P) {
+    DeviceCtx& ctx = device_ctx(P.device);
+    std::lock_guard<std::mutex> lock(ctx.mu);
+    if (!ctx.const_uploaded) {
+        std::vector<double> g(KMAX);
+        std::vector<float> gf(KMAX);
+        FMM_CUDA_CHECK(cudaMemcpy(g.data(), ctx.tab.d_g, KMAX * sizeof(double), cudaMemcpyDeviceToHost));
+        for (int i = 0; i < KMAX; ++i) gf[i] = (float)g[i];
+        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_g, g.data(), KMAX * sizeof(double)));
+        FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
+        ctx.const_uploaded = true;
     }
 }
 
@@ -883,6 +901,101 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     after(st, sF, Pl.e_done);
 }
 
+
+// ------------------------------------------------------------------------------------------------ target-sharded evaluate
+// SURVEY 8(e) / PAPER.md:226 ("distribution of data across multiple GPUs is not yet supported"): targets are independent once the
+// multipoles are known, and a contiguous range of leaves is a set of subtrees (Z-order layout).  Shard r of n owns the
+// leaves [n_leaves r / n, n_leaves (r+1) / n):
+//   upward   : permute all charges (they are replicated), P2M for ITS leaves only;
+//   exchange : the caller all-gathers the leaf rows of the multipole array (the one data-path collective; fmm.py uses NCCL);
+//   downward : M2M for all boxes (cheap, redundant), then M2L / L2L for its boxes and their ancestors only, P2P and L2P for its
+//              leaves -- outputs are written for the shard's particles only.
+template <typename T>
+void shard_upward_t(const Plan& Pl, int64_t lo, int64_t hi, const void* d_q, cudaStream_t st) {
+    using T4 = typename V4<T>::type;
+    permute_k<T><<<nblocks(Pl.N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)Pl.pq.p, Pl.src_slot.p,
+                                                     sizeof(T) == 4 ? Pl.srcg.p : nullptr, Pl.N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    dispatch_p2m_l2p<T>(Pl, false, nullptr, nullptr, st, lo, hi);
+    FMM_CUDA_CHECK(cudaGetLastError());
+}
+
+template <typename T>
+void shard_downward_t(const Plan& Pl, const Plan::Shard& sh, void* d_pot, void* d_field, cudaStream_t st) {
+    const int L = Pl.L;
+    FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, st));
+    if (L > 0) FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), st));
+    for (int l = L; l >= 1; --l) xlate_fast_launch(Pl, 0, l, st);                       // M2M: every box (redundant on every shard)
+    for (int l = 0; l <= L; ++l)
+        if (sh.e1[l] > sh.e0[l]) xlate_fast_launch(Pl, 1, 0, st, sh.e0[l], sh.e1[l]);   // M2L: targets of this shard on level l
+    for (int l = 1; l <= L; ++l)
+        if (sh.box_hi[l] > sh.box_lo[l]) xlate_fast_launch(Pl, 2, l, st, sh.box_lo[l], sh.box_hi[l]);  // L2L into its boxes
+    if (sizeof(T) == 4) p2p_fast_launch(Pl, st, d_field != nullptr, sh.item0, sh.item1);
+    else p2p_fast64_launch(Pl, st, d_field != nullptr, sh.item0, sh.item1);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    dispatch_p2m_l2p<T>(Pl, true, d_pot, d_field, st, sh.leaf_lo, sh.leaf_hi);
+    FMM_CUDA_CHECK(cudaGetLastError());
+}
+
+const Plan::Shard& shard_info(const Plan& P, int n_shards, int shard, cudaStream_t st) {
+    Plan::Shard& sh = P.shard_cache;
+    if (sh.n_shards == n_shards && sh.shard == shard) return sh;
+    const int L = P.L;
+    sh.box_lo.assign(L + 1, 0); sh.box_hi.assign(L + 1, 0); sh.e0.assign(L + 1, 0); sh.e1.assign(L + 1, 0);
+    for (int l = 0; l <= L; ++l) shard_box_range(L, P.s, n_shards, shard, l, &sh.box_lo[l], &sh.box_hi[l]);
+    sh.leaf_lo = sh.box_lo[L]; sh.leaf_hi = sh.box_hi[L];
+    std::vector<int64_t> h(2 * (L + 1) + 2, 0);
+    for (int l = 0; l <= L; ++l) {
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&h[2 * l], P.weak_off.p + P.level_off[l] + sh.box_lo[l], sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA_CHECK(cudaMemcpyAsync(&h[2 * l + 1], P.weak_off.p + P.level_off[l] + sh.box_hi[l], sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    }
+    FMM_CUDA_CHECK(cudaMemcpyAsync(&h[2 * L + 2], P.p2p_item_off.p + sh.leaf_lo, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaMemcpyAsync(&h[2 * L + 3], P.p2p_item_off.p + sh.leaf_hi, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    for (int l = 0; l <= L; ++l) { sh.e0[l] = h[2 * l]; sh.e1[l] = sh.box_hi[l] > sh.box_lo[l] ? h[2 * l + 1] : h[2 * l]; }
+    sh.item0 = h[2 * L + 2]; sh.item1 = h[2 * L + 3];
+    sh.n_shards = n_shards; sh.shard = shard;
+    return sh;
+}
+
+void check_shardable(const Plan& P, int n_shards, int shard) {
+    if (n_shards < 1 || shard < 0 || shard >= n_shards) { set_error("shard index out of range"); throw CudaFail{FMM_ERR_INVALID_ARG}; }
+    if (P.S) { set_error("sharded evaluate: plans with separate targets are not supported"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+    if (!xlate_fast_available(P.p, P.dtype) || P.m2l_variant != 0) {
+        set_error("sharded evaluate needs the specialised kernels (1 <= p <= 12, m2l_variant 0)");
+        throw CudaFail{FMM_ERR_UNSUPPORTED};
+    }
+}
+
+}  // namespace
+
+// level-local box range [b0, b1) that shard `shard` of `n_shards` touches on `level`: its leaves on level L, their ancestors above
+void shard_box_range(int L, int s, int n_shards, int shard, int level, int64_t* b0, int64_t* b1) {
+    const int64_t n_leaves = (int64_t)1 << (s * L);
+    const int64_t lo = n_leaves * shard / n_shards, hi = n_leaves * (shard + 1) / n_shards;
+    const int sh = s * (L - level);
+    *b0 = lo >> sh;
+    *b1 = hi > lo ? ((hi - 1) >> sh) + 1 : (lo >> sh);
+}
+
+void run_shard_upward(const Plan& P, int n_shards, int shard, const void* d_q, cudaStream_t st) {
+    check_shardable(P, n_shards, shard);
+    ensure_constants(P);
+    int64_t lo, hi;
+    shard_box_range(P.L, P.s, n_shards, shard, P.L, &lo, &hi);
+    if (P.dtype == FMM_F32) shard_upward_t<float>(P, lo, hi, d_q, st);
+    else shard_upward_t<double>(P, lo, hi, d_q, st);
+}
+
+void run_shard_downward(const Plan& P, int n_shards, int shard, void* d_pot, void* d_field, cudaStream_t st) {
+    check_shardable(P, n_shards, shard);
+    ensure_constants(P);
+    const Plan::Shard& sh = shard_info(P, n_shards, shard, st);
+    if (P.dtype == FMM_F32) shard_downward_t<float>(P, sh, d_pot, d_field, st);
+    else shard_downward_t<double>(P, sh, d_pot, d_field, st);
+}
+
+namespace {
 }  // namespace
 
 int64_t evaluate_launches(const Plan& P) {
@@ -895,19 +1008,7 @@ int64_t evaluate_launches(const Plan& P) {
 }
 
 void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
-    {   // __constant__ copies of g_n^m: one upload per device
-        DeviceCtx& ctx = device_ctx(P.device);
-        std::lock_guard<std::mutex> lock(ctx.mu);
-        if (!ctx.const_uploaded) {
-            std::vector<double> g(KMAX);
-            std::vector<float> gf(KMAX);
-            FMM_CUDA_CHECK(cudaMemcpy(g.data(), ctx.tab.d_g, KMAX * sizeof(double), cudaMemcpyDeviceToHost));
-            for (int i = 0; i < KMAX; ++i) gf[i] = (float)g[i];
-            FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_g, g.data(), KMAX * sizeof(double)));
-            FMM_CUDA_CHECK(cudaMemcpyToSymbol(c_gf, gf.data(), KMAX * sizeof(float)));
-            ctx.const_uploaded = true;
-        }
-    }
+    ensure_constants(P);
     if (P.S) {
         if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev, d_dip);
         else run_st<double>(P, d_q, d_pot, d_field, st, ev, d_dip);

@@ -147,6 +147,18 @@ struct Plan {
     // aliases of the hierarchy arrays plus the transposed interaction lists -- built on first use (plan.cu build_adjoint_view).
     // Declared after S: it is destroyed first, while the buffers it aliases are still alive.
     std::unique_ptr<Plan> adj;
+    // Target-sharded evaluate (fmm_evaluate_shard_*): what shard `shard` of `n_shards` owns -- a contiguous range of target leaves,
+    // i.e. a set of subtrees (the tree order is a Z-order), the weak pairs whose target is one of its boxes or one of
+    // their ancestors (per level a contiguous piece of the list, which is sorted by target) and its P2P work items.  Host copy of the
+    // few offsets involved, cached for the shard used last.
+    struct Shard {
+        int n_shards = 0, shard = -1;
+        int64_t leaf_lo = 0, leaf_hi = 0;
+        std::vector<int64_t> box_lo, box_hi;  // per level: level-local box range
+        std::vector<int64_t> e0, e1;          // per level: weak pairs [e0, e1)
+        int64_t item0 = 0, item1 = 0;         // P2P work items
+    };
+    mutable Shard shard_cache;
     bool no_split = false;  // evaluate schedule: never run the leaf-level M2L beside the M2M pass (sources may be coarser than targets)
     std::vector<int> march_steps;  // (l_trg, l_src) pairs visited by the level march (cross_level = 1 or separate targets)
 
@@ -171,6 +183,7 @@ struct Plan {
     DevBuf<float> m2l_geo;   // xlate_fast.cu: per batch of 32 weak pairs a 1 KB geometry record (fp32, p <= 8)
     int64_t m2l_seg_e0[2] = {0, 0}, m2l_seg_rec[2] = {0, 0};  // the two segments of the weak list the records are batched by: first pair, first record
     DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
+    DevBuf<int64_t> p2p_item_off;  // n_leaves + 1: first work item of every target leaf (items are stored in leaf order)
     int64_t n_p2p_items = 0;
     bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
     DevBuf<float> srcg;
@@ -205,14 +218,20 @@ int64_t evaluate_launches(const Plan& P);  // kernels launched by one run_evalua
 // levels, `level` ignored), 2 = L2L from level-1 into `level`.  Results are ADDED (atomically) to the output rows.
 bool xlate_fast_available(int p, fmm_dtype dt);  // false if no register kernel exists for (p, dtype)
 void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]);  // {FMA, MUL, ADD} instructions of one translation (0 if generic only)
-void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0 = 0, int64_t e1 = -1);  // kind 1: weak pairs [e0, e1)
+// kind 1: weak pairs [e0, e1); kinds 0 / 2: children [e0, e1) of `level` (level-local indices; e1 < 0: all)
+void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0 = 0, int64_t e1 = -1);
 // xlate_smem.cu: the same three operators for 9 <= p <= 12, one thread per translation with the state vector in shared memory
 bool xlate_smem_available(int p, fmm_dtype dt);
 void xlate_smem_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1);
 bool m2l_geo_wanted(int p, fmm_dtype dt);        // fp32, p <= 8: the M2L kernel reads per-pair geometry records
 void m2l_geo_prepare(Plan& P, cudaStream_t st);  // plan time, after build_lists: writes Plan::m2l_geo
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic
-void p2p_fast_launch(const Plan& P, cudaStream_t st, bool want_field);  // want_field = false: potential only (cheaper inner loop)
-void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field);  // fp64: same mapping, scalar DFMA arithmetic, sources read through L1
+// want_field = false: potential only (cheaper inner loop); work items [item0, item1) of Plan::p2p_items (item1 < 0: all)
+void p2p_fast_launch(const Plan& P, cudaStream_t st, bool want_field, int64_t item0 = 0, int64_t item1 = -1);
+void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field, int64_t item0 = 0, int64_t item1 = -1);  // fp64: same mapping, scalar DFMA arithmetic
+// evaluate.cu: target-sharded evaluate (see Plan::Shard); both run serially on st
+void shard_box_range(int L, int s, int n_shards, int shard, int level, int64_t* b0, int64_t* b1);
+void run_shard_upward(const Plan& P, int n_shards, int shard, const void* d_q, cudaStream_t st);
+void run_shard_downward(const Plan& P, int n_shards, int shard, void* d_pot, void* d_field, cudaStream_t st);
 
 }  // namespace fmm

@@ -362,19 +362,20 @@ __global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restric
 }  // namespace
 
 template <int TPT, int HS>
-static void p2p_launch_t(const Plan& P, cudaStream_t st, bool wf) {
+static void p2p_launch_t(const Plan& P, cudaStream_t st, bool wf, int64_t item0, int64_t item1) {
     const int64_t leaf0 = P.level_off[P.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
-    const int64_t n_items = P.n_p2p_items * nchunk;
+    if (item1 < 0) { item0 = 0; item1 = P.n_p2p_items; }
+    const int64_t n_items = (item1 - item0) * nchunk;
     // separate targets: a target leaf may have an empty strong list and then no work item; its near field must read zero
     if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources (separate targets)
     if (wf) p2p_fast_k<TPT, HS, true, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
     else p2p_fast_k<TPT, HS, false, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
 }
 
 // Targets per lane.  A median-split tree gives every leaf the same population (+-1), so max_leaf decides the lane layout for
@@ -395,44 +396,45 @@ static int choose_tpt(int max_leaf) {
     return best;
 }
 
-void p2p_fast_launch(const Plan& P, cudaStream_t st, bool wf) {
+void p2p_fast_launch(const Plan& P, cudaStream_t st, bool wf, int64_t i0, int64_t i1) {
     switch (choose_tpt(P.max_leaf)) {
-        case 1: p2p_launch_t<1, 2>(P, st, wf); break;
-        case 2: p2p_launch_t<2, 2>(P, st, wf); break;
-        case 3: p2p_launch_t<3, 2>(P, st, wf); break;
-        case 4: p2p_launch_t<4, 2>(P, st, wf); break;
-        case 5: p2p_launch_t<5, 1>(P, st, wf); break;
-        case 6: p2p_launch_t<6, 1>(P, st, wf); break;
-        case 7: p2p_launch_t<7, 1>(P, st, wf); break;
-        default: p2p_launch_t<8, 1>(P, st, wf); break;
+        case 1: p2p_launch_t<1, 2>(P, st, wf, i0, i1); break;
+        case 2: p2p_launch_t<2, 2>(P, st, wf, i0, i1); break;
+        case 3: p2p_launch_t<3, 2>(P, st, wf, i0, i1); break;
+        case 4: p2p_launch_t<4, 2>(P, st, wf, i0, i1); break;
+        case 5: p2p_launch_t<5, 1>(P, st, wf, i0, i1); break;
+        case 6: p2p_launch_t<6, 1>(P, st, wf, i0, i1); break;
+        case 7: p2p_launch_t<7, 1>(P, st, wf, i0, i1); break;
+        default: p2p_launch_t<8, 1>(P, st, wf, i0, i1); break;
     }
 }
 
 template <int TPT>
-static void p2p_launch64_t(const Plan& P, cudaStream_t st, bool wf) {
+static void p2p_launch64_t(const Plan& P, cudaStream_t st, bool wf, int64_t item0, int64_t item1) {
     const Plan& PS = P.S ? *P.S : P;
     const int64_t sleaf0 = PS.level_off[PS.L];
     const int nchunk = (P.max_leaf + 32 * TPT - 1) / (32 * TPT);
-    const int64_t n_items = P.n_p2p_items * nchunk;
+    if (item1 < 0) { item0 = 0; item1 = P.n_p2p_items; }
+    const int64_t n_items = (item1 - item0) * nchunk;
     if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
     const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     if (wf) p2p_warp64_k<TPT, true><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
-                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
     else p2p_warp64_k<TPT, false><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
-                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p), P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
 }
 
-void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool wf) {
+void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool wf, int64_t i0, int64_t i1) {
     switch (choose_tpt(P.max_leaf)) {
-        case 1: p2p_launch64_t<1>(P, st, wf); break;
-        case 2: p2p_launch64_t<2>(P, st, wf); break;
-        case 3: p2p_launch64_t<3>(P, st, wf); break;
-        case 4: p2p_launch64_t<4>(P, st, wf); break;
-        case 5: p2p_launch64_t<5>(P, st, wf); break;
-        case 6: p2p_launch64_t<6>(P, st, wf); break;
-        case 7: p2p_launch64_t<7>(P, st, wf); break;
-        default: p2p_launch64_t<8>(P, st, wf); break;
+        case 1: p2p_launch64_t<1>(P, st, wf, i0, i1); break;
+        case 2: p2p_launch64_t<2>(P, st, wf, i0, i1); break;
+        case 3: p2p_launch64_t<3>(P, st, wf, i0, i1); break;
+        case 4: p2p_launch64_t<4>(P, st, wf, i0, i1); break;
+        case 5: p2p_launch64_t<5>(P, st, wf, i0, i1); break;
+        case 6: p2p_launch64_t<6>(P, st, wf, i0, i1); break;
+        case 7: p2p_launch64_t<7>(P, st, wf, i0, i1); break;
+        default: p2p_launch64_t<8>(P, st, wf, i0, i1); break;
     }
 }
 

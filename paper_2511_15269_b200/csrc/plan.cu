@@ -691,6 +691,8 @@ static void finish_lists(Plan& P, cudaStream_t st) {
         FMM_CUDA_CHECK(cudaStreamSynchronize(st));
         P.n_p2p_items = n_items;
         P.p2p_multi = multi != 0;
+        P.p2p_item_off.alloc(P.n_leaves + 1);
+        FMM_CUDA_CHECK(cudaMemcpyAsync(P.p2p_item_off.p, seg_off.p, (P.n_leaves + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
         P.p2p_items.alloc((size_t)n_items * sizeof(P2PItem));
         if (n_items > 0) {
             p2p_segments_k<<<nblocks(P.n_leaves, 128), 128, 0, st>>>(P.strong_off.p, P.strong_src.p, P.box_start.p + P.level_off[L], lcnt, scnt, P.n_leaves, budget, nseg.p, seg_off.p,

@@ -46,6 +46,7 @@ struct Geo {
 
 struct XArgs {
     int device;                   // host side only: the plan's device (per-device kernel attributes)
+    int64_t first;                // KIND 0 / 2: first child (level-local index) of this launch
     int64_t n;                    // number of translations
     const int32_t *tgt, *src;     // KIND 1: global ids per pair
     int64_t off_parent, off_child;
@@ -79,12 +80,15 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
         const float* r = a.geo + (e >> 5) * 256 + lane;
 #pragma unroll
         for (int w = 0; w < 7; ++w) rec[w] = r[32 * w];
-        gt = reinterpret_cast<const int*>(r)[224];
-        if (e < a.n) gs = a.src[e];
+        if (e < a.n) {  // a launch may cover only a prefix of the segment (sharded evaluate): pairs beyond it are not this launch's
+            gt = reinterpret_cast<const int*>(r)[224];
+            gs = a.src[e];
+        }
     } else if (e < a.n) {
         if constexpr (KIND == 1) { gs = a.src[e]; gt = a.tgt[e]; }
         else {
-            const int64_t gc = a.off_child + e, gp = a.off_parent + (e >> a.s);
+            const int64_t c = a.first + e;
+            const int64_t gc = a.off_child + c, gp = a.off_parent + (c >> a.s);
             if (a.box_count[gc] > 0) {
                 if constexpr (KIND == 0) { gs = (int)gc; gt = (int)gp; }
                 else { gs = (int)gp; gt = (int)gc; }
@@ -305,7 +309,9 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
             }
         }
     } else {
-        a.n = (int64_t)1 << (P.s * level);  // children on `level`
+        const int64_t nch = (int64_t)1 << (P.s * level);  // children on `level`
+        a.first = e1 < 0 ? 0 : e0;
+        a.n = e1 < 0 ? nch : e1 - e0;
         a.off_parent = P.level_off[level - 1];
         a.off_child = P.level_off[level];
         a.in = kind == 0 ? P.Mc.p : P.Lc.p;

@@ -23,6 +23,7 @@ using namespace xr;
 
 struct SArgs {
     int device;                   // host side only: the plan's device (per-device kernel attributes)
+    int64_t first;                // KIND 0 / 2: first child (level-local index) of this launch
     int64_t n;                    // number of translations
     const int32_t *tgt, *src;     // KIND 1: global ids per pair
     int64_t off_parent, off_child;
@@ -170,7 +171,8 @@ __global__ void __launch_bounds__(NT) xlate_smem_k(SArgs a) {
     if (e < a.n) {
         if constexpr (KIND == 1) { gs = a.src[e]; gt = a.tgt[e]; }
         else {
-            const int64_t gc = a.off_child + e, gp = a.off_parent + (e >> a.s);
+            const int64_t c = a.first + e;
+            const int64_t gc = a.off_child + c, gp = a.off_parent + (c >> a.s);
             if (a.box_count[gc] > 0) {
                 if constexpr (KIND == 0) { gs = (int)gc; gt = (int)gp; }
                 else { gs = (int)gp; gt = (int)gc; }
@@ -267,7 +269,8 @@ bool smem_launch_t(const Plan& P, int kind, int level, cudaStream_t st, int64_t 
         a.out = P.Lc.p;
         if (P.S) { a.ctr_s = P.S->box_ctr.p; a.scale_s = P.S->box_scale.p; a.in = P.S->Mc.p; }
     } else {
-        a.n = (int64_t)1 << (P.s * level);  // children on `level`
+        a.first = e1 < 0 ? 0 : e0;
+        a.n = e1 < 0 ? ((int64_t)1 << (P.s * level)) : e1 - e0;  // children on `level`
         a.off_parent = P.level_off[level - 1];
         a.off_child = P.level_off[level];
         a.in = kind == 0 ? P.Mc.p : P.Lc.p;

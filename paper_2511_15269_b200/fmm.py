@@ -18,7 +18,8 @@ FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
-           "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
+           "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_shard_box_range", "fmm_evaluate_shard_upward",
+           "fmm_evaluate_shard_downward", "fmm_plan_leaf_multipoles", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
 
 class fmm_admissibility(C.Structure):
@@ -53,6 +54,10 @@ def lib():
         L.fmm_plan_copy_lists.argtypes = [vp, i64p, i32p, i64p, i32p]
         L.fmm_plan_create_targets.argtypes = [vp, C.c_int64, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
         L.fmm_plan_update.argtypes = [vp, vp, vp, vp]
+        L.fmm_shard_box_range.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, i64p, i64p]
+        L.fmm_evaluate_shard_upward.argtypes = [vp, C.c_int, C.c_int, vp, vp]
+        L.fmm_evaluate_shard_downward.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp]
+        L.fmm_plan_leaf_multipoles.argtypes = [vp, C.c_int, C.c_int64, C.c_int64, vp, i64p, vp]
         L.fmm_plan_source_info.argtypes = [vp, i64p, C.POINTER(C.c_int), i64p, i64p]
         L.fmm_plan_copy_source_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
         L.fmm_plan_copy_march.argtypes = [vp, i32p, i32p]
@@ -174,6 +179,54 @@ def fmm_plan_update(plan, positions=None, targets=None, stream=None):
             raise ValueError("new positions must be contiguous CUDA tensors of shape (%d, 3) and dtype %s on %s" % (n, tdtype, device))
     p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
     _check(lib().fmm_plan_update(plan, p(positions), p(targets), _stream_ptr(stream)))
+
+
+def fmm_shard_box_range(L, s, n_shards, shard, level):
+    """level-local [begin, end) of the boxes of `level` that shard `shard` of `n_shards` touches (no device needed)"""
+    a, b = C.c_int64(), C.c_int64()
+    _check(lib().fmm_shard_box_range(int(L), int(s), int(n_shards), int(shard), int(level), C.byref(a), C.byref(b)))
+    return a.value, b.value
+
+
+def fmm_evaluate_shard_upward(plan, n_shards, shard, charges, stream=None):
+    _check_io(plan, charges, None, None)
+    _check(lib().fmm_evaluate_shard_upward(plan, int(n_shards), int(shard), C.c_void_p(charges.data_ptr()), _stream_ptr(stream)))
+
+
+def fmm_evaluate_shard_downward(plan, n_shards, shard, potential=None, field=None, stream=None):
+    _check_io(plan, None, potential, field)
+    p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().fmm_evaluate_shard_downward(plan, int(n_shards), int(shard), p(potential), p(field), _stream_ptr(stream)))
+
+
+def fmm_plan_leaf_multipoles(plan, copy_in, leaf_begin, leaf_end, rows=None, stream=None):
+    """copies leaf rows of the multipole array out of (copy_in = 0) or into (1) the plan; returns the row length in elements"""
+    n = C.c_int64()
+    _check(lib().fmm_plan_leaf_multipoles(plan, int(copy_in), int(leaf_begin), int(leaf_end), C.c_void_p(rows.data_ptr()) if rows is not None else None,
+                                          C.byref(n), _stream_ptr(stream)))
+    return n.value
+
+
+def evaluate_sharded(plan, n_leaves, charges, potential=None, field=None, group=None):
+    """One evaluate with the targets sharded over the ranks of a torch.distributed process group (one process per GPU; every rank
+    holds the same plan and all charges): upward pass for the own leaves, ONE all-gather of the leaf multipoles (NCCL over NVLink
+    on GPUs), downward pass for the own targets.  Writes the potential / field of the own particles only."""
+    import torch
+    import torch.distributed as dist
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    fmm_evaluate_shard_upward(plan, world, rank, charges)
+    if world > 1:
+        kp = fmm_plan_leaf_multipoles(plan, 0, 0, 0)
+        bounds = [n_leaves * r // world for r in range(world + 1)]
+        rows = max(b - a for a, b in zip(bounds, bounds[1:]))
+        mine = torch.zeros((rows, kp), dtype=charges.dtype, device=charges.device)
+        fmm_plan_leaf_multipoles(plan, 0, bounds[rank], bounds[rank + 1], mine)
+        allrows = torch.empty((world, rows, kp), dtype=charges.dtype, device=charges.device)
+        dist.all_gather_into_tensor(allrows, mine, group=group)
+        for r in range(world):
+            if r != rank and bounds[r + 1] > bounds[r]:
+                fmm_plan_leaf_multipoles(plan, 1, bounds[r], bounds[r + 1], allrows[r])
+    fmm_evaluate_shard_downward(plan, world, rank, potential, field)
 
 
 def fmm_plan_source_info(plan):
