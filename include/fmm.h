@@ -202,6 +202,14 @@ fmm_status fmm_plan_timings(const fmm_plan* plan, double* h_ms);
  * both dtypes; a second, independent implementation of App. B that the tests cross-check against the oracle). */
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant);
 
+/* Reproducibility.  By default the translation kernels add the partial sums of a row of the coefficient arrays with floating-point
+ * atomics and a leaf with a very long strong list is summed in several pieces, so two evaluates of the same input agree to rounding
+ * (1e-13 relative in fp64), not bit for bit.  on = 1: every sum has ONE contributor that adds in list order -- the M2L runs with one
+ * warp per target box (p <= 8) or in the generic warp-per-box kernel (p >= 9), the P2P with one work item per leaf, and the kernels
+ * run in the serial schedule: two evaluates of the same charges on the same plan return identical bits.  Costs about 16 % at
+ * N = 1M, p = 8, fp32 (1.28 -> 1.49 ms per evaluate on B200).  Requires s <= 5.  Synchronises the device (the P2P work items are rebuilt). */
+fmm_status fmm_plan_set_deterministic(fmm_plan* plan, int on, void* cuda_stream);
+
 /* Schedule of subsequent fmm_evaluate / fmm_evaluate_host calls on this plan.  0 (default) = concurrent: the call forks
  * three internal streams from cuda_stream and joins them back before it returns control of the stream -- the near field
  * (P2P) runs beside the whole far-field chain and the M2M pass beside the leaf-level M2L; for the caller the call is

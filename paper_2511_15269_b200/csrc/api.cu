@@ -512,6 +512,25 @@ fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial) {
     return FMM_OK;
 }
 
+fmm_status fmm_plan_set_deterministic(fmm_plan* plan, int on, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || on < 0 || on > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+        Plan& P = plan->P;
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
+        if (P.s > 5) { set_error("deterministic mode needs s <= 5 (the children of a box must fit one warp)"); return FMM_ERR_UNSUPPORTED; }
+        if (P.deterministic == (on != 0)) return FMM_OK;
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
+        FMM_CUDA_CHECK(cudaDeviceSynchronize());
+        P.deterministic = on != 0;
+        // one P2P work item per leaf (no partial sums combined with atomics) / the load-balanced segments again
+        if (P.n_leaves > 0 && P.strong_off.p) build_p2p_items(P, st, P.deterministic);
+        P.shard_cache = Plan::Shard();
+        P.adj.reset();
+        return FMM_OK;
+    });
+}
+
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {
     if (!plan || variant < 0 || variant > 1) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
     plan->P.m2l_variant = variant;

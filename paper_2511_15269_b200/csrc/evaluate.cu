@@ -704,7 +704,7 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     const Tables& tb = tables(Pl.device);
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
     const int p = Pl.p, s = Pl.s;
-    const bool serial = ev != nullptr || Pl.serial;
+    const bool serial = ev != nullptr || Pl.serial || Pl.deterministic;
     cudaStream_t sF = st, sN = st;
     if (!serial) {
         ensure_streams(Pl);
@@ -762,7 +762,9 @@ void run_st(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStr
     }
     mark(3);
     if (Pl.n_weak > 0) {
-        if (fast) xlate_fast_launch(Pl, 1, 0, sF, 0, Pl.n_weak);
+        // deterministic: one warp per target row (p <= 8) or the generic warp-per-box kernel -- both sum a row in list order
+        if (fast && Pl.deterministic && m2l_row_available(p, Pl.dtype)) m2l_row_launch(Pl, sF);
+        else if (fast && !Pl.deterministic) xlate_fast_launch(Pl, 1, 0, sF, 0, Pl.n_weak);
         else
             m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(
                 p, Pl.n_boxes, Pl.weak_off.p, Pl.weak_src.p, Pl.box_ctr.p, (const T*)Pl.box_scale.p, S.box_ctr.p, (const T*)S.box_scale.p, Pl.Kp,
@@ -798,7 +800,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     TabPtrs tp{sizeof(T) == 4 ? (const void*)tb.d_Bf : (const void*)tb.d_B, tb.d_H, tb.d_A};
     const int p = Pl.p, s = Pl.s, L = Pl.L;
     const int64_t N = Pl.N;
-    const bool serial = ev != nullptr || Pl.serial;
+    const bool serial = ev != nullptr || Pl.serial || Pl.deterministic;
     cudaStream_t sF = st, sU = st, sN = st;
     if (!serial) {
         ensure_streams(Pl);
@@ -870,7 +872,9 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
         if (split) {
             m2l_range(w_leaf, Pl.n_weak, sF);
             m2l_range(0, w_leaf, sU);
-        } else if (fast) {
+        } else if (fast && Pl.deterministic && m2l_row_available(p, Pl.dtype)) {
+            m2l_row_launch(Pl, sF);  // one warp per target row, sums in list order (see run_st)
+        } else if (fast && !Pl.deterministic) {
             m2l_range(0, Pl.n_weak, sF);
         } else {
             m2l_generic_k<T><<<nblocks(Pl.n_boxes, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sF>>>(

@@ -185,6 +185,7 @@ struct Plan {
     DevBuf<char> p2p_items;  // n_p2p_items x P2PItem
     DevBuf<int64_t> p2p_item_off;  // n_leaves + 1: first work item of every target leaf (items are stored in leaf order)
     int64_t n_p2p_items = 0;
+    int64_t p2p_src_total = 0;  // sum over the non-empty target leaves of the source particles in their strong lists
     bool p2p_multi = false;  // some leaf has more than one item: `near` is zeroed before P2P and those leaves use atomics
     DevBuf<float> srcg;
     DevBuf<int32_t> src_slot;
@@ -194,6 +195,7 @@ struct Plan {
     mutable cudaStream_t s_far = nullptr, s_up = nullptr, s_near = nullptr;
     mutable cudaEvent_t e_fork = nullptr, e_perm = nullptr, e_p2m = nullptr, e_up = nullptr, e_near = nullptr, e_done = nullptr;
     bool serial = false;  // true: every kernel on the caller's stream (fmm_plan_set_schedule)
+    bool deterministic = false;  // fmm_plan_set_deterministic: serial schedule, no floating-point atomics with more than one contributor
     ~Plan() {
         for (cudaStream_t q : {s_far, s_up, s_near})
             if (q) cudaStreamDestroy(q);
@@ -208,6 +210,7 @@ struct Plan {
 // plan.cu
 void build_tree(Plan& P, const void* d_positions, cudaStream_t st);
 void build_lists(Plan& P, cudaStream_t st);
+void build_p2p_items(Plan& P, cudaStream_t st, bool single_segment);  // (re)builds Plan::p2p_items; synchronises the stream
 void build_adjoint_view(Plan& P, cudaStream_t st);  // fills P.adj (transposed lists; synchronises the stream)
 // evaluate.cu
 // d_q: charges (may be null = zero charges), d_dip: optional dipole moments (N_sources x 3, input order): the sources then also
@@ -223,6 +226,8 @@ void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int6
 // xlate_smem.cu: the same three operators for 9 <= p <= 12, one thread per translation with the state vector in shared memory
 bool xlate_smem_available(int p, fmm_dtype dt);
 void xlate_smem_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1);
+bool m2l_row_available(int p, fmm_dtype dt);     // deterministic M2L, one warp per target box (p <= 8)
+void m2l_row_launch(const Plan& P, cudaStream_t st);
 bool m2l_geo_wanted(int p, fmm_dtype dt);        // fp32, p <= 8: the M2L kernel reads per-pair geometry records
 void m2l_geo_prepare(Plan& P, cudaStream_t st);  // plan time, after build_lists: writes Plan::m2l_geo
 // p2p_fast.cu: fp32 near field + finalize, one target leaf per warp, packed f32x2 arithmetic

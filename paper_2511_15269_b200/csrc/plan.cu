@@ -661,18 +661,30 @@ static void finish_lists(Plan& P, cudaStream_t st) {
     FMM_CUDA_CHECK(cudaMemcpyAsync(h, cnt.p, 16, cudaMemcpyDeviceToHost, st));
     FMM_CUDA_CHECK(cudaStreamSynchronize(st));
     P.n_p2p_pairs = (int64_t)h[0];
+    P.p2p_src_total = (int64_t)h[1];
+    build_p2p_items(P, st, P.deterministic);
+}
+
+// Work items of the P2P kernels: the strong list of a target leaf cut into segments (p2p_segments_k).  single_segment: one item per
+// leaf whatever its length -- no partial sums to combine with atomics (fmm_plan_set_deterministic).
+void build_p2p_items(Plan& P, cudaStream_t st, bool single_segment) {
+    const int L = P.L;
+    const Plan& PS = P.S ? *P.S : P;
+    const int32_t* scnt = PS.box_count.p + PS.level_off[PS.L];
+    const unsigned long long h1 = (unsigned long long)P.p2p_src_total;
     {
         // work items of the P2P kernel: budget = twice the mean number of source particles per target leaf (at least 1024)
         const int32_t* lcnt = P.box_count.p + P.level_off[L];
-        const int64_t mean_src = (int64_t)(h[1] / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
+        const int64_t mean_src = (int64_t)(h1 / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
         int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
         // small problems: fewer target leaves than the chip has warp slots -- cut the lists finer (down to 128 source particles
         // per item) so that about 8 warps per SM find work; the partial sums of a leaf are then combined with atomics
         const int64_t want_items = 148 * 8;
         if (P.n_leaves < want_items) {
-            const int64_t fine = (int64_t)(h[1] / (unsigned long long)want_items);
+            const int64_t fine = (int64_t)(h1 / (unsigned long long)want_items);
             budget = std::min(budget, std::max<int64_t>(128, fine));
         }
+        if (single_segment) budget = INT64_MAX / 4;
         DevBuf<int32_t> nseg, any_multi;
         DevBuf<int64_t> seg_off, scratch;
         nseg.alloc(P.n_leaves);

@@ -58,6 +58,7 @@ struct XArgs {
     const void* scale_s;          //     a source hierarchy to a separate target hierarchy)
     const void* in;
     void* out;
+    const int64_t* woff;          // m2l_row_k: CSR offsets of the weak list by target box
     const float* geo;             // KIND 1, GEO kernels: geometry records of the pairs (m2l_geo_prepare), 1 KB per batch of 32
 };
 
@@ -193,6 +194,120 @@ void launch(const XArgs& a, cudaStream_t st) {
     xlate_fast_k<T, P, KIND, XW, GEO><<<grid, XW * 32, smem, st>>>(a);
 }
 
+
+// Deterministic M2L (fmm_plan_set_deterministic): ONE WARP PER TARGET BOX walks the box's row of the weak list (CSR by target) in
+// batches of 32 pairs and keeps the sums of the translated rows in registers, batch after batch and row after row in list order;
+// the single contributor of a row of the local array adds its total at the end.  No floating-point atomics whose order could vary,
+// at the price of idle lanes in the last batch of every row (~9 % at config 2) and of the plan-time geometry records (their batches
+// are cut differently).
+template <typename T, int P, int XW>
+__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : 4) m2l_row_k(XArgs a) {
+    using G = Geo<T, P>;
+    using V = typename Vec16<T>::type;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    V* sm = reinterpret_cast<V*>(smraw) + (size_t)warp * 32 * G::KSB;
+    const int64_t ti = (int64_t)blockIdx.x * XW + warp;
+    if (ti >= a.n) return;
+    const int gt = (int)(a.first + ti);
+    const int64_t e0 = a.woff[gt], e1 = a.woff[gt + 1];
+    if (e0 == e1) return;
+    constexpr uint32_t ROWB = G::CH * 16;
+    const uint32_t bar = smem_u32(reinterpret_cast<unsigned long long*>(smraw + (size_t)XW * 32 * G::KSB * 16) + warp);
+    if (lane == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    const T* sc = reinterpret_cast<const T*>(a.scale);
+    const T* scs = reinterpret_cast<const T*>(a.scale_s);
+    const double tx = a.ctr[3 * (int64_t)gt], ty = a.ctr[3 * (int64_t)gt + 1], tz = a.ctr[3 * (int64_t)gt + 2];
+    const T a_new = sc[gt];
+    const T* smT = reinterpret_cast<const T*>(sm);
+    constexpr int RS = G::KSB * G::E;
+    T acc[G::NJ];
+#pragma unroll
+    for (int j = 0; j < G::NJ; ++j) acc[j] = T(0);
+    uint32_t phase = 0;
+#pragma unroll 1
+    for (int64_t eb = e0; eb < e1; eb += 32) {
+        const int64_t e = eb + lane;
+        const int gs = e < e1 ? a.src[e] : -1;
+        const unsigned vmask = __ballot_sync(0xffffffffu, gs >= 0);
+        {
+            const int gprev = __shfl_up_sync(0xffffffffu, gs, 1);
+            const bool head = lane == 0 || gs < 0 || gprev < 0 || gs != gprev + 1 || G::KSB != G::CH;
+            const unsigned hm = __ballot_sync(0xffffffffu, head);
+            const unsigned above = lane == 31 ? 0u : (hm >> (lane + 1));
+            const int len = above ? __ffs(above) : 32 - lane;
+            if (head && gs >= 0)
+                bulk_g2s(smem_u32(sm + lane * G::KSB), reinterpret_cast<const char*>(a.in) + (int64_t)gs * ROWB, (uint32_t)len * ROWB, bar);
+        }
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)__popc(vmask) * ROWB);
+        T bx = T(0), by = T(0), bz = T(1), a_old = T(1);
+        if (gs >= 0) {
+            bx = (T)(a.ctr_s[3 * (int64_t)gs] - tx);
+            by = (T)(a.ctr_s[3 * (int64_t)gs + 1] - ty);
+            bz = (T)(a.ctr_s[3 * (int64_t)gs + 2] - tz);
+            a_old = scs[gs];
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1u;
+        V* row = sm + lane * G::KSB;
+        if (gs >= 0) {
+            T v[G::KV];
+            sfor<G::CH>([&](auto cc) {
+                constexpr int c = decltype(cc)::value;
+                const V x = row[c];
+                if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
+                else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
+            });
+            translate_qz<T, P, 1, qz_mode<T>()>(v, bx, by, bz, a_old, a_new);
+            sfor<G::CH>([&](auto cc) {
+                constexpr int c = decltype(cc)::value;
+                V x;
+                if constexpr (G::E == 4) { x.x = v[4 * c]; x.y = v[4 * c + 1]; x.z = v[4 * c + 2]; x.w = v[4 * c + 3]; }
+                else { x.x = v[2 * c]; x.y = v[2 * c + 1]; }
+                row[c] = x;
+            });
+        }
+        __syncwarp();
+        const int nv = (int)min((int64_t)32, e1 - eb);
+#pragma unroll 4
+        for (int r = 0; r < nv; ++r) {
+#pragma unroll
+            for (int j = 0; j < G::NJ; ++j)
+                if (lane + 32 * j < G::K) acc[j] += smT[r * RS + lane + 32 * j];
+        }
+        __syncwarp();  // every lane has read the rows before the next batch's bulk copies overwrite them
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    T* out = reinterpret_cast<T*>(a.out) + (int64_t)gt * G::Kp;
+#pragma unroll
+    for (int j = 0; j < G::NJ; ++j)
+        if (lane + 32 * j < G::K) out[lane + 32 * j] += acc[j];
+}
+
+template <typename T, int P>
+void launch_row(const XArgs& a, cudaStream_t st) {
+    using G = Geo<T, P>;
+    constexpr int XW = 4;
+    constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;
+    static AttrOnce once;
+    once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(m2l_row_k<T, P, XW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
+    m2l_row_k<T, P, XW><<<(unsigned)((a.n + XW - 1) / XW), XW * 32, smem, st>>>(a);
+}
+
+template <typename T>
+bool dispatch_row(int p, const XArgs& a, cudaStream_t st) {
+    switch (p) {
+#define FMM_CASE(PP) case PP: launch_row<T, PP>(a, st); return true;
+        FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
+#undef FMM_CASE
+        default: return false;
+    }
+}
+
 template <typename T, int KIND>
 bool dispatch(int p, const XArgs& a, cudaStream_t st) {
     switch (p) {
@@ -280,6 +395,25 @@ void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]) {
 
 // p <= 8: state vector in registers (this file); 9 <= p <= 12: state vector in shared memory (xlate_smem.cu)
 bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && ((p >= 1 && p <= 8) || xlate_smem_available(p, dt)); }
+
+// deterministic M2L over all target boxes (p <= 8): see m2l_row_k
+bool m2l_row_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && p >= 1 && p <= 8; }
+void m2l_row_launch(const Plan& P, cudaStream_t st) {
+    XArgs a{};
+    a.device = P.device;
+    a.first = 0;
+    a.n = P.n_boxes;
+    a.woff = P.weak_off.p;
+    a.src = P.weak_src.p;
+    a.ctr = a.ctr_s = P.box_ctr.p;
+    a.scale = a.scale_s = P.box_scale.p;
+    a.in = P.Mc.p;
+    a.out = P.Lc.p;
+    if (P.S) { a.ctr_s = P.S->box_ctr.p; a.scale_s = P.S->box_scale.p; a.in = P.S->Mc.p; }
+    if (P.n_weak <= 0) return;
+    const bool ok = P.dtype == FMM_F64 ? dispatch_row<double>(P.p, a, st) : dispatch_row<float>(P.p, a, st);
+    if (!ok) { set_error("no deterministic register M2L kernel for this order"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+}
 
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
     if (P.p > 8) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }

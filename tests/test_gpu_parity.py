@@ -240,6 +240,30 @@ def test_plan_reuse_and_linearity():
     P.close()
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("gen,N,N_max,s,p,cross", [("cube", 20000, 32, 3, 8, 0), ("cube", 6000, 16, 2, 6, 1), ("clusters", 30000, 48, 1, 5, 0),
+                                                    ("cube", 3000, 20, 2, 10, 0), ("cube", 1500, 512, 3, 4, 0)])
+def test_deterministic_mode_is_bit_for_bit_reproducible(dtype, gen, N, N_max, s, p, cross):
+    """fmm_plan_set_deterministic: two evaluates of the same charges return identical bits (no float atomics with several contributors,
+    serial schedule), the result still meets the parity tolerance, and switching the mode off again restores the default kernels."""
+    pos, q = (inputs.uniform_cube if gen == "cube" else inputs.gaussian_clusters)(N, 41, dtype)
+    P = gpu_plan(pos, p, N_max, s, 0.77, cross_level=cross)
+    Po = O.Plan(pos, p, N_max, s, 0.77, cross_level=cross)
+    uo, fo = Po.evaluate(q, fp32_rule=dtype == np.float32)
+    fmm.fmm_plan_set_deterministic(P.handle, 1)
+    runs = [gpu_eval(P, q) for _ in range(4)]
+    for u, f in runs[1:]:
+        assert np.array_equal(u, runs[0][0]) and np.array_equal(f, runs[0][1])
+    assert rel2(runs[0][0], uo) <= TOL[dtype] and rel2(runs[0][1], fo) <= TOL[dtype]
+    u2, f2 = gpu_eval(P, -q)  # another charge vector in between must not leave anything behind
+    u3, f3 = gpu_eval(P, q)
+    assert np.array_equal(u3, runs[0][0]) and np.array_equal(f3, runs[0][1]) and np.array_equal(u2, -runs[0][0])
+    fmm.fmm_plan_set_deterministic(P.handle, 0)
+    u, f = gpu_eval(P, q)
+    assert rel2(u, uo) <= TOL[dtype] and rel2(f, fo) <= TOL[dtype]
+    P.close()
+
+
 @pytest.mark.parametrize("N,N_max,s,p", [(4096, 64, 3, 8), (3001, 8, 3, 8), (5000, 40, 1, 5), (2000, 16, 2, 1)])
 def test_kernel_families_agree_with_the_oracle_fp32(N, N_max, s, p):
     """fmm_plan_set_m2l_variant: the one-translation-per-thread kernels (0) and the generic warp-per-box kernels (1) are two
