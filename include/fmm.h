@@ -218,8 +218,20 @@ fmm_status fmm_plan_set_deterministic(fmm_plan* plan, int on, void* cuda_stream)
  * order of the floating-point atomics. */
 fmm_status fmm_plan_set_schedule(fmm_plan* plan, int serial);
 
+/* CUDA graphs.  on = 1: the second fmm_evaluate / fmm_evaluate_adjoint / fmm_evaluate_host call that sees the same
+ * device pointers (charges, potential, field) captures the launches of one evaluate -- kernels, memsets and the fork / join
+ * edges of the concurrent schedule -- into a CUDA graph on a stream the plan owns; every later call with those pointers is one
+ * cudaGraphLaunch on cuda_stream (the plan keeps the graphs of the last four pointer sets).  Same kernels, same data, same
+ * results; what changes is the host cost of an evaluate (about 10 + 2 L launches -> 1), which bounds the evaluate time below
+ * N ~ 1e5.  A call made while cuda_stream is itself being captured by the caller launches plainly, so the evaluate can be part
+ * of a caller's graph.  As before, two evaluates of ONE plan must not overlap: order them on one stream or with events.
+ * on = 0: always launch plainly.  on = 2 (default): as 1 for plans with fewer than 2^19 points (sources + targets), as 0 above
+ * -- there the device time hides the launches and the replay measured 2-3 % slower than the stream schedule (N = 1M, B200).
+ * A failed capture disables the graphs of the plan and falls back to plain launches. */
+fmm_status fmm_plan_set_graph(fmm_plan* plan, int on);
+
 /* Number of kernels of this library that one fmm_evaluate call on this plan launches (HOST out): permute, P2M, one M2M
- * and one L2L per level, M2L (when the weak list is not empty; two launches -- leaf level and upper levels -- in the
+ * and one L2L per level below the coarsest level that holds a weak pair (levels above it carry no far field), M2L (when the weak list is not empty; two launches -- leaf level and upper levels -- in the
  * concurrent schedule with the register kernels), P2P, L2P (which also finalizes).  cudaMemset nodes are not counted. */
 fmm_status fmm_plan_launches(const fmm_plan* plan, int64_t* h_launches_per_evaluate);
 

@@ -259,6 +259,7 @@ fmm_status fmm_plan_update(fmm_plan* plan, const void* d_positions, const void* 
         FMM_CUDA_CHECK(cudaEventRecord(e0, st));
         P.adj.reset();  // the transposed lists belong to the old positions
         P.shard_cache = Plan::Shard();
+        ++P.epoch;      // captured evaluate graphs point into arrays that are reallocated below
         double sort_ms = 0, tree_ms = 0;
         if (P.S) {
             if (d_positions) { build_tree(*P.S, d_positions, st); sort_ms += P.S->plan_ms[0]; tree_ms += P.S->plan_ms[1]; }
@@ -347,7 +348,7 @@ fmm_status fmm_evaluate_adjoint(fmm_plan* plan, const void* d_cotangent_potentia
         const bool self_adjoint = !P.S && !P.cross_level;
         if (!self_adjoint) build_adjoint_view(P, st);
         const Plan& V = self_adjoint ? P : *P.adj;
-        if (!self_adjoint) { P.adj->m2l_variant = P.m2l_variant; P.adj->serial = P.serial; }
+        if (!self_adjoint) { P.adj->m2l_variant = P.m2l_variant; P.adj->serial = P.serial; P.adj->use_graph = P.use_graph; }
         run_evaluate(V, d_cotangent_potential, d_charge_grad, nullptr, st, nullptr, d_cotangent_field);
         return FMM_OK;
     });
@@ -523,12 +524,20 @@ fmm_status fmm_plan_set_deterministic(fmm_plan* plan, int on, void* cuda_stream)
         AllocScope scope(st);
         FMM_CUDA_CHECK(cudaDeviceSynchronize());
         P.deterministic = on != 0;
+        ++P.epoch;
         // one P2P work item per leaf (no partial sums combined with atomics) / the load-balanced segments again
         if (P.n_leaves > 0 && P.strong_off.p) build_p2p_items(P, st, P.deterministic);
         P.shard_cache = Plan::Shard();
         P.adj.reset();
         return FMM_OK;
     });
+}
+
+fmm_status fmm_plan_set_graph(fmm_plan* plan, int on) {
+    if (!plan || on < 0 || on > 2) { set_error("bad argument"); return FMM_ERR_INVALID_ARG; }
+    plan->P.use_graph = on;
+    if (plan->P.adj) plan->P.adj->use_graph = on;
+    return FMM_OK;
 }
 
 fmm_status fmm_plan_set_m2l_variant(fmm_plan* plan, int variant) {

@@ -856,7 +856,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     const bool split = !serial && fast && L > 0 && !Pl.no_split;
     if (split) after(sU, sF, Pl.e_p2m);
     cudaStream_t sM = split ? sU : sF;
-    for (int l = L; l >= 1; --l) {
+    for (int l = L; l > Pl.top_level; --l) {
         if (fast) { xlate_fast_launch(Pl, 0, l, sM); continue; }
         const int64_t nbp = (int64_t)1 << (s * (l - 1));
         m2m_k<T><<<nblocks(nbp, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sM>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbp, Pl.box_count.p,
@@ -887,7 +887,7 @@ void run_t(const Plan& Pl, const void* d_q, void* d_pot, void* d_field, cudaStre
     // L2L (a7).  The register kernels ADD into the children with atomics, exactly like the M2L, so in the split schedule the
     // whole downward pass runs on sU right behind the upper levels' M2L and beside the leaf-level M2L on sF.
     cudaStream_t sL = split ? sU : sF;
-    for (int l = 1; l <= L; ++l) {
+    for (int l = Pl.top_level + 1; l <= L; ++l) {
         if (fast) { xlate_fast_launch(Pl, 2, l, sL); continue; }
         const int64_t nbc = (int64_t)1 << (s * l);
         l2l_k<T><<<nblocks(nbc, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, sL>>>(p, s, Pl.level_off[l - 1], Pl.level_off[l], nbc, Pl.box_count.p,
@@ -929,10 +929,10 @@ void shard_downward_t(const Plan& Pl, const Plan::Shard& sh, void* d_pot, void* 
     const int L = Pl.L;
     FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Lc.p, 0, Pl.Lc.n, st));
     if (L > 0) FMM_CUDA_CHECK(cudaMemsetAsync(Pl.Mc.p, 0, (size_t)Pl.level_off[L] * Pl.Kp * sizeof(T), st));
-    for (int l = L; l >= 1; --l) xlate_fast_launch(Pl, 0, l, st);                       // M2M: every box (redundant on every shard)
+    for (int l = L; l > Pl.top_level; --l) xlate_fast_launch(Pl, 0, l, st);              // M2M: every box (redundant on every shard)
     for (int l = 0; l <= L; ++l)
         if (sh.e1[l] > sh.e0[l]) xlate_fast_launch(Pl, 1, 0, st, sh.e0[l], sh.e1[l]);   // M2L: targets of this shard on level l
-    for (int l = 1; l <= L; ++l)
+    for (int l = Pl.top_level + 1; l <= L; ++l)
         if (sh.box_hi[l] > sh.box_lo[l]) xlate_fast_launch(Pl, 2, l, st, sh.box_lo[l], sh.box_hi[l]);  // L2L into its boxes
     if (sizeof(T) == 4) p2p_fast_launch(Pl, st, d_field != nullptr, sh.item0, sh.item1);
     else p2p_fast64_launch(Pl, st, d_field != nullptr, sh.item0, sh.item1);
@@ -1008,16 +1008,70 @@ int64_t evaluate_launches(const Plan& P) {
     const int64_t w_leaf = (int64_t)P.weak_level_off.size() > P.L ? P.weak_level_off[P.L] : 0;
     int64_t m2l = P.n_weak > 0 ? 1 : 0;
     if (fast && !P.serial && P.L > 0 && w_leaf > 0 && w_leaf < P.n_weak) m2l = 2;  // leaf level and upper levels on two streams
-    return 4 + 2 * (int64_t)P.L + m2l;  // permute, P2M, P2P, L2P(+finalize) + M2M/L2L per level + M2L
+    return 4 + 2 * (int64_t)(P.L - P.top_level) + m2l;  // permute, P2M, P2P, L2P(+finalize) + M2M/L2L per level below top_level + M2L
 }
 
-void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
-    ensure_constants(P);
+static void run_plain(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
     if (P.S) {
         if (P.dtype == FMM_F32) run_st<float>(P, d_q, d_pot, d_field, st, ev, d_dip);
         else run_st<double>(P, d_q, d_pot, d_field, st, ev, d_dip);
     } else if (P.dtype == FMM_F32) run_t<float>(P, d_q, d_pot, d_field, st, ev, d_dip);
     else run_t<double>(P, d_q, d_pot, d_field, st, ev, d_dip);
+}
+
+// One evaluate = about 10 + 2 L launches on three streams; below N ~ 1e5 the host cannot issue them as fast as the device retires
+// them.  The second evaluate with the same caller pointers is therefore captured (on the plan's own stream: the caller's may be
+// the legacy stream, which cannot be captured) and every later one is a single cudaGraphLaunch on the caller's stream.
+void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cudaStream_t st, cudaEvent_t* ev, const void* d_dip) {
+    ensure_constants(P);
+    // above ~5e5 points the device time dwarfs the host's launch cost and the replay measured 2-3 % SLOWER than the stream
+    // schedule at N = 1M (the graph starts its branches in another order): large plans keep the plain launches unless told otherwise
+    const bool want = P.use_graph == 1 || (P.use_graph == 2 && P.N + (P.S ? P.S->N : 0) < ((int64_t)1 << 19));
+    if (ev || !want) { run_plain(P, d_q, d_pot, d_field, st, ev, d_dip); return; }
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        (void)cudaGetLastError();  // the caller is capturing our launches into a graph of their own: the plain schedule is capturable
+        run_plain(P, d_q, d_pot, d_field, st, nullptr, d_dip);
+        return;
+    }
+    const uint64_t stamp = (P.epoch << 8) | ((uint64_t)P.m2l_variant << 2) | (P.serial ? 2u : 0u) | (P.deterministic ? 1u : 0u);
+    Plan::EvalGraph* g = nullptr;
+    for (Plan::EvalGraph& c : P.graphs)
+        if (c.seen > 0 && c.q == d_q && c.pot == d_pot && c.fld == d_field && c.dip == d_dip && c.stamp == stamp) { g = &c; break; }
+    if (g && g->exec) { FMM_CUDA_CHECK(cudaGraphLaunch(g->exec, st)); return; }
+    if (!g) {
+        g = &P.graphs[P.graph_next];
+        P.graph_next = (P.graph_next + 1) % Plan::N_GRAPHS;
+        if (g->exec) {
+            FMM_CUDA_CHECK(cudaDeviceSynchronize());  // rare: a fifth set of pointers evicts a graph that may still be running
+            cudaGraphExecDestroy(g->exec);
+        }
+        *g = Plan::EvalGraph();
+        g->q = d_q; g->pot = d_pot; g->fld = d_field; g->dip = d_dip; g->stamp = stamp;
+    }
+    if (g->seen++ == 0) { run_plain(P, d_q, d_pot, d_field, st, nullptr, d_dip); return; }
+    if (!P.s_cap) FMM_CUDA_CHECK(cudaStreamCreateWithFlags(&P.s_cap, cudaStreamNonBlocking));
+    auto give_up = [&]() {
+        (void)cudaGetLastError();
+        P.use_graph = 0;
+        run_plain(P, d_q, d_pot, d_field, st, nullptr, d_dip);
+    };
+    if (cudaStreamBeginCapture(P.s_cap, cudaStreamCaptureModeRelaxed) != cudaSuccess) { give_up(); return; }
+    cudaGraph_t gr = nullptr;
+    try {
+        run_plain(P, d_q, d_pot, d_field, P.s_cap, nullptr, d_dip);
+    } catch (...) {
+        cudaStreamEndCapture(P.s_cap, &gr);
+        if (gr) cudaGraphDestroy(gr);
+        (void)cudaGetLastError();
+        P.use_graph = 0;
+        throw;
+    }
+    if (cudaStreamEndCapture(P.s_cap, &gr) != cudaSuccess || !gr) { give_up(); return; }
+    const cudaError_t e = cudaGraphInstantiate(&g->exec, gr, 0);
+    cudaGraphDestroy(gr);
+    if (e != cudaSuccess) { g->exec = nullptr; give_up(); return; }
+    FMM_CUDA_CHECK(cudaGraphLaunch(g->exec, st));
 }
 
 }  // namespace fmm

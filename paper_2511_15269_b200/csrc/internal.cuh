@@ -159,6 +159,7 @@ struct Plan {
         int64_t item0 = 0, item1 = 0;         // P2P work items
     };
     mutable Shard shard_cache;
+    int top_level = 0;      // M2M / L2L passes run between the leaf level and this one (finish_lists)
     bool no_split = false;  // evaluate schedule: never run the leaf-level M2L beside the M2M pass (sources may be coarser than targets)
     std::vector<int> march_steps;  // (l_trg, l_src) pairs visited by the level march (cross_level = 1 or separate targets)
 
@@ -194,10 +195,28 @@ struct Plan {
     // internal streams / events of the concurrent evaluate schedule (evaluate.cu), created on first use
     mutable cudaStream_t s_far = nullptr, s_up = nullptr, s_near = nullptr;
     mutable cudaEvent_t e_fork = nullptr, e_perm = nullptr, e_p2m = nullptr, e_up = nullptr, e_near = nullptr, e_done = nullptr;
+    // CUDA graphs of the evaluate schedule (evaluate.cu run_evaluate): the launches of one evaluate -- kernels, memsets and the
+    // fork / join edges between the internal streams -- are captured once per set of caller pointers on s_cap and replayed with one
+    // cudaGraphLaunch; a small cache because forward and adjoint evaluates alternate in an optimisation loop.
+    struct EvalGraph {
+        cudaGraphExec_t exec = nullptr;
+        const void *q = nullptr, *dip = nullptr;
+        void *pot = nullptr, *fld = nullptr;
+        uint64_t stamp = ~0ull;  // Plan::epoch and the schedule switches the graph was captured under
+        int seen = 0;            // evaluates with this key so far (the first runs plainly: one-time attribute / allocation work)
+    };
+    static constexpr int N_GRAPHS = 4;
+    mutable EvalGraph graphs[N_GRAPHS];
+    mutable int graph_next = 0;
+    mutable cudaStream_t s_cap = nullptr;
+    mutable int use_graph = 2;      // fmm_plan_set_graph: 0 never, 1 always, 2 (default) plans with fewer than 2^19 points; set to 0 if a capture fails
+    uint64_t epoch = 0;             // bumped whenever arrays the graphs point into are rebuilt (update, deterministic switch)
     bool serial = false;  // true: every kernel on the caller's stream (fmm_plan_set_schedule)
     bool deterministic = false;  // fmm_plan_set_deterministic: serial schedule, no floating-point atomics with more than one contributor
     ~Plan() {
-        for (cudaStream_t q : {s_far, s_up, s_near})
+        for (EvalGraph& g : graphs)
+            if (g.exec) cudaGraphExecDestroy(g.exec);
+        for (cudaStream_t q : {s_far, s_up, s_near, s_cap})
             if (q) cudaStreamDestroy(q);
         for (cudaEvent_t e : {e_fork, e_perm, e_p2m, e_up, e_near, e_done})
             if (e) cudaEventDestroy(e);

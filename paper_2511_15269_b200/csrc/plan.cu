@@ -663,6 +663,14 @@ static void finish_lists(Plan& P, cudaStream_t st) {
     P.n_p2p_pairs = (int64_t)h[0];
     P.p2p_src_total = (int64_t)h[1];
     build_p2p_items(P, st, P.deterministic);
+    // coarsest level that holds a weak pair: above it no multipole is read and no local expansion is non-zero, so the M2M and
+    // L2L passes stop there (one point set: sources sit on the target's level or one finer, PAPER.md:122-131 / reading S9)
+    P.top_level = 0;
+    if (!P.S && (int)P.weak_level_off.size() == L + 2) {
+        int t = 0;
+        while (t < L && P.weak_level_off[t + 1] == P.weak_level_off[t]) ++t;
+        P.top_level = t;
+    }
 }
 
 // Work items of the P2P kernels: the strong list of a target leaf cut into segments (p2p_segments_k).  single_segment: one item per
@@ -743,23 +751,46 @@ static void sort_by_key(DevBuf<int32_t>& keys, DevBuf<int32_t>& vals, int64_t n,
     FMM_CUDA_CHECK(cudaStreamSynchronize(st));
 }
 
-// mean radius of the non-empty boxes of every level, summed in box order on the host ("average box radius";
-// the oracle sums in the same order, so the comparison of two levels takes the same decision on both sides)
-static std::vector<double> mean_radii(const Plan& P, cudaStream_t st) {
-    std::vector<double> rad(P.n_boxes);
-    std::vector<int32_t> cnt(P.n_boxes);
-    FMM_CUDA_CHECK(cudaMemcpyAsync(rad.data(), P.box_rad.p, P.n_boxes * sizeof(double), cudaMemcpyDeviceToHost, st));
-    FMM_CUDA_CHECK(cudaMemcpyAsync(cnt.data(), P.box_count.p, P.n_boxes * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
-    std::vector<double> m(P.L + 1, 0.0);
-    for (int l = 0; l <= P.L; ++l) {
-        double sum = 0.0;
-        int64_t n = 0;
-        for (int64_t g = P.level_off[l]; g < P.level_off[l + 1]; ++g)
-            if (cnt[g] > 0) { sum += rad[g]; ++n; }
-        m[l] = n ? sum / (double)n : 0.0;
+// mean radius of the non-empty boxes of every level ("average box radius").  The oracle sums a level in box order in
+// fp64; so does the device: one warp per level reads 32 radii at a time (coalesced) and lane 0 adds them one after the other with
+// __dadd_rn, so the comparison of two levels takes the same decision on both sides bit for bit.  A dependent chain of n additions:
+// 0.1 ms for the 32 768 leaves of N = 1M, N_max = 128.
+__global__ void mean_radius_k(const double* __restrict__ rad, const int32_t* __restrict__ cnt, const int64_t* __restrict__ level_off, double* __restrict__ mean) {
+    const int l = blockIdx.x, lane = threadIdx.x;
+    const int64_t g0 = level_off[l], g1 = level_off[l + 1];
+    double sum = 0.0;
+    int64_t n = 0;
+    for (int64_t g = g0; g < g1; g += 32) {
+        const bool in = g + lane < g1;
+        const double r = in ? rad[g + lane] : 0.0;
+        const bool use = in && cnt[g + lane] > 0;
+        const unsigned m = __ballot_sync(0xffffffffu, use);
+        n += __popc(m);
+        if (m == 0xffffffffu) {
+#pragma unroll
+            for (int k = 0; k < 32; ++k) sum = __dadd_rn(sum, __shfl_sync(0xffffffffu, r, k));
+        } else {
+            for (int k = 0; k < 32; ++k) {
+                const double rk = __shfl_sync(0xffffffffu, r, k);
+                if ((m >> k) & 1u) sum = __dadd_rn(sum, rk);
+            }
+        }
     }
-    return m;
+    if (lane == 0) mean[l] = n ? __ddiv_rn(sum, (double)n) : 0.0;
+}
+
+static std::vector<double> mean_radii(const Plan& P, cudaStream_t st) {
+    DevBuf<int64_t> off;
+    DevBuf<double> mean;
+    off.alloc(P.L + 2);
+    mean.alloc(P.L + 1);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(off.p, P.level_off.data(), (P.L + 2) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    mean_radius_k<<<P.L + 1, 32, 0, st>>>(P.box_rad.p, P.box_count.p, off.p, mean.p);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    std::vector<double> m(P.L + 1, 0.0);
+    FMM_CUDA_CHECK(cudaMemcpyAsync(m.data(), mean.p, (P.L + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+    return m;  // L + 1 numbers: the host only compares them to pick the next launch of the march
 }
 
 // Level marching over the target hierarchy (P) and the source hierarchy (P.S, or P itself when sources and targets share one

@@ -17,7 +17,7 @@ FMM_F32, FMM_F64 = 0, 1
 FMM_P_MAX = 16
 
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
-           "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_deterministic", "fmm_plan_set_schedule", "fmm_plan_launches", "fmm_last_error",
+           "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_deterministic", "fmm_plan_set_schedule", "fmm_plan_set_graph", "fmm_plan_launches", "fmm_last_error",
            "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_shard_box_range", "fmm_evaluate_shard_upward",
            "fmm_evaluate_shard_downward", "fmm_plan_leaf_multipoles", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
@@ -65,6 +65,7 @@ def lib():
         L.fmm_plan_set_m2l_variant.argtypes = [vp, C.c_int]
         L.fmm_plan_set_deterministic.argtypes = [vp, C.c_int, vp]
         L.fmm_plan_set_schedule.argtypes = [vp, C.c_int]
+        L.fmm_plan_set_graph.argtypes = [vp, C.c_int]
         L.fmm_plan_launches.argtypes = [vp, i64p]
         L.fmm_translation_work.argtypes = [C.c_int, C.c_int, C.c_int, i64p, i64p, i64p]
         L.fmm_last_error.restype = C.c_char_p
@@ -331,6 +332,11 @@ def fmm_translation_work(p, dtype, kind):
 
 def fmm_plan_set_schedule(plan, serial):
     _check(lib().fmm_plan_set_schedule(plan, int(serial)))
+
+
+def fmm_plan_set_graph(plan, on):
+    """0 never / 1 always / 2 (default) below 2^19 points: repeated evaluates with the same device pointers replay a captured CUDA graph"""
+    _check(lib().fmm_plan_set_graph(plan, int(on)))
 
 
 def fmm_plan_set_deterministic(plan, on, stream=None):
