@@ -67,7 +67,6 @@ struct XArgs {
 // that depends on the ids, and no square roots or divisions in the kernel
 template <typename T, int P, int KIND, int XW, bool GEO>
 __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (XW == 4 ? 4 : 1))) xlate_fast_k(XArgs a) {
-    constexpr bool SYNC = false;
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -97,9 +96,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
         }
     }
     const unsigned vmask = __ballot_sync(0xffffffffu, gs >= 0);
-    if constexpr (!SYNC) {
-        if (vmask == 0) return;
-    }
+    if (vmask == 0) return;
 
     // source rows (CH * 16 contiguous bytes each) arrive by TMA bulk copies that complete on one mbarrier per warp, so the
     // whole batch is in flight at once while the geometry is being loaded
@@ -137,7 +134,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
 
     T v[G::KV];
     V* row = sm + lane * G::KSB;
-    if (SYNC || gs >= 0) {
+    if (gs >= 0) {
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             const V x = row[c];

@@ -1,8 +1,8 @@
 // xlate_reg.cuh -- building blocks of the register ("fast") translation kernels (xlate_fast.cu, xlate_smem.cuh):
 // compile-time loops, application of the constant matrices B_n / B_n^T of rot_tables.cuh with every entry an FFMA
 // immediate, azimuthal rotations (App. B.1 PAPER.md:441 in the normalised basis) and cos/sin(m x) tables.
-// translate_reg is the whole rotate / z-shift / rotate-back operator for one translation held in registers.
-// The value type T is float, double, or the packed pair f2 (two independent translations per thread, f32x2 SASS).
+// translate_qz is the whole rotate / z-shift / rotate-back operator for one translation held in registers (the Q Z loop).
+// The value type T is float or double.
 #pragma once
 #include <type_traits>
 #include <utility>
@@ -13,23 +13,7 @@
 namespace fmm {
 namespace xr {
 
-// ---- packed pair of floats: lane-wise arithmetic on two independent translations (FADD2 / FMUL2 / FFMA2, sm_100)
-struct f2 {
-    unsigned long long v;
-    f2() = default;
-    __device__ __forceinline__ explicit f2(float x) { asm("mov.b64 %0, {%1, %1};" : "=l"(v) : "f"(x)); }
-    __device__ __forceinline__ explicit f2(double x) : f2((float)x) {}
-    __device__ __forceinline__ f2(float lo, float hi) { asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi)); }
-    __device__ __forceinline__ float lo() const { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
-    __device__ __forceinline__ float hi() const { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
-};
-__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2& operator*=(f2& a, f2 b) { a = a * b; return a; }
-__device__ __forceinline__ f2 fma(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
-// a*b - c   (ptxas contracts the packed form into one FFMA2 with a negated addend)
-__device__ __forceinline__ f2 fmsub(f2 a, f2 b, f2 c) { return a * b - c; }
+// a*b - c and a*b + c in the value type
 __device__ __forceinline__ float fmsub(float a, float b, float c) { return ::fmaf(a, b, -c); }
 __device__ __forceinline__ double fmsub(double a, double b, double c) { return ::fma(a, b, -c); }
 __device__ __forceinline__ float fma(float a, float b, float c) { return ::fmaf(a, b, c); }
