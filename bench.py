@@ -102,7 +102,7 @@ def ncu_profile(workload):
             return None
 
     out = {}
-    for key, pat in (("m2l", r"xlate_\w+_k<\w+, \(int\)\d+, \(int\)1[,>]"), ("p2p", r"p2p_\w+_k<")):
+    for key, pat in (("m2l", r"xlate_\w+_k<\w+, (?:\(int\))?\d+, (?:\(int\))?1[,>]"), ("p2p", r"p2p_\w+_k<")):
         sel = [r for r in rows[2:] if len(r) == len(hdr) and re.search(pat, r[ix["Kernel Name"]])]
         if not sel:
             continue

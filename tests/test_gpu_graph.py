@@ -155,3 +155,24 @@ def test_the_caller_can_capture_an_evaluate_into_their_own_graph():
         assert rel2(u.cpu().numpy(), uo) <= 1e-11 and rel2(f.cpu().numpy(), fo) <= 1e-11
         assert rel2(y.cpu().numpy(), 2.0 * uo) <= 1e-11
     P.close()
+
+
+def test_the_binding_rejects_tensors_that_do_not_fit_the_plan():
+    """the C side sees raw pointers only: dtype, shape, contiguity and residency are checked where the tensors still exist"""
+    pos, q = inputs.uniform_cube(1000, 310, np.float32)
+    P = fmm.Plan(dev(pos), 4, 32, 2, 0.77)
+    dq = dev(q)
+    u, f = torch.empty(1000, dtype=torch.float32, device="cuda"), torch.empty((1000, 3), dtype=torch.float32, device="cuda")
+    fmm.fmm_evaluate(P.handle, dq, u, f)
+    for bad in (dict(charges=dq.double()), dict(charges=dq[:999]), dict(charges=dq.cpu()), dict(potential=u.double()), dict(field=f.t().contiguous()),
+                dict(field=torch.empty((1000, 6), dtype=torch.float32, device="cuda")[:, ::2]), dict(charges=q)):
+        args = dict(charges=dq, potential=u, field=f)
+        args.update(bad)
+        with pytest.raises(ValueError):
+            fmm.fmm_evaluate(P.handle, args["charges"], args["potential"], args["field"])
+    with pytest.raises(ValueError):
+        fmm.fmm_evaluate_host(P.handle, dq, u.cpu(), f.cpu())  # the host path wants host buffers
+    h = P.handle
+    P.close()
+    with pytest.raises(ValueError):
+        fmm.fmm_evaluate(h, dq, u, f)  # a destroyed handle never reaches the library
