@@ -122,6 +122,28 @@ fmm_status fmm_evaluate_shard_downward(const fmm_plan* plan, int n_shards, int s
 fmm_status fmm_plan_leaf_multipoles(const fmm_plan* plan, int copy_in, int64_t leaf_begin, int64_t leaf_end, void* d_rows, int64_t* h_row_elems,
                                     void* cuda_stream);
 
+/* Leaf multipoles WITHOUT ANY ALLOCATION, for callers that must not reach cudaMalloc (code under stream capture, tight serving
+ * loops, harnesses that forbid it).  Computes what fmm_evaluate_shard_upward(plan, 1, 0, ...) followed by
+ * fmm_plan_leaf_multipoles(plan, 0, 0, n_leaves, ...) delivers -- the P2M step, eq. (13), for ALL leaves:
+ *     d_rows[leaf * row + n^2 + n + m] = M_n^m of leaf `leaf` for the charges d_charges,  row = *h_row_elems = (p+1)^2 rounded up
+ *     to a multiple of 4 (normalised, length-scaled coefficients; the padding of a row is written as zero)
+ * but with the intermediate array of that step (the particles in tree order, packed x, y, z, q) in a STATIC device array of
+ * FMM_NOALLOC_MAX_BYTES instead of the plan's own scratch, and the rows written straight into the caller's buffer.  The call
+ * writes nothing in the plan (it may run beside an evaluate of the same plan) and calls no cudaMalloc / cudaFree / allocating
+ * library routine.
+ *   plan       : a plan over ONE point set (FMM_ERR_UNSUPPORTED for fmm_plan_create_targets plans), any order p.
+ *   d_charges  : DEVICE, N, dtype, input order.      d_rows : DEVICE, n_leaves x row, dtype, overwritten.
+ *   h_row_elems: HOST out (may be NULL).  d_charges = d_rows = NULL only queries it.
+ * Limit: N x 4 x sizeof(dtype) <= FMM_NOALLOC_MAX_BYTES, i.e. N <= 524 288 (fp32) / 262 144 (fp64); beyond it the call returns
+ * FMM_ERR_UNSUPPORTED with the sizes in fmm_last_error() and launches nothing.
+ * The static array costs FMM_NOALLOC_MAX_BYTES on every GPU that loads the library, until the process exits.  ALL calls on a
+ * device share it: calls that may overlap on the GPU (different streams without an ordering between them) race -- order them.
+ * It keeps the contents of the last call; every call overwrites the part it reads, nothing has to be cleared.
+ * The first call on a device does one-time set-up (symbol address, constant tables) and is not capturable; later calls are
+ * asynchronous on cuda_stream and consist of one memset and two kernel launches. */
+#define FMM_NOALLOC_MAX_BYTES (8u << 20)
+fmm_status fmm_leaf_multipoles_noalloc(const fmm_plan* plan, const void* d_charges, void* d_rows, int64_t* h_row_elems, void* cuda_stream);
+
 /* Same operation with HOST buffers: copies charges host->device, evaluates, copies the results back and
  * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);

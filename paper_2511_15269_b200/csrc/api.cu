@@ -402,6 +402,20 @@ fmm_status fmm_plan_leaf_multipoles(const fmm_plan* plan, int copy_in, int64_t l
     });
 }
 
+fmm_status fmm_leaf_multipoles_noalloc(const fmm_plan* plan, const void* d_charges, void* d_rows, int64_t* h_row_elems, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        const Plan& P = plan->P;
+        if (P.S) { set_error("plans with separate targets are not supported"); return FMM_ERR_UNSUPPORTED; }
+        if (h_row_elems) *h_row_elems = P.Kp;
+        if (!d_charges && !d_rows) return FMM_OK;  // query only
+        if (!d_charges || !d_rows) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(P)) return FMM_ERR_INVALID_ARG;
+        run_leaf_multipoles_noalloc(P, d_charges, d_rows, (cudaStream_t)cuda_stream);  // no AllocScope: nothing is allocated
+        return FMM_OK;
+    });
+}
+
 fmm_status fmm_evaluate_profiled(const fmm_plan* plan, const void* d_charges, void* d_potential, void* d_field, void* cuda_stream,
                                  double* h_stage_ms) {
     return guarded([&]() -> fmm_status {

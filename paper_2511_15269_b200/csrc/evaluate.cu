@@ -1074,4 +1074,84 @@ void run_evaluate(const Plan& P, const void* d_q, void* d_pot, void* d_field, cu
     FMM_CUDA_CHECK(cudaGraphLaunch(g->exec, st));
 }
 
+// ------------------------------------------------------------------------------------------------ leaf multipoles without allocation
+// fmm_leaf_multipoles_noalloc (include/fmm.h): permute + P2M (eq. (13)) of all leaves with the intermediate array of
+// the pair -- the particles in tree order packed as (x, y, z, q), which the evaluate keeps in Plan::pq -- in STATIC device memory,
+// and the rows written straight into the caller's buffer.  For callers that must not reach cudaMalloc (stream capture, serving
+// loops): no allocation here, and nothing of the plan is written, so the call may run beside an evaluate of the same plan.
+//
+// g_noalloc_pq is a file-scope device array: every GPU that loads the library holds its NOALLOC_BYTES until the process exits.
+// In HOST code its name is only a stand-in for the symbol -- never a device address: the address a kernel may be given comes from
+// cudaGetSymbolAddress, asked once per device with that device current (noalloc_scratch below).  All calls on a device share the
+// array and it keeps the last call's contents: permute_k overwrites records [0, N) and p2m_k reads no others, so nothing has to
+// be cleared, but two calls that overlap on the GPU (different streams) race on it.
+namespace {
+
+constexpr size_t NOALLOC_BYTES = (size_t)FMM_NOALLOC_MAX_BYTES;
+static __device__ __align__(256) unsigned char g_noalloc_pq[NOALLOC_BYTES];
+
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[MAX_DEVICES] = {};
+
+void* noalloc_scratch(int dev) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (dev < 0 || dev >= MAX_DEVICES) { set_error("device ordinal out of range"); throw CudaFail{FMM_ERR_UNSUPPORTED}; }
+    if (!g_noalloc_ptr[dev]) {
+        if (current_device() != dev) { set_error("noalloc scratch: not the current device"); throw CudaFail{FMM_ERR_INVALID_ARG}; }
+        void* ptr = nullptr;
+        FMM_CUDA_CHECK(cudaGetSymbolAddress(&ptr, g_noalloc_pq));
+        g_noalloc_ptr[dev] = ptr;
+    }
+    return g_noalloc_ptr[dev];
+}
+
+template <typename T, int P>
+void launch_p2m_to(const Plan& Pl, const void* pq, T* rows_base, cudaStream_t st) {
+    using T4 = typename V4<T>::type;
+    const int64_t leaf0 = Pl.level_off[Pl.L], nl = Pl.n_leaves;
+    if constexpr (sizeof(T) == 4 && P <= 8) {  // the same choice of instantiation as launch_p2m_l2p
+        if (Pl.max_leaf <= 16) {
+            p2m_k<T, P, 16><<<nblocks(nl, WARPS_PER_BLOCK * 2), WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)pq, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
+                                                                                             (const T*)Pl.box_scale.p, leaf0, nl, Pl.Kp, rows_base);
+            return;
+        }
+    }
+    p2m_k<T, P, 32><<<nblocks(nl, WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, 0, st>>>((const T4*)pq, Pl.box_start.p, Pl.box_count.p, Pl.box_ctr.p,
+                                                                                  (const T*)Pl.box_scale.p, leaf0, nl, Pl.Kp, rows_base);
+}
+
+template <typename T>
+void leaf_multipoles_noalloc_t(const Plan& Pl, const void* d_q, void* d_rows, void* scratch, cudaStream_t st) {
+    using T4 = typename V4<T>::type;
+    // rows of the leaves only: p2m_k addresses row g of a whole-tree array, so hand it the base that puts leaf 0 at d_rows
+    T* rows_base = (T*)d_rows - (int64_t)Pl.level_off[Pl.L] * Pl.Kp;
+    FMM_CUDA_CHECK(cudaMemsetAsync(d_rows, 0, (size_t)Pl.n_leaves * Pl.Kp * sizeof(T), st));  // the padding of a row (K..Kp) is zero
+    permute_k<T><<<nblocks(Pl.N, 256), 256, 0, st>>>((const T*)Pl.pos_tree.p, (const T*)d_q, Pl.perm.p, (T4*)scratch, nullptr, nullptr, Pl.N);
+    FMM_CUDA_CHECK(cudaGetLastError());
+    switch (Pl.p) {
+#define FMM_CASE(PP) case PP: launch_p2m_to<T, PP>(Pl, scratch, rows_base, st); break;
+        FMM_CASE(0) FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
+        FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12) FMM_CASE(13) FMM_CASE(14) FMM_CASE(15) FMM_CASE(16)
+#undef FMM_CASE
+    }
+    FMM_CUDA_CHECK(cudaGetLastError());
+}
+
+}  // namespace
+
+int64_t noalloc_max_particles(fmm_dtype dt) { return (int64_t)(NOALLOC_BYTES / (4 * (dt == FMM_F32 ? 4 : 8))); }
+
+void run_leaf_multipoles_noalloc(const Plan& P, const void* d_q, void* d_rows, cudaStream_t st) {
+    if (P.N > noalloc_max_particles(P.dtype)) {
+        set_error("fmm_leaf_multipoles_noalloc: " + std::to_string((long long)P.N) + " particles need " +
+                  std::to_string((long long)P.N * 4 * (P.dtype == FMM_F32 ? 4 : 8)) + " bytes of scratch, the static array holds FMM_NOALLOC_MAX_BYTES = " +
+                  std::to_string((long long)NOALLOC_BYTES) + " (at most " + std::to_string((long long)noalloc_max_particles(P.dtype)) + " particles of this dtype)");
+        throw CudaFail{FMM_ERR_UNSUPPORTED};
+    }
+    ensure_constants(P);                        // once per device: the g_n^m table in constant memory (a copy, no allocation)
+    void* scratch = noalloc_scratch(P.device);  // once per device: cudaGetSymbolAddress
+    if (P.dtype == FMM_F32) leaf_multipoles_noalloc_t<float>(P, d_q, d_rows, scratch, st);
+    else leaf_multipoles_noalloc_t<double>(P, d_q, d_rows, scratch, st);
+}
+
 }  // namespace fmm

@@ -257,5 +257,8 @@ void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool want_field, int64_t 
 void shard_box_range(int L, int s, int n_shards, int shard, int level, int64_t* b0, int64_t* b1);
 void run_shard_upward(const Plan& P, int n_shards, int shard, const void* d_q, cudaStream_t st);
 void run_shard_downward(const Plan& P, int n_shards, int shard, void* d_pot, void* d_field, cudaStream_t st);
+// leaf multipoles of all leaves into the caller's rows, permuted particles in static device memory (fmm_leaf_multipoles_noalloc)
+int64_t noalloc_max_particles(fmm_dtype dt);
+void run_leaf_multipoles_noalloc(const Plan& P, const void* d_q, void* d_rows, cudaStream_t st);
 
 }  // namespace fmm

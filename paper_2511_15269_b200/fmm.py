@@ -19,7 +19,7 @@ FMM_P_MAX = 16
 EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_deterministic", "fmm_plan_set_schedule", "fmm_plan_set_graph", "fmm_plan_launches", "fmm_last_error",
            "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_shard_box_range", "fmm_evaluate_shard_upward",
-           "fmm_evaluate_shard_downward", "fmm_plan_leaf_multipoles", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
+           "fmm_evaluate_shard_downward", "fmm_plan_leaf_multipoles", "fmm_leaf_multipoles_noalloc", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
 
 
 class fmm_admissibility(C.Structure):
@@ -58,6 +58,7 @@ def lib():
         L.fmm_evaluate_shard_upward.argtypes = [vp, C.c_int, C.c_int, vp, vp]
         L.fmm_evaluate_shard_downward.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp]
         L.fmm_plan_leaf_multipoles.argtypes = [vp, C.c_int, C.c_int64, C.c_int64, vp, i64p, vp]
+        L.fmm_leaf_multipoles_noalloc.argtypes = [vp, vp, vp, i64p, vp]
         L.fmm_plan_source_info.argtypes = [vp, i64p, C.POINTER(C.c_int), i64p, i64p]
         L.fmm_plan_copy_source_tree.argtypes = [vp, i32p, i32p, i32p, vp, vp, dp, dp]
         L.fmm_plan_copy_march.argtypes = [vp, i32p, i32p]
@@ -206,6 +207,25 @@ def fmm_plan_leaf_multipoles(plan, copy_in, leaf_begin, leaf_end, rows=None, str
     n = C.c_int64()
     _check(lib().fmm_plan_leaf_multipoles(plan, int(copy_in), int(leaf_begin), int(leaf_end), C.c_void_p(rows.data_ptr()) if rows is not None else None,
                                           C.byref(n), _stream_ptr(stream)))
+    return n.value
+
+
+FMM_NOALLOC_MAX_BYTES = 8 << 20
+
+
+def fmm_leaf_multipoles_noalloc(plan, charges=None, rows=None, stream=None):
+    """P2M of all leaves for `charges` (N,) into `rows` (n_leaves, row): no allocation, scratch in a static device array of
+    FMM_NOALLOC_MAX_BYTES (N <= 524288 fp32 / 262144 fp64), nothing of the plan is written; see include/fmm.h.  Returns the row
+    length in elements; charges = rows = None only queries it."""
+    n = C.c_int64()
+    if charges is not None:
+        _check_io(plan, charges, None, None)
+    if rows is not None:
+        meta = _PLANS.get(plan.value)
+        if meta is None or rows.dtype != meta[0] or not rows.is_cuda or not rows.is_contiguous() or rows.device != meta[3]:
+            raise ValueError("rows must be a contiguous CUDA tensor of the plan's dtype on the plan's device")
+    _check(lib().fmm_leaf_multipoles_noalloc(plan, C.c_void_p(charges.data_ptr()) if charges is not None else None,
+                                             C.c_void_p(rows.data_ptr()) if rows is not None else None, C.byref(n), _stream_ptr(stream)))
     return n.value
 
 
