@@ -148,6 +148,20 @@ fmm_status fmm_leaf_multipoles_noalloc(const fmm_plan* plan, const void* d_charg
  * synchronises.  h_potential / h_field may be NULL.  (The end-to-end path timed by bench.py's "e2e".) */
 fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);
 
+/* The host path as a two-deep pipeline, for callers that evaluate many charge vectors on one plan (time stepping, the
+ * optimisation loop of PAPER.md:281-310): _submit enqueues what fmm_evaluate_host does -- charges host->device, evaluate,
+ * results device->host -- and returns without waiting; _wait blocks until the OLDEST submitted call has delivered its results
+ * into the host buffers it was given.  The copies run on two internal streams, so the 4 B / particle in and 16 B / particle out
+ * of one call cross PCIe while the other call's kernels run (the evaluates themselves stay ordered on cuda_stream: they
+ * share the plan's coefficient arrays).  Each of the two slots owns device staging for charges and results.
+ *   h_charges, h_potential, h_field: HOST, as for fmm_evaluate_host; PINNED memory is needed for the copies to overlap; the
+ *   buffers of a call belong to the library until the matching _wait returns (use two sets when two calls are in flight).
+ * At most two calls may be in flight: a third _submit returns FMM_ERR_UNSUPPORTED; _wait with nothing in flight returns
+ * FMM_ERR_INVALID_ARG.  Results are those of fmm_evaluate_host (same kernels, same schedule).  fmm_plan_update and
+ * fmm_plan_destroy must not be called with calls in flight (destroy waits for them). */
+fmm_status fmm_evaluate_host_submit(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream);
+fmm_status fmm_evaluate_host_wait(const fmm_plan* plan);
+
 /* Separate sources and targets: potential and field AT the Nt targets caused by charges AT the Ns sources.
  * Two hierarchies are built with the same rules (N_max, s): one over the sources, one over the targets; source boxes are
  * compared with target boxes by eq. (4) while marching through the levels from (l_trg, l_src) = (0, 0): 1. increase the

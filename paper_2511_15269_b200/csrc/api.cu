@@ -463,6 +463,58 @@ fmm_status fmm_evaluate_host(const fmm_plan* plan, const void* h_charges, void* 
     });
 }
 
+fmm_status fmm_evaluate_host_submit(const fmm_plan* plan, const void* h_charges, void* h_potential, void* h_field, void* cuda_stream) {
+    return guarded([&]() -> fmm_status {
+        if (!plan || !h_charges) { set_error("NULL pointer argument"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
+        Plan& P = const_cast<Plan&>(plan->P);
+        if (P.hs_count >= 2) { set_error("two submitted calls are in flight: call fmm_evaluate_host_wait first"); return FMM_ERR_UNSUPPORTED; }
+        const size_t es = esize(P.dtype);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        AllocScope scope(st);
+        const int64_t Nq = P.S ? P.S->N : P.N;
+        Plan::HostSlot& h = P.hslot[(P.hs_head + P.hs_count) & 1];
+        if (!P.s_h2d) {
+            FMM_CUDA_CHECK(cudaStreamCreateWithFlags(&P.s_h2d, cudaStreamNonBlocking));
+            FMM_CUDA_CHECK(cudaStreamCreateWithFlags(&P.s_d2h, cudaStreamNonBlocking));
+        }
+        if (!h.q.p) {  // first use of the slot: its buffers come from the pool on st and are used on the copy streams
+            h.q.alloc((size_t)Nq * es);
+            h.out.alloc((size_t)P.N * 4 * es);
+            for (cudaEvent_t* e : {&h.e_in, &h.e_eval, &h.e_out}) FMM_CUDA_CHECK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+            FMM_CUDA_CHECK(cudaStreamSynchronize(st));
+        }
+        // charges in, beside whatever st is still computing (the slot's previous call has been waited for)
+        FMM_CUDA_CHECK(cudaMemcpyAsync(h.q.p, h_charges, (size_t)Nq * es, cudaMemcpyHostToDevice, P.s_h2d));
+        FMM_CUDA_CHECK(cudaEventRecord(h.e_in, P.s_h2d));
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(st, h.e_in, 0));
+        char* dpot = h_potential ? h.out.p : nullptr;
+        char* dfld = h_field ? h.out.p + (size_t)P.N * es : nullptr;
+        run_evaluate(P, h.q.p, dpot, dfld, st, nullptr);
+        FMM_CUDA_CHECK(cudaEventRecord(h.e_eval, st));
+        // results out, beside the next call's evaluate
+        FMM_CUDA_CHECK(cudaStreamWaitEvent(P.s_d2h, h.e_eval, 0));
+        if (h_potential) FMM_CUDA_CHECK(cudaMemcpyAsync(h_potential, dpot, (size_t)P.N * es, cudaMemcpyDeviceToHost, P.s_d2h));
+        if (h_field) FMM_CUDA_CHECK(cudaMemcpyAsync(h_field, dfld, (size_t)P.N * 3 * es, cudaMemcpyDeviceToHost, P.s_d2h));
+        FMM_CUDA_CHECK(cudaEventRecord(h.e_out, P.s_d2h));
+        ++P.hs_count;
+        return FMM_OK;
+    });
+}
+
+fmm_status fmm_evaluate_host_wait(const fmm_plan* plan) {
+    return guarded([&]() -> fmm_status {
+        if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }
+        if (!on_plan_device(plan->P)) return FMM_ERR_INVALID_ARG;
+        Plan& P = const_cast<Plan&>(plan->P);
+        if (P.hs_count == 0) { set_error("no submitted call is in flight"); return FMM_ERR_INVALID_ARG; }
+        FMM_CUDA_CHECK(cudaEventSynchronize(P.hslot[P.hs_head].e_out));
+        P.hs_head ^= 1;
+        --P.hs_count;
+        return FMM_OK;
+    });
+}
+
 fmm_status fmm_plan_info(const fmm_plan* plan, int* L, int64_t* n_boxes, int64_t* n_leaves, int64_t* n_weak, int64_t* n_strong,
                          int64_t* n_p2p_pairs) {
     if (!plan) { set_error("NULL plan"); return FMM_ERR_INVALID_ARG; }

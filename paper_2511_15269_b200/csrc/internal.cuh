@@ -192,6 +192,15 @@ struct Plan {
     DevBuf<int32_t> src_slot;
     int src_G = 0;
     DevBuf<char> h2d_q, d2h_out;  // staging for fmm_evaluate_host
+    // fmm_evaluate_host_submit / _wait (api.cu): two calls may be in flight; the copies of one run on s_h2d / s_d2h beside the
+    // evaluate of the other.  head = oldest call not yet waited for.
+    struct HostSlot {
+        DevBuf<char> q, out;
+        cudaEvent_t e_in = nullptr, e_eval = nullptr, e_out = nullptr;
+    };
+    HostSlot hslot[2];
+    int hs_head = 0, hs_count = 0;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     // internal streams / events of the concurrent evaluate schedule (evaluate.cu), created on first use
     mutable cudaStream_t s_far = nullptr, s_up = nullptr, s_near = nullptr;
     mutable cudaEvent_t e_fork = nullptr, e_perm = nullptr, e_p2m = nullptr, e_up = nullptr, e_near = nullptr, e_done = nullptr;
@@ -216,7 +225,12 @@ struct Plan {
     ~Plan() {
         for (EvalGraph& g : graphs)
             if (g.exec) cudaGraphExecDestroy(g.exec);
-        for (cudaStream_t q : {s_far, s_up, s_near, s_cap})
+        for (HostSlot& h : hslot) {
+            if (h.e_out && hs_count > 0) cudaEventSynchronize(h.e_out);
+            for (cudaEvent_t e : {h.e_in, h.e_eval, h.e_out})
+                if (e) cudaEventDestroy(e);
+        }
+        for (cudaStream_t q : {s_far, s_up, s_near, s_cap, s_h2d, s_d2h})
             if (q) cudaStreamDestroy(q);
         for (cudaEvent_t e : {e_fork, e_perm, e_p2m, e_up, e_near, e_done})
             if (e) cudaEventDestroy(e);

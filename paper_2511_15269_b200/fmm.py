@@ -16,7 +16,7 @@ FMM_OK, FMM_ERR_INVALID_ARG, FMM_ERR_ALLOC, FMM_ERR_CUDA, FMM_ERR_UNSUPPORTED = 
 FMM_F32, FMM_F64 = 0, 1
 FMM_P_MAX = 16
 
-EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
+EXPORTS = ["fmm_plan_create", "fmm_evaluate", "fmm_evaluate_adjoint", "fmm_evaluate_host", "fmm_evaluate_host_submit", "fmm_evaluate_host_wait", "fmm_plan_destroy", "fmm_plan_info", "fmm_plan_copy_tree",
            "fmm_plan_copy_lists", "fmm_evaluate_profiled", "fmm_plan_timings", "fmm_plan_set_m2l_variant", "fmm_plan_set_deterministic", "fmm_plan_set_schedule", "fmm_plan_set_graph", "fmm_plan_launches", "fmm_last_error",
            "fmm_version", "fmm_translation_work", "fmm_plan_update", "fmm_shard_box_range", "fmm_evaluate_shard_upward",
            "fmm_evaluate_shard_downward", "fmm_plan_leaf_multipoles", "fmm_leaf_multipoles_noalloc", "fmm_plan_create_targets", "fmm_plan_source_info", "fmm_plan_copy_source_tree", "fmm_plan_copy_march"]
@@ -46,6 +46,8 @@ def lib():
         L.fmm_plan_create.argtypes = [vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(fmm_admissibility), C.c_int, vp, C.POINTER(vp)]
         L.fmm_evaluate.argtypes = [vp, vp, vp, vp, vp]
         L.fmm_evaluate_host.argtypes = [vp, vp, vp, vp, vp]
+        L.fmm_evaluate_host_submit.argtypes = [vp, vp, vp, vp, vp]
+        L.fmm_evaluate_host_wait.argtypes = [vp]
         L.fmm_evaluate_adjoint.argtypes = [vp, vp, vp, vp, vp]
         L.fmm_evaluate_profiled.argtypes = [vp, vp, vp, vp, vp, dp]
         L.fmm_plan_destroy.argtypes = [vp]
@@ -322,6 +324,25 @@ def fmm_evaluate_host(plan, h_charges, h_potential=None, h_field=None, stream=No
             return C.c_void_p(a.ctypes.data)
         return C.c_void_p(a.data_ptr())
     _check(lib().fmm_evaluate_host(plan, ptr(h_charges), ptr(h_potential), ptr(h_field), _stream_ptr(stream)))
+
+
+def _host_ptr(a):
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return C.c_void_p(a.ctypes.data)
+    return C.c_void_p(a.data_ptr())
+
+
+def fmm_evaluate_host_submit(plan, h_charges, h_potential=None, h_field=None, stream=None):
+    """Pipelined host path: enqueue H2D + evaluate + D2H and return; at most two calls in flight (pinned buffers to overlap)."""
+    _check_io(plan, h_charges, h_potential, h_field, host=True)
+    _check(lib().fmm_evaluate_host_submit(plan, _host_ptr(h_charges), _host_ptr(h_potential), _host_ptr(h_field), _stream_ptr(stream)))
+
+
+def fmm_evaluate_host_wait(plan):
+    """Block until the oldest submitted call has written its results into its host buffers."""
+    _check(lib().fmm_evaluate_host_wait(plan))
 
 
 def fmm_plan_info(plan):
