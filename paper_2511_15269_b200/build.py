@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfmm_b200.so")
-SOURCES = ["api.cu", "plan.cu", "tables.cu", "evaluate.cu", "xlate_fast.cu", "xlate_smem.cu", "xlate_smem_f32.cu", "xlate_smem_f64.cu", "p2p_fast.cu"]
+SOURCES = ["api.cu", "plan.cu", "tables.cu", "evaluate.cu", "xlate_fast.cu", "xlate_smem.cu", "p2p_fast.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr", "--extended-lambda", "-Xptxas", "-v"]
 

@@ -1,11 +1,13 @@
 // xlate_fast.cu -- register ("fast") translation kernels: M2M (a5), M2L (a6) and L2L (a7) with ONE THREAD PER TRANSLATION.
+// Orders 1..8 in fp32 and fp64, orders 9..12 in fp32 (169 state registers + one degree of temporaries fit the 255-register budget
+// at two CTAs of four warps per SM: fp32 p = 12 M2L at N = 1M 2.04 ms against 3.30 ms with the state in shared memory).
 //
 // The operator is the paper's rotate / shift-along-z / rotate-back (App. B) in the
 // normalised, length-scaled representation of tables.cu, where rotations are orthogonal and the polar rotation factors
-// as Q(theta) = B Z(theta) B^T with constant matrices B (rot_tables.cuh).  One translation is
-//     Z(-phi) B Z(-theta) B^T  [z-shift]  B Z(theta) B^T Z(phi)
-// i.e. four azimuthal rotations (2 FP32 instructions per coefficient), four applications of the constant, 3/4-empty B
-// (247 MACs each at p=8) and one O(p^3) z-shift (489 MACs at p=8): about 2.3 k FP32 instructions at p=8.
+// through ONE constant matrix Q_n = polar rotation by pi/2 (rot_tables.cuh), applied four times between azimuthal rotations:
+//     Z(pi/2 - phi) Q Z(pi - theta) Q  [(-1)^m z-shift]  Q Z(theta + pi) Q Z(phi + pi/2)         (xlate_reg.cuh translate_qz)
+// i.e. four azimuthal rotations (4 FP32 instructions per +-m pair), four applications of the constant, 3/4-empty Q (247 MACs each at
+// p = 8) and one O(p^3) z-shift (489 MACs at p = 8): about 2.35 k FP32 instructions at p = 8, run as a loop over one copy of the Q code.
 //
 // Why one thread per translation instead of the paper's / north_star's "one warp per interaction": every step is a
 // batch of small, ragged mat-vecs (block sizes 1..2p+1) with a different right-hand side per interaction, which maps
@@ -20,8 +22,9 @@
 
 // Form of the Q Z loop (xlate_reg.cuh translate_qz), measured on B200 (N = 1M, p = 8, M2L stage): fp32: MODE 0 (A / B trips, no
 // register copies) 0.691 ms, MODE 2 (Q in place) 0.700 ms, MODE 1 (one Q copy + identity trip) 0.75 ms; fp64: MODE 2 1.55 ms,
-// MODE 0 1.66 ms (255 registers either way; MODE 0 spills a little more).
-template <typename T> constexpr int qz_mode() { return sizeof(T) == 4 ? 0 : 2; }
+// MODE 0 1.66 ms (255 registers either way; MODE 0 spills a little more).  fp32, p = 9 / 10 / 12: MODE 2 0.92 / 1.17 / 2.04 ms, MODE 0
+// 0.95 / 1.35 / 2.04 ms.
+template <typename T, int P = 8> constexpr int qz_mode() { return (P > 8 || sizeof(T) == 8) ? 2 : 0; }
 
 namespace fmm {
 namespace {
@@ -66,7 +69,7 @@ struct XArgs {
 // come from records written at plan time (m2l_geo_prepare) -- one coalesced load per word instead of a gather of fp64 centres
 // that depends on the ids, and no square roots or divisions in the kernel
 template <typename T, int P, int KIND, int XW, bool GEO>
-__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (XW == 4 ? 4 : 1))) xlate_fast_k(XArgs a) {
+__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (P > 8 ? (P > 10 ? 2 : 3) : (XW == 8 ? 2 : (XW == 4 ? 4 : 1)))) xlate_fast_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -141,8 +144,8 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (XW == 8 ? 2 : (
             if constexpr (G::E == 4) { v[4 * c] = x.x; v[4 * c + 1] = x.y; v[4 * c + 2] = x.z; v[4 * c + 3] = x.w; }
             else { v[2 * c] = x.x; v[2 * c + 1] = x.y; }
         });
-        if constexpr (GEO) translate_qz_geo<T, P, KIND, qz_mode<T>()>(v, (T)rec[0], (T)rec[1], (T)rec[2], (T)rec[3], (T)rec[4], (T)rec[5], (T)rec[6]);
-        else translate_qz<T, P, KIND, qz_mode<T>()>(v, bx, by, bz, a_old, a_new);
+        if constexpr (GEO) translate_qz_geo<T, P, KIND, qz_mode<T, P>()>(v, (T)rec[0], (T)rec[1], (T)rec[2], (T)rec[3], (T)rec[4], (T)rec[5], (T)rec[6]);
+        else translate_qz<T, P, KIND, qz_mode<T, P>()>(v, bx, by, bz, a_old, a_new);
         sfor<G::CH>([&](auto cc) {
             constexpr int c = decltype(cc)::value;
             V x;
@@ -313,6 +316,9 @@ bool dispatch(int p, const XArgs& a, cudaStream_t st) {
         launch<T, PP, KIND, 4, false>(a, st); return true;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
+#define FMM_CASE(PP) case PP: if constexpr (sizeof(T) == 4) { launch<T, PP, KIND, 4, false>(a, st); return true; } return false;
+        FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12)
+#undef FMM_CASE
         default: return false;
     }
 }
@@ -373,8 +379,7 @@ void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]) {
     if (p < 1 || p > ct::PF) return;
     const int64_t K = (int64_t)(p + 1) * (p + 1), rows = K - 1, nnz = ct::bnnz(p) - 1;  // degree 0 is never touched
     const int64_t zpairs = (int64_t)p * (p + 1) / 2;                                    // (m, -m) pairs of all degrees
-    const bool qz = p <= 8;                                                            // register kernels: Q Z loop
-    const int n_trig = qz ? 4 : 2;                                                     // cos / sin tables built per translation
+    const int n_trig = 4;                                                              // cos / sin tables built per translation (Q Z loop: one per rotation)
     int64_t fma = 0, mul = 0;
     fma += (int64_t)n_trig * p * 2; mul += (int64_t)n_trig * p * 2;                      // addition-theorem recurrences
     fma += 4 * zpairs * 2; mul += 4 * zpairs * 2;                                      // four azimuthal rotations
@@ -390,8 +395,10 @@ void xlate_work(int p, fmm_dtype dt, int kind, int64_t w[3]) {
     w[0] = fma; w[1] = mul; w[2] = 0;
 }
 
-// p <= 8: state vector in registers (this file); 9 <= p <= 12: state vector in shared memory (xlate_smem.cu)
-bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && ((p >= 1 && p <= 8) || xlate_smem_available(p, dt)); }
+// state vector in registers (this file): p <= 8, and fp32 up to p = 12 (169 + 50 registers of 255, two CTAs of four warps per SM);
+// fp64 9 <= p <= 12: state vector in shared memory (xlate_smem.cu)
+static bool reg_kernel(int p, fmm_dtype dt) { return p >= 1 && (p <= 8 || (p <= 12 && dt == FMM_F32)); }
+bool xlate_fast_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && (reg_kernel(p, dt) || xlate_smem_available(p, dt)); }
 
 // deterministic M2L over all target boxes (p <= 8): see m2l_row_k
 bool m2l_row_available(int p, fmm_dtype dt) { return (dt == FMM_F32 || dt == FMM_F64) && p >= 1 && p <= 8; }
@@ -413,7 +420,7 @@ void m2l_row_launch(const Plan& P, cudaStream_t st) {
 }
 
 void xlate_fast_launch(const Plan& P, int kind, int level, cudaStream_t st, int64_t e0, int64_t e1) {
-    if (P.p > 8) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }
+    if (!reg_kernel(P.p, P.dtype)) { xlate_smem_launch(P, kind, level, st, e0, e1); return; }
     XArgs a{};
     a.device = P.device;
     a.box_count = P.box_count.p;

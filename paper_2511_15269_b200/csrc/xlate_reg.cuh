@@ -1,6 +1,7 @@
 // xlate_reg.cuh -- building blocks of the register ("fast") translation kernels (xlate_fast.cu, xlate_smem.cuh):
-// compile-time loops, application of the constant matrices B_n / B_n^T of rot_tables.cuh with every entry an FFMA
-// immediate, azimuthal rotations (App. B.1 PAPER.md:441 in the normalised basis) and cos/sin(m x) tables.
+// compile-time loops, application of the constant matrices Q_n of rot_tables.cuh with every entry an FFMA immediate (fp32) or a
+// materialised constant shared by a symmetric pair (fp64), azimuthal rotations (App. B.1 PAPER.md:441 in the normalised basis) and
+// cos/sin(m x) tables.
 // translate_qz is the whole rotate / z-shift / rotate-back operator for one translation held in registers (the Q Z loop).
 // The value type T is float or double.
 #pragma once
@@ -27,39 +28,6 @@ __device__ __forceinline__ void sfor_impl(F&& f, std::integer_sequence<int, I...
 template <int N, class F>
 __device__ __forceinline__ void sfor(F&& f) {
     if constexpr (N > 0) sfor_impl(f, std::make_integer_sequence<int, N>{});
-}
-
-template <int n, bool TR>
-constexpr double bent(int i, int j) {
-    constexpr int w = 2 * n + 1;
-    return TR ? ct::kTab.B[ct::boff(n) + j * w + i] : ct::kTab.B[ct::boff(n) + i * w + j];
-}
-template <int n, bool TR>
-constexpr bool bfirst(int i, int j) {
-    for (int jj = 0; jj < j; ++jj)
-        if (bent<n, TR>(i, jj) != 0.0) return false;
-    return true;
-}
-
-// v[o .. o+2n] <- B_n v  (TR = false)  or  B_n^T v  (TR = true)
-template <typename T, int n, bool TR, int KV>
-__device__ __forceinline__ void apply_B(T (&v)[KV]) {
-    constexpr int w = 2 * n + 1, o = n * n;
-    T t[w];
-    sfor<w>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        T acc = T(0.f);
-        sfor<w>([&](auto jc) {
-            constexpr int j = decltype(jc)::value;
-            constexpr double b = bent<n, TR>(i, j);
-            if constexpr (b != 0.0) {
-                if constexpr (bfirst<n, TR>(i, j)) acc = T(b) * v[o + j];
-                else acc = fma(T(b), v[o + j], acc);
-            }
-        });
-        t[i] = acc;
-    });
-    sfor<w>([&](auto ic) { v[o + decltype(ic)::value] = t[decltype(ic)::value]; });
 }
 
 // azimuthal rotation of degree n (App. B.1 PAPER.md:441 in the normalised basis); SG = +1 forward, -1 inverse
@@ -105,9 +73,10 @@ __device__ __forceinline__ void trig_table(T c1, T s1, T (&c)[P1], T (&s)[P1]) {
 // the azimuthal code (35 KB of SASS at p = 8, 48 KB with prologue and epilogue); this form is 20 KB, so the whole kernel
 // stays inside the 32 KB instruction cache of an SM.  Measured on B200 with a synthetic FFMA stream (4 warps per
 // scheduler): bodies up to 32 KB issue at 0.97 instructions per clock and scheduler, bodies of 48 KB and more at 0.5.
-// Matrix entries are immediates of the FMA that uses them (fp32) or are materialised by two uniform moves (fp64).  Measured: taking
-// the fp64 entries from a 59 KB __constant__ table instead (one LDC / LDCU per one or two entries) makes the fp64 p = 8 M2L 1.7x
-// slower (2.64 vs 1.55 ms at N = 1M): the table does not fit the constant cache.
+// Matrix entries are immediates of the FMA that uses them (fp32) or are materialised by two uniform moves (fp64).  Measured on B200
+// (N = 1M, fp64 M2L): entries from a compact __constant__ table in the order of use (one 16-byte uniform load per two entries)
+// 1.89 vs 1.55 ms at p = 8 and 13.4 vs 11.3 ms at p = 12; entries from a table in shared memory (broadcast LDS.128, one per two
+// entries) 1.87 vs 1.55 ms and 13.1 vs 11.3 ms: every memory-sourced operand loses against the two uniform moves.
 template <typename T, int n, int i, int j>
 __device__ __forceinline__ T q_coef() {
     constexpr double v = ct::kTab.Q[ct::boff(n) + i * (2 * n + 1) + j];
@@ -136,24 +105,55 @@ constexpr bool qfirst(int i, int j) {
     return true;
 }
 
-// dst[od .. od+2n] <- Q_n src[os .. os+2n]   (src and dst must be different register sets)
-template <typename T, int n, int os, int od, int NS, int ND>
+// dst[od .. od+2n] <- Q_n src[os .. os+2n]   (src and dst must be different register sets)                        FORM 0
+// fp64 (FORM 1 / 2): a double is not an immediate but two uniform moves per use.  Q_n^T = D Q_n D with D = Z(pi) = diag((-1)^m)
+// (rot_tables.cuh), hence Q D and D Q are SYMMETRIC matrices: FORM 1 applies S = Q D, FORM 2 applies S = D Q, and the entries (i, j) and
+// (j, i) are served by ONE materialised constant -- half the moves, a quarter of all instructions of an fp64 translation.  The
+// missing D costs nothing: next to an azimuthal rotation it is a half turn of the angle (Z(a) D = D Z(a) = Z(a + pi)), next to the
+// z-shift it cancels the (-1)^m that the Q Z form folds into the shift constants.  fp32 entries are free immediates and keep the
+// row-by-row form (shorter live ranges).
+template <int n, int FORM>
+constexpr double sent(int i, int j) {
+    const double q = qent<n>(i, j);
+    const int k = FORM == 1 ? j : i;  // the index whose order m = k - n carries the sign
+    return FORM == 0 ? q : (((k - n) & 1) ? -q : q);
+}
+template <typename T, int n, int os, int od, int FORM = 0, int NS, int ND>
 __device__ __forceinline__ void q_from_to(const T (&src)[NS], T (&dst)[ND]) {
     constexpr int w = 2 * n + 1;
-    sfor<w>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        T acc = T(0.f);
-        sfor<w>([&](auto jc) {
-            constexpr int j = decltype(jc)::value;
-            constexpr double b = qent<n>(i, j);
-            if constexpr (b != 0.0) {
-                if constexpr (qfirst<n>(i, j)) acc = q_coef<T, n, i, j>() * src[os + j];
-                else acc = fma(q_coef<T, n, i, j>(), src[os + j], acc);
-            }
+    if constexpr (FORM != 0) {
+        sfor<w>([&](auto ic) { dst[od + decltype(ic)::value] = T(0); });
+        sfor<w>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            sfor<w - i>([&](auto dc) {
+                constexpr int j = i + decltype(dc)::value;
+                constexpr double b = sent<n, FORM>(i, j), bt = sent<n, FORM>(j, i);
+                static_assert(b - bt < 1e-13 && bt - b < 1e-13, "Q D and D Q are symmetric");
+                if constexpr (b != 0.0) {
+                    const T c = T(b);
+                    dst[od + i] = fma(c, src[os + j], dst[od + i]);
+                    if constexpr (j != i) dst[od + j] = fma(c, src[os + i], dst[od + j]);
+                }
+            });
         });
-        dst[od + i] = acc;
-    });
+    } else {
+        sfor<w>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            T acc = T(0.f);
+            sfor<w>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                constexpr double b = qent<n>(i, j);
+                if constexpr (b != 0.0) {
+                    if constexpr (qfirst<n>(i, j)) acc = q_coef<T, n, i, j>() * src[os + j];
+                    else acc = fma(q_coef<T, n, i, j>(), src[os + j], acc);
+                }
+            });
+            dst[od + i] = acc;
+        });
+    }
 }
+template <typename T>
+constexpr int q_form(int which) { return sizeof(T) == 8 ? which : 0; }
 
 // dst <- Z_n(angle) src for one degree (App. B.1 PAPER.md:441 in the normalised basis, forward sense); order 0 is copied
 template <typename T, int n, int os, int od, int NS, int ND, int P1>
@@ -169,7 +169,8 @@ __device__ __forceinline__ void az_from_to(const T (&src)[NS], T (&dst)[ND], con
 
 // z-shift of App. B.3 in the normalised, scaled representation, times (-1)^m (see above); in place.
 // M2L expects v already scaled by x2^k and applies x1^n / r; M2M expects v scaled by x2^k; L2L applies x2^n itself.
-template <typename T, int P, int KIND, bool FUSE, int KV>
+// SIGNED = false: the plain shift (the (-1)^m has been cancelled by the D of a symmetric Q form, see q_from_to)
+template <typename T, int P, int KIND, bool FUSE, bool SIGNED = true, int KV>
 __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
     constexpr int P1 = P + 1;
     if constexpr (KIND == 1) {
@@ -180,17 +181,33 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
         }
         sfor<2 * P + 1>([&](auto mi) {
             constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-            constexpr double sg = (am & 1) ? -1.0 : 1.0;
+            constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
             T t[cnt];
-            sfor<cnt>([&](auto ni) {
-                constexpr int n = am + decltype(ni)::value;
-                T acc = h_coef<T, am, n, am, (sg < 0)>() * v[am * am + am + m];
-                sfor<cnt - 1>([&](auto ki) {
-                    constexpr int k = am + 1 + decltype(ki)::value;
-                    acc = fma(h_coef<T, am, n, k, (sg < 0)>(), v[k * k + k + m], acc);
+            if constexpr (!SIGNED) {
+                // fp64 (symmetric forms): H[m][n][k] = (-1)^(k+m) X(n, k) with X symmetric; the caller has scaled v by (-x2)^k, so the
+                // matrix left is (-1)^m X(n, k), and its entries (n, k) and (k, n) share one materialised constant (see q_from_to)
+                sfor<cnt>([&](auto ni) { t[decltype(ni)::value] = T(0); });
+                sfor<cnt>([&](auto ni) {
+                    constexpr int n = am + decltype(ni)::value;
+                    sfor<cnt - decltype(ni)::value>([&](auto dk) {
+                        constexpr int k = n + decltype(dk)::value;
+                        constexpr double b = ((k & 1) ? -1.0 : 1.0) * ct::kTab.H[am][n][k];
+                        const T c = T(b);
+                        t[n - am] = fma(c, v[k * k + k + m], t[n - am]);
+                        if constexpr (k != n) t[k - am] = fma(c, v[n * n + n + m], t[k - am]);
+                    });
                 });
-                t[decltype(ni)::value] = acc;
-            });
+            } else {
+                sfor<cnt>([&](auto ni) {
+                    constexpr int n = am + decltype(ni)::value;
+                    T acc = h_coef<T, am, n, am, (sg < 0)>() * v[am * am + am + m];
+                    sfor<cnt - 1>([&](auto ki) {
+                        constexpr int k = am + 1 + decltype(ki)::value;
+                        acc = fma(h_coef<T, am, n, k, (sg < 0)>(), v[k * k + k + m], acc);
+                    });
+                    t[decltype(ni)::value] = acc;
+                });
+            }
             // the output scaling x1^n / r is also the write-back (no register copies inside the run-time loop of translate_qz)
             sfor<cnt>([&](auto ni) {
                 constexpr int n = am + decltype(ni)::value;
@@ -214,10 +231,10 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
             // out[n] = (-1)^m sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (A[m][n][n] = 1): in place, n descending
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                constexpr double sg = (am & 1) ? -1.0 : 1.0;
+                constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = P - decltype(ni)::value;
-                    T acc = (am & 1) ? T(0) - v[n * n + n + m] : v[n * n + n + m];
+                    T acc = (SIGNED && (am & 1)) ? T(0) - v[n * n + n + m] : v[n * n + n + m];
                     sfor<n - am>([&](auto ki) {
                         constexpr int k = am + decltype(ki)::value;
                         acc = fma(a_coef<T, am, n, k, (sg < 0)>() * pw1[n - k], v[k * k + k + m], acc);
@@ -232,7 +249,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
             sfor<P>([&](auto jc) { pw2[decltype(jc)::value + 1] = pw2[decltype(jc)::value] * x2; });
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                constexpr double sg = (am & 1) ? -1.0 : 1.0;
+                constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = am + decltype(ni)::value;
                     T acc = v[n * n + n + m];
@@ -292,28 +309,39 @@ template <typename T, int P, int KIND, int MODE, int KV>
 __device__ __forceinline__ void translate_qz_geo(T (&v)[KV], T ct_, T st_, T cp_, T sp_, T rinv, T x1, T x2) {
     constexpr int P1 = P + 1;
     if constexpr (KIND != 2) {  // M2M / M2L: the source scaling x2^n commutes with the rotations
+        // fp64 M2L (symmetric shift, see shift_signed): (-x2)^n
+        const T xs = (KIND == 1 && MODE == 2 && sizeof(T) == 8) ? T(0) - x2 : x2;
         T pw = T(1);
         sfor<P>([&](auto nc) {
             constexpr int n = decltype(nc)::value + 1;
-            pw *= x2;
+            pw *= xs;
             sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] *= pw; });
         });
     }
-    if constexpr (MODE == 2) {  // experiment: Z | Q Z | Q S | Q Z | Q Z with Q in place (register copies at the back edge)
+    if constexpr (MODE == 2) {  // Z | Q Z | Q S | Q Z | Q Z with Q in place (register copies at the back edge)
+        // fp64: Q = D (D Q) with the symmetric D Q applied from paired constants (q_from_to FORM 2); the D that is left turns the
+        // rotation that follows by pi -- Z(theta + pi) D = Z(theta), Z(pi - theta) D = Z(-theta), Z(pi/2 - phi) D = Z(3 pi/2 - phi)
+        // -- and takes the (-1)^m out of the shift
+        constexpr bool SYM = sizeof(T) == 8;
 #pragma unroll 1
         for (int t = 0; t < 5; ++t) {
             if (t > 0)
                 sfor<P>([&](auto nc) {
                     constexpr int n = decltype(nc)::value + 1;
                     T tt[2 * n + 1];
-                    q_from_to<T, n, n * n, 0>(v, tt);
+                    q_from_to<T, n, n * n, 0, q_form<T>(2)>(v, tt);
                     sfor<2 * n + 1>([&](auto ic) { v[n * n + decltype(ic)::value] = tt[decltype(ic)::value]; });
                 });
             if (t == 2) {
-                shift_signed<T, P, KIND, (MODE != 2)>(v, x1, x2, rinv);
+                shift_signed<T, P, KIND, (MODE != 2), !SYM>(v, x1, x2, rinv);
             } else {
                 T c1, s1, c[P1], s[P1];
-                qz_angle<T>(t < 2 ? t : t - 1, ct_, st_, cp_, sp_, c1, s1);
+                if constexpr (SYM) {
+                    c1 = t == 0 ? T(0) - sp_ : (t == 4 ? T(0) - sp_ : ct_);
+                    s1 = t == 0 ? cp_ : (t == 1 ? st_ : (t == 3 ? T(0) - st_ : T(0) - cp_));
+                } else {
+                    qz_angle<T>(t < 2 ? t : t - 1, ct_, st_, cp_, sp_, c1, s1);
+                }
                 trig_table<T, P1>(c1, s1, c, s);
                 sfor<P>([&](auto nc) { apply_az<T, decltype(nc)::value + 1, +1>(v, c, s); });
             }
