@@ -82,7 +82,10 @@ __device__ __forceinline__ void regular_rec(T x, T y, T z, F&& emit) {
 }
 
 // ------------------------------------------------------------------------------------------------ P2M (a4), warp per leaf
-constexpr int WARPS_PER_BLOCK = 4;
+#ifndef FMM_WPB
+#define FMM_WPB 4
+#endif
+constexpr int WARPS_PER_BLOCK = FMM_WPB;
 
 // LPL = lanes per leaf: 32 (a warp per leaf) or 16 (two leaves per warp, for plans whose leaves hold <= 16 particles).
 template <typename T, int P, int LPL>

@@ -53,7 +53,9 @@ __device__ __forceinline__ float rsq(float x) {
     return r;
 }
 
-constexpr int PW = 4;   // warps per CTA (independent of one another)
+// warps per CTA (independent of one another).  One: a CTA's resources are held until its slowest warp is done and the items differ (a leaf has
+// 8-27 strong-list entries); measured on B200, P2P of config 2: 4 warps 0.480 ms, 2: 0.477, 1: 0.463 ms; config 4: 0.451 -> 0.405 ms
+constexpr int PW = 1;
 constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two tiles per warp = 8 KB of shared memory
 
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond

@@ -67,9 +67,15 @@ struct XArgs {
 
 // XW warps per CTA; GEO (fp32 M2L only): target ids and the geometry of every pair (cos / sin of the two angles, 1/r, scale ratios)
 // come from records written at plan time (m2l_geo_prepare) -- one coalesced load per word instead of a gather of fp64 centres
-// that depends on the ids, and no square roots or divisions in the kernel
+// that depends on the ids, and no square roots or divisions in the kernel.
+// One warp per CTA (XW = 1): the warps of a CTA never cooperate, and a CTA keeps its registers and shared memory until its slowest
+// warp is done -- batches differ (number of target runs in the epilogue, TMA copies in the prologue).  Measured on B200, config 2 M2L:
+// 4 warps per CTA 0.695 ms, 2: 0.683 ms, 1: 0.659 ms (config 4, p = 6: 1.60 -> 1.28 ms).  Warps per SM by the register budget:
+// fp32 p <= 8: 16 (128 registers), p = 9, 10: 12 (168), fp32 p = 11, 12 and fp64: 8 (255).
+template <typename T, int P>
+constexpr int xlate_warps_per_sm() { return sizeof(T) == 8 ? 8 : (P > 10 ? 8 : (P > 8 ? 12 : 16)); }
 template <typename T, int P, int KIND, int XW, bool GEO>
-__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (P > 8 ? (P > 10 ? 2 : 3) : (XW == 8 ? 2 : (XW == 4 ? 4 : 1)))) xlate_fast_k(XArgs a) {
+__global__ void __launch_bounds__(XW * 32, xlate_warps_per_sm<T, P>() / XW) xlate_fast_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -184,7 +190,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : (P > 8 ? (P > 10
     }
 }
 
-template <typename T, int P, int KIND, int XW = 4, bool GEO = false>
+template <typename T, int P, int KIND, int XW = 1, bool GEO = false>
 void launch(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
     constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;  // rows + one mbarrier per warp
@@ -201,7 +207,7 @@ void launch(const XArgs& a, cudaStream_t st) {
 // at the price of idle lanes in the last batch of every row (~9 % at config 2) and of the plan-time geometry records (their batches
 // are cut differently).
 template <typename T, int P, int XW>
-__global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : 4) m2l_row_k(XArgs a) {
+__global__ void __launch_bounds__(XW * 32, xlate_warps_per_sm<T, P>() / XW) m2l_row_k(XArgs a) {
     using G = Geo<T, P>;
     using V = typename Vec16<T>::type;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -291,7 +297,7 @@ __global__ void __launch_bounds__(XW * 32, sizeof(T) == 8 ? 1 : 4) m2l_row_k(XAr
 template <typename T, int P>
 void launch_row(const XArgs& a, cudaStream_t st) {
     using G = Geo<T, P>;
-    constexpr int XW = 4;
+    constexpr int XW = 1;  // rows differ in length: one warp per CTA (see xlate_fast_k)
     constexpr size_t smem = (size_t)XW * 32 * G::KSB * 16 + XW * 8;
     static AttrOnce once;
     once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(m2l_row_k<T, P, XW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
@@ -312,11 +318,11 @@ template <typename T, int KIND>
 bool dispatch(int p, const XArgs& a, cudaStream_t st) {
     switch (p) {
 #define FMM_CASE(PP) case PP: \
-        if constexpr (sizeof(T) == 4 && KIND == 1) { if (a.geo) { launch<T, PP, KIND, 4, true>(a, st); return true; } } \
-        launch<T, PP, KIND, 4, false>(a, st); return true;
+        if constexpr (sizeof(T) == 4 && KIND == 1) { if (a.geo) { launch<T, PP, KIND, 1, true>(a, st); return true; } } \
+        launch<T, PP, KIND, 1, false>(a, st); return true;
         FMM_CASE(1) FMM_CASE(2) FMM_CASE(3) FMM_CASE(4) FMM_CASE(5) FMM_CASE(6) FMM_CASE(7) FMM_CASE(8)
 #undef FMM_CASE
-#define FMM_CASE(PP) case PP: if constexpr (sizeof(T) == 4) { launch<T, PP, KIND, 4, false>(a, st); return true; } return false;
+#define FMM_CASE(PP) case PP: if constexpr (sizeof(T) == 4) { launch<T, PP, KIND, 1, false>(a, st); return true; } return false;
         FMM_CASE(9) FMM_CASE(10) FMM_CASE(11) FMM_CASE(12)
 #undef FMM_CASE
         default: return false;
