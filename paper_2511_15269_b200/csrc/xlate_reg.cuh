@@ -181,7 +181,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
         }
         sfor<2 * P + 1>([&](auto mi) {
             constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-            constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
+            [[maybe_unused]] constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
             T t[cnt];
             if constexpr (!SIGNED) {
                 // fp64 (symmetric forms): H[m][n][k] = (-1)^(k+m) X(n, k) with X symmetric; the caller has scaled v by (-x2)^k, so the
@@ -231,7 +231,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
             // out[n] = (-1)^m sum_{k=|m|..n} A[|m|][n][k] x1^(n-k) v[k]   (A[m][n][n] = 1): in place, n descending
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
+                [[maybe_unused]] constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = P - decltype(ni)::value;
                     T acc = (SIGNED && (am & 1)) ? T(0) - v[n * n + n + m] : v[n * n + n + m];
@@ -249,7 +249,7 @@ __device__ __forceinline__ void shift_signed(T (&v)[KV], T x1, T x2, T rinv) {
             sfor<P>([&](auto jc) { pw2[decltype(jc)::value + 1] = pw2[decltype(jc)::value] * x2; });
             sfor<2 * P + 1>([&](auto mi) {
                 constexpr int m = decltype(mi)::value - P, am = m < 0 ? -m : m, cnt = P - am + 1;
-                constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
+                [[maybe_unused]] constexpr double sg = (SIGNED && (am & 1)) ? -1.0 : 1.0;
                 sfor<cnt>([&](auto ni) {
                     constexpr int n = am + decltype(ni)::value;
                     T acc = v[n * n + n + m];
