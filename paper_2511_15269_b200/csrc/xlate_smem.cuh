@@ -15,13 +15,15 @@
 // cooperative row copies / run sums (fixed column, consecutive idx) are both conflict-free.
 // History (N = 1M uniform cube, fp64 M2L, B200, ms at p = 9 / 10 / 11 / 12): round 1's straight-line B form (three passes over the state,
 // 100+ KB of code at p = 12) 3.06 / 5.34 / 7.88 / 14.17; Q Z trips 3.80 / 5.67 / 7.37 / 11.30; trips with two roles 3.56 / 4.82 / 7.76 /
-// 9.95; trips, two roles, symmetric constants (this file) 3.22 / 4.06 / 6.64 / 8.63.
+// 9.95; + symmetric constants 3.22 / 4.06 / 6.64 / 8.63 (8.57 with the other kernels' one-warp CTAs beside it); + the two roles paired step by
+// step (two degrees per step; +m and -m of the shift at the same time on the same code) 3.06 / 3.76 / 6.17 / 7.86 (this file).
 #pragma once
 #include "xlate_reg.cuh"
 
 #ifndef FMM_SMEM_ROLES
 #define FMM_SMEM_ROLES 2
 #endif
+
 
 namespace fmm {
 namespace {
@@ -56,13 +58,9 @@ __device__ __forceinline__ void meet() {
 }
 
 // state element idx of this thread: col[idx * LD]
-// R = 2: two warps share the 32 columns of a batch and split every pass between them -- the rotations by degree (mine_n), the
-// z-shift by order (mine_m) -- with a CTA barrier where the ownership changes (before and after the shift).  The state of a
+// R = 2: two warps share the 32 columns of a batch and split every pass between them -- the rotations by degree, the z-shift by
+// order (+m / -m) -- with a CTA barrier where the ownership changes (before and after the shift).  The state of a
 // translation stays one column of shared memory; what doubles is the number of warps that work on it.
-template <int P, int R>
-__device__ __forceinline__ bool mine_n(int n, int role) { return R == 1 || (((P - n) & 3) == 0 || ((P - n) & 3) == 3) == (role == 0); }  // sum of (2n+1)^2 balanced to 4 %
-template <int R>
-__device__ __forceinline__ bool mine_m(int am, int neg, int role) { return R == 1 || ((am + neg) & 1) == role; }                    // +m and -m cost the same
 template <int R>
 __device__ __forceinline__ void handover() {
     if constexpr (R > 1) __syncthreads();
@@ -151,10 +149,11 @@ __device__ __forceinline__ void translate_trips(T* __restrict__ col, T bx, T by,
             sfor<P1>([&](auto mi) {
                 constexpr int am = decltype(mi)::value, cnt = P - am + 1;
                 constexpr bool NEG = !SYM && (am & 1) != 0;
+                // one role: order +am, then -am (same weights, same code); two roles: one of the two orders each, at the same time
+                const int sg0 = R == 1 ? 0 : ((role + am) & 1), sg1 = R == 1 ? (am ? 2 : 1) : ((am || sg0 == 0) ? sg0 + 1 : sg0);
 #pragma unroll 1
-                for (int sg = 0; sg < (am ? 2 : 1); ++sg) {
-                    if (!mine_m<R>(am, sg, role)) continue;
-                    T* cm = col + (sg ? -am : am) * LD;  // order +am, then -am: same weights
+                for (int sg = sg0; sg < sg1; ++sg) {
+                    T* cm = col + (sg ? -am : am) * LD;
                     T w[cnt];
                     sfor<cnt>([&](auto ki) {
                         constexpr int k = am + decltype(ki)::value;
@@ -166,8 +165,9 @@ __device__ __forceinline__ void translate_trips(T* __restrict__ col, T bx, T by,
                         constexpr int k = am + decltype(ki)::value;
                         cm[(k * k + k) * LD] = w[decltype(ki)::value];
                     });
-                    meet<SYNC>();
+                    if constexpr (R == 1) meet<SYNC>();
                 }
+                if constexpr (R > 1) meet<SYNC>();  // outside the loop: both roles pass here once per |m|
             });
             handover<R>();
             continue;
@@ -184,21 +184,36 @@ __device__ __forceinline__ void translate_trips(T* __restrict__ col, T bx, T by,
             }
             trig_table<T, P1>(c1, s1, c, s);
         }
-        sfor<P>([&](auto nc) {
-            constexpr int n = decltype(nc)::value + 1, w = 2 * n + 1;
-            if (!mine_n<P, R>(n, role)) return;
-            T v[w];
-            sfor<w>([&](auto ic) { v[decltype(ic)::value] = col[(n * n + decltype(ic)::value) * LD]; });
-            if (doZ) az_from_to<T, n, 0, 0>(v, v, c, s);
-            if (doQ) {
-                T tt[w];
-                q_from_to<T, n, 0, 0, q_form<T>(1)>(v, tt);
-                sfor<w>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = tt[decltype(ic)::value]; });
-            } else {
-                sfor<w>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = v[decltype(ic)::value]; });
+        auto rotate_degree = [&](auto nc) {
+            constexpr int n = decltype(nc)::value, w = 2 * n + 1;
+            if constexpr (n >= 1 && n <= P) {
+                T v[w];
+                sfor<w>([&](auto ic) { v[decltype(ic)::value] = col[(n * n + decltype(ic)::value) * LD]; });
+                if (doZ) az_from_to<T, n, 0, 0>(v, v, c, s);
+                if (doQ) {
+                    T tt[w];
+                    q_from_to<T, n, 0, 0, q_form<T>(1)>(v, tt);
+                    sfor<w>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = tt[decltype(ic)::value]; });
+                } else {
+                    sfor<w>([&](auto ic) { col[(n * n + decltype(ic)::value) * LD] = v[decltype(ic)::value]; });
+                }
             }
-            meet<SYNC>();
-        });
+        };
+        if constexpr (R == 1) {
+            sfor<P>([&](auto nc) {
+                rotate_degree(std::integral_constant<int, decltype(nc)::value + 1>{});
+                meet<SYNC>();
+            });
+        } else {
+            // two roles: step k pairs the degrees P - 4 (k / 2) - {0, 3} (role 0) and P - 4 (k / 2) - {1, 2} (role 1): the sums of
+            // (2n+1)^2 of the two roles agree to 4 %, and both roles pass the same number of meeting points
+            sfor<(P + 1) / 2>([&](auto kc) {
+                constexpr int k = decltype(kc)::value, base = P - 4 * (k / 2);
+                if (role == 0) rotate_degree(std::integral_constant<int, base - ((k & 1) ? 3 : 0)>{});
+                else rotate_degree(std::integral_constant<int, base - ((k & 1) ? 2 : 1)>{});
+                meet<SYNC>();
+            });
+        }
     }
 }
 
@@ -281,7 +296,9 @@ template <typename T, int P, int KIND>
 void launch(const SArgs& a, cudaStream_t st) {
     constexpr int K = (P + 1) * (P + 1);
     // M2L: 32 translations per CTA, two warps share them (R = 2) -- twice the warps for the same shared memory; M2M / L2L: 64 per CTA
-    constexpr int R = KIND == 1 ? FMM_SMEM_ROLES : 1, NT = KIND == 1 ? 32 * R : 64, MT = R > 1 ? 1 : 2;
+    // Measured (fp64 M2L, N = 1M, p = 9 / 10 / 11 / 12): 32 columns per CTA, no barrier inside a pass 3.06 / 3.76 / 6.17 / 7.86 ms; ONE CTA of
+    // 160 columns x 2 roles per SM whose ten warps meet at a barrier after every block (they walk the code together) 4.78 / 5.51 / 6.28 / 7.64 ms
+    constexpr int R = KIND == 1 ? FMM_SMEM_ROLES : 1, NT = KIND == 1 ? 32 * R : 64, MT = 1;
     constexpr size_t smem = (size_t)K * (NT / R + 1) * sizeof(T);
     static AttrOnce once;
     once.ensure(a.device, [&] { FMM_CUDA_CHECK(cudaFuncSetAttribute(xlate_smem_k<T, P, KIND, NT, MT, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); });
