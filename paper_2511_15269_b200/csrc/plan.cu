@@ -685,12 +685,13 @@ void build_p2p_items(Plan& P, cudaStream_t st, bool single_segment) {
         const int32_t* lcnt = P.box_count.p + P.level_off[L];
         const int64_t mean_src = (int64_t)(h1 / (unsigned long long)(P.n_leaves > 0 ? P.n_leaves : 1));
         int64_t budget = mean_src * 2 > 1024 ? mean_src * 2 : 1024;
-        // small problems: fewer target leaves than the chip has warp slots -- cut the lists finer (down to 128 source particles
-        // per item) so that about 8 warps per SM find work; the partial sums of a leaf are then combined with atomics
-        const int64_t want_items = 148 * 8;
+        // small problems: fewer target leaves than the chip has warp slots -- cut the lists finer (down to 64 source particles
+        // per item; a list is cut between source leaves) so that about 16 warps per SM find work; the partial sums of a leaf are then
+        // combined with atomics.  Config 1 (N = 4096, fp64, 64 leaves of 64): 8 warps per SM / 128 sources 43.0 us per evaluate, this 32.9 us
+        const int64_t want_items = 148 * 16;
         if (P.n_leaves < want_items) {
             const int64_t fine = (int64_t)(h1 / (unsigned long long)want_items);
-            budget = std::min(budget, std::max<int64_t>(128, fine));
+            budget = std::min(budget, std::max<int64_t>(64, fine));
         }
         if (single_segment) budget = INT64_MAX / 4;
         DevBuf<int32_t> nseg, any_multi;
