@@ -284,13 +284,16 @@ __device__ __forceinline__ double drsqrt(double x) {
 // one (target, source) pair costs ~13 DFMA-class instructions plus a double-precision rsqrt (MUFU.RSQ64H + Newton steps), so a
 // source (one 32-byte (x, y, z, q) record) is simply read from `pq` through L1 -- eight lanes of a slice read the same address --
 // and no shared-memory staging is needed: 2 loads against ~90 FP64 instructions per source and lane.
-template <int TPT, bool WF>
-__global__ void __launch_bounds__(PW * 32) p2p_warp64_k(const double4* __restrict__ pq, const double4* __restrict__ pq_s,
+// PW64 warps per CTA: this kernel leans on L1 / L2 for its sources, and neighbouring work items (neighbouring leaves) read the same ones.
+// One warp per CTA (see PW) wins while the particles fit the L2 and leaves are small (N = 1M, leaves of 30: 1.43 -> 1.39 ms); four warps
+// keep neighbours on one SM and win otherwise (N = 1e7, leaves of 19: 5.36 against 5.66 ms; leaves of 256 at N = 2^20: 79 against 90 ms).
+template <int TPT, bool WF, int PW64>
+__global__ void __launch_bounds__(PW64 * 32, PW64 == 4 ? 4 : 1) p2p_warp64_k(const double4* __restrict__ pq, const double4* __restrict__ pq_s,
                                                         const int32_t* __restrict__ sleaf_start, const int32_t* __restrict__ sleaf_cnt,
                                                         const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
                                                         double4* __restrict__ near, int64_t n_items, int nchunk) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t item = (int64_t)blockIdx.x * PW + warp;
+    const int64_t item = (int64_t)blockIdx.x * PW64 + warp;
     if (item >= n_items) return;
     const int64_t iw = item / nchunk;
     const int chunk = (int)(item - iw * nchunk);
@@ -420,11 +423,16 @@ static void p2p_launch64_t(const Plan& P, cudaStream_t st, bool wf, int64_t item
     const int64_t n_items = (item1 - item0) * nchunk;
     if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
-    const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
-    if (wf) p2p_warp64_k<TPT, true><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
-                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
-    else p2p_warp64_k<TPT, false><<<grid, PW * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
-                                                reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+    auto go = [&](auto pwc) {
+        constexpr int PW64 = decltype(pwc)::value;
+        const unsigned grid = (unsigned)((n_items + PW64 - 1) / PW64);
+        if (wf) p2p_warp64_k<TPT, true, PW64><<<grid, PW64 * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
+                                                    reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+        else p2p_warp64_k<TPT, false, PW64><<<grid, PW64 * 32, 0, st>>>((const double4*)P.pq.p, (const double4*)PS.pq.p, PS.box_start.p + sleaf0, PS.box_count.p + sleaf0,
+                                                    reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, (double4*)P.near.p, n_items, nchunk);
+    };
+    if (PS.N <= 3000000 && P.max_leaf <= 128) go(std::integral_constant<int, 1>{});
+    else go(std::integral_constant<int, 4>{});
 }
 
 void p2p_fast64_launch(const Plan& P, cudaStream_t st, bool wf, int64_t i0, int64_t i1) {
