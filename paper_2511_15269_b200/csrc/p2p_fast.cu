@@ -53,9 +53,10 @@ __device__ __forceinline__ float rsq(float x) {
     return r;
 }
 
-// warps per CTA (independent of one another).  One: a CTA's resources are held until its slowest warp is done and the items differ (a leaf has
-// 8-27 strong-list entries); measured on B200, P2P of config 2: 4 warps 0.480 ms, 2: 0.477, 1: 0.463 ms; config 4: 0.451 -> 0.405 ms
-constexpr int PW = 1;
+// PW = warps per CTA (independent of one another).  One: a CTA's resources are held until its slowest warp is done and the items differ (a leaf has
+// 8-27 strong-list entries); measured on B200, P2P of config 2: 4 warps 0.480 ms, 2: 0.477, 1: 0.463 ms; config 4: 0.451 -> 0.405 ms.  Leaves of
+// more than 128 particles keep four warps per CTA: their items are long, and neighbours on one SM share the staged sources' L2 lines
+// (N = 1e7, leaves of 488: 38.8 against 42.5 ms).
 constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two tiles per warp = 8 KB of shared memory
 
 // Source particles come from `srcg`: per leaf a block of G groups; group = 16 floats (-x[4], -y[4], -z[4], q[4]); slots beyond
@@ -63,7 +64,7 @@ constexpr int TG = 64;  // groups (of four sources, 64 bytes) per warp tile; two
 // WF = false: potential only (fmm_evaluate with d_field == NULL): 7 instead of 13 packed instructions per two pairs
 // ZT = true: tiles without a touching leaf pair skip the zero-distance mask (pays for leaves of >~ 32 particles; with small
 // leaves every tile holds the target leaf itself)
-template <int TPT, int HS, bool WF, bool ZT>
+template <int TPT, int HS, bool WF, bool ZT, int PW = 1>
 __global__ void __launch_bounds__(PW * 32) p2p_fast_k(const float4* __restrict__ pq, const float* __restrict__ srcg, int G,
                                                       const int32_t* __restrict__ leaf_start, const int32_t* __restrict__ leaf_cnt,
                                                       const P2PItem* __restrict__ items, const int32_t* __restrict__ strong_src,
@@ -285,7 +286,7 @@ __device__ __forceinline__ double drsqrt(double x) {
 // source (one 32-byte (x, y, z, q) record) is simply read from `pq` through L1 -- eight lanes of a slice read the same address --
 // and no shared-memory staging is needed: 2 loads against ~90 FP64 instructions per source and lane.
 // PW64 warps per CTA: this kernel leans on L1 / L2 for its sources, and neighbouring work items (neighbouring leaves) read the same ones.
-// One warp per CTA (see PW) wins while the particles fit the L2 and leaves are small (N = 1M, leaves of 30: 1.43 -> 1.39 ms); four warps
+// One warp per CTA (see p2p_fast_k) wins while the particles fit the L2 and leaves are small (N = 1M, leaves of 30: 1.43 -> 1.39 ms); four warps
 // keep neighbours on one SM and win otherwise (N = 1e7, leaves of 19: 5.36 against 5.66 ms; leaves of 256 at N = 2^20: 79 against 90 ms).
 template <int TPT, bool WF, int PW64>
 __global__ void __launch_bounds__(PW64 * 32, PW64 == 4 ? 4 : 1) p2p_warp64_k(const double4* __restrict__ pq, const double4* __restrict__ pq_s,
@@ -375,12 +376,17 @@ static void p2p_launch_t(const Plan& P, cudaStream_t st, bool wf, int64_t item0,
     // separate targets: a target leaf may have an empty strong list and then no work item; its near field must read zero
     if (P.p2p_multi || P.S) FMM_CUDA_CHECK(cudaMemsetAsync(P.near.p, 0, P.near.n, st));
     if (n_items == 0) return;
-    const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
     const Plan& PS = P.S ? *P.S : P;  // hierarchy of the sources (separate targets)
-    if (wf) p2p_fast_k<TPT, HS, true, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
-    else p2p_fast_k<TPT, HS, false, (TPT > 2)><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
-                                              reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+    auto go = [&](auto pwc) {
+        constexpr int PW = decltype(pwc)::value;
+        const unsigned grid = (unsigned)((n_items + PW - 1) / PW);
+        if (wf) p2p_fast_k<TPT, HS, true, (TPT > 2), PW><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+                                                  reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+        else p2p_fast_k<TPT, HS, false, (TPT > 2), PW><<<grid, PW * 32, 0, st>>>((const float4*)P.pq.p, (const float*)PS.srcg.p, PS.src_G, P.box_start.p + leaf0, PS.box_count.p + PS.level_off[PS.L],
+                                                  reinterpret_cast<const P2PItem*>(P.p2p_items.p) + item0, P.strong_src.p, P.strong_touch.p, (float4*)P.near.p, n_items, nchunk);
+    };
+    if (P.max_leaf <= 128) go(std::integral_constant<int, 1>{});
+    else go(std::integral_constant<int, 4>{});
 }
 
 // Targets per lane.  A median-split tree gives every leaf the same population (+-1), so max_leaf decides the lane layout for
